@@ -1,0 +1,145 @@
+/*
+ * corr.h -- C ABI of libcorr.so: the X-engine of an FX software correlator on NVIDIA B200 (sm_100a).
+ *
+ * What it computes (Wang & Harris, arXiv:1305.5639; Sec. 2, Eq. 2):
+ *
+ *     V_ij[c] = sum_{t=0}^{T-1} conj(x_i[t][c]) * x_j[t][c]
+ *
+ * for every frequency channel c, every station pair i >= j INCLUDING the autocorrelations i == j
+ * ("triangle pattern for all non-redundant pairs", Sec. 4; autocorrelations on the
+ * hypotenuse, Sec. 4.2) and all P x P polarisation products, as raw sums (Eq. 2 has
+ * no normalisation), optionally integrated across successive calls ("results are usually then
+ * accumulated", Sec. 2).
+ *
+ * Every function is extern "C", never throws and never aborts.  Pointers are plain; each
+ * argument says whether it is a HOST or a DEVICE pointer.  The library links only the CUDA
+ * runtime; callers may use anything (e.g. PyTorch) for device memory and streams.
+ *
+ * Layouts (C-contiguous, fastest axis last)
+ *   in   [n_time][n_chan][n_station][n_pol] complex, (re, im) interleaved:
+ *          CORR_CI8  : 2 x int8  per sample (2 bytes);  any value in [-128, 127] is exact
+ *          CORR_CF16 : 2 x IEEE binary16 per sample (4 bytes); values must be finite
+ *   out  [n_chan][B][n_pol][n_pol] complex, (re, im) interleaved, B = n_station(n_station+1)/2:
+ *          CORR_CI8  : 2 x int32 (8 bytes per visibility), exact
+ *          CORR_CF16 : 2 x fp32  (8 bytes per visibility), fp32 accumulation
+ *        baseline b(i,j) = i(i+1)/2 + j for j <= i (corr_baseline_index); the first polarisation
+ *        axis p belongs to the conjugated station i, the second (q) to station j.  Autocorrelation
+ *        rows keep all P x P products, so V_ii^{XY} and V_ii^{YX} = conj(V_ii^{XY}) are both stored.
+ *
+ * Threading: one handle is used from one host thread at a time; handles are independent.
+ */
+#ifndef CORR_H_
+#define CORR_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct corr_plan* corr_handle;
+
+/* dtype */
+enum { CORR_CI8 = 0, CORR_CF16 = 1 };
+
+/* return codes */
+enum {
+    CORR_OK = 0,
+    CORR_EINVAL = -1,        /* bad argument (size, NULL pointer, alignment, unknown enum)       */
+    CORR_EUNSUPPORTED = -2,  /* no CUDA device, or the device is not compute capability 10.x     */
+    CORR_ENOMEM = -3,        /* host or device allocation failed                                 */
+    CORR_ECUDA = -4,         /* a CUDA call failed; corr_last_error() carries the CUDA string    */
+    CORR_EOVERFLOW = -5      /* CORR_CI8: integration would exceed the exact int32 range         */
+};
+
+/* operand feeder of the tensor-core kernel (corr_set_feed) */
+enum {
+    CORR_FEED_DIRECT = 0,       /* default: TMA reads `in` in place as MN-major operands (no staging)  */
+    CORR_FEED_CORNER_TURN = 1   /* corner-turn kernel -> channel-major, time-inner workspace (K-major) */
+};
+
+/*
+ * corr_create -- plan for one problem geometry on the CURRENT CUDA device (host call).
+ *   n_station >= 1, n_pol in {1, 2}, n_chan >= 1, n_time >= 1, dtype in {CORR_CI8, CORR_CF16}.
+ * Builds the triangular tile schedule (only tiles touching s_i >= s_j are scheduled), uploads it,
+ * and sizes the workspace.  Returns NULL on failure; the reason is corr_last_error(NULL).
+ * The handle owns its device allocations until corr_destroy.
+ */
+corr_handle corr_create(int n_station, int n_pol, int n_chan, int n_time, int dtype);
+
+/*
+ * corr_xengine -- one integration of n_time samples (Eq. 2), asynchronous on `stream`.
+ *   in         DEVICE pointer, corr_input_bytes(h) bytes, 16-byte aligned, layout above; must stay
+ *              valid and unmodified until `stream` has passed this call.  Not written.
+ *   out        DEVICE pointer, corr_output_bytes(h) bytes, 16-byte aligned, layout above.
+ *              accumulate == 0: every word is overwritten (no pre-zeroing needed).
+ *              accumulate != 0: out <- out + V; `out` must hold an earlier result of the same geometry.
+ *   stream     a cudaStream_t passed as void* (NULL = the legacy default stream).
+ * Returns CORR_OK or a negative code.  CORR_CI8 with accumulate != 0 returns CORR_EOVERFLOW,
+ * launching nothing, once the samples integrated through this handle since the last accumulate == 0
+ * call would exceed 65535 (|V| <= 2 * 128^2 * T_total must fit int32).
+ */
+int corr_xengine(corr_handle h, const void* in, void* out, int accumulate, void* stream);
+
+/*
+ * corr_xengine_host -- same operation with HOST buffers (blocking): copies `in_host` to a device
+ * staging buffer owned by the handle, runs corr_xengine on the handle's own stream, copies the
+ * result to `out_host` and synchronises.  With accumulate != 0 the running sum lives in the
+ * handle's device staging buffer (state of the previous corr_xengine_host call on this handle) and
+ * `out_host` receives the updated integration.  Pinned host memory makes the copies DMA directly.
+ */
+int corr_xengine_host(corr_handle h, const void* in_host, void* out_host, int accumulate);
+
+/* corr_destroy -- frees the handle and everything it owns.  NULL is a no-op. */
+void corr_destroy(corr_handle h);
+
+/* ---- helpers ------------------------------------------------------------------------------ */
+
+size_t corr_input_bytes(corr_handle h);      /* T*C*N*P * (2 or 4); 0 for NULL                  */
+size_t corr_output_bytes(corr_handle h);     /* C*B*P*P * 8;        0 for NULL                  */
+long long corr_baseline_index(int i, int j); /* i(i+1)/2 + j for 0 <= j <= i, else -1           */
+
+/* Message of the last failure on this handle (or, for NULL, of the last failed corr_create on this
+ * thread).  The string is owned by the library and valid until the next call on the same handle. */
+const char* corr_last_error(corr_handle h);
+
+/* Choose the operand feeder for subsequent corr_xengine calls (see enum above).  The corner-turn
+ * feeder allocates its workspace (corr_workspace_bytes) on first use. */
+int corr_set_feed(corr_handle h, int feed);
+int corr_get_feed(corr_handle h);
+
+/* Which kernel corr_xengine will launch for this geometry: 1 = tcgen05 tensor-core kernel,
+ * 0 = SIMT kernel (geometries whose input row pitch C*N*P*sample_bytes is not a multiple of 16,
+ * which TMA cannot address). */
+int corr_uses_tensor_cores(corr_handle h);
+
+/*
+ * Corner turn (pre-X-engine data re-ordering; the GPU analogue of the paper's "indexing ... for
+ * optimizing the GPU memory access"):
+ *     ws    [c][m][t] = in[t][c][m]            (m = s*n_pol + p, complex kept interleaved)
+ *     ws_rot[c][m][t] = (im, -re) of the same sample           (feeds the imaginary part)
+ * with the time axis padded to corr_workspace_time(h) samples (zero filled).
+ *   in      DEVICE pointer as for corr_xengine.
+ *   ws      DEVICE pointer, corr_workspace_bytes(h) bytes, 1024-byte aligned: the two planes,
+ *           ws then ws_rot, each n_chan * M * corr_workspace_time(h) samples.
+ * Asynchronous on `stream`.  corr_xengine with CORR_FEED_CORNER_TURN runs this internally.
+ */
+int corr_corner_turn(corr_handle h, const void* in, void* ws, void* stream);
+size_t corr_workspace_bytes(corr_handle h);
+int corr_workspace_time(corr_handle h);
+
+/*
+ * Introspection of the triangular tile schedule (host logic, no GPU work): writes up to `max_tiles`
+ * entries of {row0, col0, ncols} (units: real components u = 2*m + {re:0, im:1} within a channel,
+ * rows = conjugated side) for ONE channel and returns the number of tiles per channel.
+ * Usable without a handle or a GPU.  `feed` selects the feeder whose schedule is reported.
+ */
+int corr_tile_schedule(int n_station, int n_pol, int dtype, int feed, int* tiles3, int max_tiles);
+
+/* Number of kernels launched by the last corr_xengine / corr_xengine_host call on this handle. */
+int corr_last_launch_count(corr_handle h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CORR_H_ */

@@ -1,0 +1,202 @@
+"""Thin ctypes binding of libcorr.so (include/corr.h): argument marshalling only.
+
+Every step of the X-engine (Eq. 2) runs inside the library's CUDA kernels.  torch is
+used by callers for device memory and streams; this module only extracts ``data_ptr()`` and the raw
+``cudaStream_t``.  There is NO CPU fallback: if the library is missing or the device is not a B200,
+the calls raise.
+"""
+import ctypes
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libcorr.so")
+
+CORR_CI8, CORR_CF16 = 0, 1
+CORR_OK, CORR_EINVAL, CORR_EUNSUPPORTED, CORR_ENOMEM, CORR_ECUDA, CORR_EOVERFLOW = 0, -1, -2, -3, -4, -5
+CORR_FEED_DIRECT, CORR_FEED_CORNER_TURN = 0, 1
+DTYPES = {"ci8": CORR_CI8, "cf16": CORR_CF16}
+
+# name -> (restype, argtypes): every symbol include/corr.h declares
+_vp, _i, _sz, _ll, _cp = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t, ctypes.c_longlong, ctypes.c_char_p
+SYMBOLS = {
+    "corr_create": (_vp, [_i, _i, _i, _i, _i]),
+    "corr_xengine": (_i, [_vp, _vp, _vp, _i, _vp]),
+    "corr_xengine_host": (_i, [_vp, _vp, _vp, _i]),
+    "corr_destroy": (None, [_vp]),
+    "corr_input_bytes": (_sz, [_vp]),
+    "corr_output_bytes": (_sz, [_vp]),
+    "corr_baseline_index": (_ll, [_i, _i]),
+    "corr_last_error": (_cp, [_vp]),
+    "corr_set_feed": (_i, [_vp, _i]),
+    "corr_get_feed": (_i, [_vp]),
+    "corr_uses_tensor_cores": (_i, [_vp]),
+    "corr_corner_turn": (_i, [_vp, _vp, _vp, _vp]),
+    "corr_workspace_bytes": (_sz, [_vp]),
+    "corr_workspace_time": (_i, [_vp]),
+    "corr_tile_schedule": (_i, [_i, _i, _i, _i, ctypes.POINTER(_i), _i]),
+    "corr_last_launch_count": (_i, [_vp]),
+}
+
+_lib = None
+
+
+class CorrError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("libcorr error %d: %s" % (code, msg))
+        self.code = code
+
+
+def lib():
+    """Load libcorr.so (building it in-tree if the sources are newer).  Raises if unavailable."""
+    global _lib
+    if _lib is None:
+        from .build import build
+        build()                       # no-op when libcorr.so is newer than its sources
+        L = ctypes.CDLL(LIB_PATH)
+        for name, (res, args) in SYMBOLS.items():
+            f = getattr(L, name)      # AttributeError if the library does not export it
+            f.restype, f.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def baseline_index(i, j):
+    return int(lib().corr_baseline_index(int(i), int(j)))
+
+
+def tile_schedule(n_station, n_pol, dtype="ci8", feed=CORR_FEED_DIRECT):
+    """Per-channel triangular tile schedule as a list of (row0, col0, ncols); host logic only."""
+    L = lib()
+    n = L.corr_tile_schedule(n_station, n_pol, DTYPES[dtype], feed, None, 0)
+    if n < 0:
+        raise CorrError(n, "corr_tile_schedule")
+    buf = (_i * (3 * n))()
+    L.corr_tile_schedule(n_station, n_pol, DTYPES[dtype], feed, buf, n)
+    return [(buf[3 * k], buf[3 * k + 1], buf[3 * k + 2]) for k in range(n)]
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(getattr(stream, "cuda_stream", stream))
+
+
+class Correlator:
+    """corr_create / corr_xengine / corr_destroy with torch tensors as the device buffers."""
+
+    def __init__(self, n_station, n_pol, n_chan, n_time, dtype="ci8"):
+        self._L = lib()
+        self.N, self.P, self.C, self.T, self.dtype = n_station, n_pol, n_chan, n_time, dtype
+        self._h = self._L.corr_create(n_station, n_pol, n_chan, n_time, DTYPES[dtype])
+        if not self._h:
+            msg = self._L.corr_last_error(None).decode()
+            raise CorrError(CORR_EINVAL if "invalid" in msg or "too large" in msg else CORR_EUNSUPPORTED, msg)
+        self.n_baseline = n_station * (n_station + 1) // 2
+
+    # ---- sizes / introspection -------------------------------------------------------------
+    @property
+    def input_bytes(self):
+        return int(self._L.corr_input_bytes(self._h))
+
+    @property
+    def output_bytes(self):
+        return int(self._L.corr_output_bytes(self._h))
+
+    @property
+    def workspace_bytes(self):
+        return int(self._L.corr_workspace_bytes(self._h))
+
+    @property
+    def workspace_time(self):
+        return int(self._L.corr_workspace_time(self._h))
+
+    @property
+    def uses_tensor_cores(self):
+        return bool(self._L.corr_uses_tensor_cores(self._h))
+
+    @property
+    def last_launch_count(self):
+        return int(self._L.corr_last_launch_count(self._h))
+
+    def set_feed(self, feed):
+        self._check(self._L.corr_set_feed(self._h, int(feed)))
+
+    def _check(self, rc):
+        if rc != CORR_OK:
+            raise CorrError(rc, self._L.corr_last_error(self._h).decode())
+
+    # ---- buffers ---------------------------------------------------------------------------
+    def input_shape(self):
+        return (self.T, self.C, self.N, self.P, 2)
+
+    def output_shape(self):
+        return (self.C, self.n_baseline, self.P, self.P, 2)
+
+    def empty_output(self, device="cuda"):
+        import torch
+        return torch.empty(self.output_shape(), device=device,
+                           dtype=torch.int32 if self.dtype == "ci8" else torch.float32)
+
+    def _check_in(self, x, device_type):
+        import torch
+        want = torch.int8 if self.dtype == "ci8" else torch.float16
+        if x.dtype != want or tuple(x.shape) != self.input_shape() or not x.is_contiguous():
+            raise ValueError("input must be a contiguous %s tensor of shape %s" % (want, self.input_shape()))
+        if x.device.type != device_type:
+            raise ValueError("input must live on %s" % device_type)
+
+    def _check_out(self, out, device_type):
+        import torch
+        want = torch.int32 if self.dtype == "ci8" else torch.float32
+        if out.dtype != want or tuple(out.shape) != self.output_shape() or not out.is_contiguous():
+            raise ValueError("output must be a contiguous %s tensor of shape %s" % (want, self.output_shape()))
+        if out.device.type != device_type:
+            raise ValueError("output must live on %s" % device_type)
+
+    # ---- the calls -------------------------------------------------------------------------
+    def xengine(self, x, out=None, accumulate=False, stream=None):
+        """corr_xengine on device tensors; asynchronous on ``stream`` (default: torch's current)."""
+        self._check_in(x, "cuda")
+        if out is None:
+            if accumulate:
+                raise ValueError("accumulate=True needs the running `out`")
+            out = self.empty_output(x.device)
+        self._check_out(out, "cuda")
+        self._check(self._L.corr_xengine(self._h, x.data_ptr(), out.data_ptr(), int(bool(accumulate)),
+                                         _stream_ptr(stream)))
+        return out
+
+    def xengine_host(self, x_host, out_host, accumulate=False):
+        """corr_xengine_host: HOST tensors in and out (blocking; copies inside the library)."""
+        self._check_in(x_host, "cpu")
+        self._check_out(out_host, "cpu")
+        self._check(self._L.corr_xengine_host(self._h, x_host.data_ptr(), out_host.data_ptr(),
+                                              int(bool(accumulate))))
+        return out_host
+
+    def corner_turn(self, x, ws=None, stream=None):
+        """corr_corner_turn: returns the uint8 workspace holding the planes ws, ws_rot."""
+        import torch
+        self._check_in(x, "cuda")
+        if ws is None:
+            ws = torch.empty((self.workspace_bytes,), dtype=torch.uint8, device=x.device)
+        self._check(self._L.corr_corner_turn(self._h, x.data_ptr(), ws.data_ptr(), _stream_ptr(stream)))
+        return ws
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.corr_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()

@@ -1,0 +1,409 @@
+// corr.cu -- libcorr.so: C ABI (include/corr.h), plan / tile schedule / launch logic.
+// The device code lives in xengine_tc.cuh (tcgen05 HERK + packed writer + accumulate),
+// corner_turn.cuh (piece a) and xengine_simt.cuh (geometries TMA cannot address).
+#include "../../include/corr.h"
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <cstdarg>
+#include <cstdint>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "corner_turn.cuh"
+#include "xengine_simt.cuh"
+#include "xengine_tc.cuh"
+
+namespace {
+
+constexpr long long kMaxIntegrationCi8 = 65535;   // 2 * 128^2 * T_total <= 2^31 - 1
+
+thread_local char g_create_error[512] = "";
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+}  // namespace
+
+struct corr_plan {
+    int N, P, C, T, dtype;
+    int M;                 // N * P
+    long long B;           // N (N + 1) / 2
+    int sample_bytes;      // 2 (ci8) or 4 (cf16)
+    int device;
+    int sm_count;
+    int feed;
+    bool tma_ok;           // input row pitch is a multiple of 16 bytes
+    long long t_total;     // samples integrated since the last accumulate == 0 call
+    int last_launches;
+
+    std::vector<xtc::TileDesc> h_tiles;
+    xtc::TileDesc* d_tiles;
+    EncodeTiledFn encode;
+
+    CUtensorMap tmap_in;
+    const void* tmap_in_ptr;
+
+    // corner-turn feed
+    int Tp;                // padded time extent of the workspace
+    void* d_ws;            // owned workspace (lazy)
+
+    // corr_xengine_host staging
+    void* d_in_stage;
+    void* d_out_stage;
+    cudaStream_t own_stream;
+
+    char err[512];
+};
+
+namespace {
+
+int fail(corr_plan* h, int code, const char* fmt, ...) {
+    char* dst = h ? h->err : g_create_error;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(dst, 512, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+int fail_cuda(corr_plan* h, cudaError_t e, const char* what) {
+    return fail(h, CORR_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+bool valid_geometry(int N, int P, int dtype) {
+    return N >= 1 && (P == 1 || P == 2) && (dtype == CORR_CI8 || dtype == CORR_CF16);
+}
+
+// Triangular tile schedule of ONE channel for the direct feed, in real components u = 2m + {re, im}.
+// Row block r covers u in [128 r, 128 r + 128); only columns up to the last station of the row block
+// are needed (s_j <= s_i), cut into column blocks of 256.
+void build_schedule_direct(int N, int P, std::vector<xtc::TileDesc>& v) {
+    v.clear();
+    const int M2 = 2 * N * P;
+    for (int row0 = 0; row0 < M2; row0 += xtc::kTileRows) {
+        const int row_end = (row0 + xtc::kTileRows < M2) ? row0 + xtc::kTileRows : M2;   // exclusive
+        const int i_max = ((row_end - 1) / 2) / P;                                      // last station in the block
+        const int need = (i_max + 1) * P * 2;                                           // columns u < need
+        for (int col0 = 0; col0 < need; col0 += xtc::kTileCols) {
+            int ncols = need - col0;
+            if (ncols > xtc::kTileCols) ncols = xtc::kTileCols;
+            ncols = (ncols + 15) & ~15;
+            v.push_back(xtc::TileDesc{row0, col0, ncols, 0});
+        }
+    }
+}
+
+size_t input_bytes(const corr_plan* h) {
+    return static_cast<size_t>(h->T) * h->C * h->M * h->sample_bytes;
+}
+size_t output_bytes(const corr_plan* h) {
+    return static_cast<size_t>(h->C) * h->B * h->P * h->P * 8;
+}
+size_t workspace_bytes(const corr_plan* h) {
+    return 2 * static_cast<size_t>(h->C) * h->M * h->Tp * h->sample_bytes;
+}
+
+int encode_input_map(corr_plan* h, const void* in) {
+    if (h->tmap_in_ptr == in) return CORR_OK;
+    const int elt = h->sample_bytes / 2;                       // bytes per real component
+    const cuuint64_t W = static_cast<cuuint64_t>(h->C) * 2 * h->M;
+    cuuint64_t dims[2] = {W, static_cast<cuuint64_t>(h->T)};
+    cuuint64_t strides[1] = {W * elt};
+    cuuint32_t box[2] = {static_cast<cuuint32_t>(128 / elt),
+                         static_cast<cuuint32_t>(elt == 1 ? xtc::Cfg<1>::kKStage : xtc::Cfg<2>::kKStage)};
+    cuuint32_t estr[2] = {1, 1};
+    const CUresult r = h->encode(&h->tmap_in, elt == 1 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16,
+                                 2, const_cast<void*>(in), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                 CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        h->tmap_in_ptr = nullptr;
+        return fail(h, CORR_ECUDA, "cuTensorMapEncodeTiled(in) failed with CUresult %d", static_cast<int>(r));
+    }
+    h->tmap_in_ptr = in;
+    return CORR_OK;
+}
+
+int launch_direct(corr_plan* h, const void* in, void* out, int accumulate, cudaStream_t st) {
+    int rc = encode_input_map(h, in);
+    if (rc != CORR_OK) return rc;
+    xtc::Params prm;
+    prm.tiles = h->d_tiles;
+    prm.tiles_per_chan = static_cast<int>(h->h_tiles.size());
+    prm.n_tiles = static_cast<long long>(h->h_tiles.size()) * h->C;
+    prm.n_station = h->N;
+    prm.n_pol = h->P;
+    prm.n_chan = h->C;
+    prm.n_time = h->T;
+    prm.M = h->M;
+    prm.n_baseline = h->B;
+    prm.out = out;
+    prm.accumulate = accumulate ? 1 : 0;
+    const long long grid = prm.n_tiles < h->sm_count ? prm.n_tiles : h->sm_count;
+    if (h->dtype == CORR_CI8)
+        xtc::xengine_direct_kernel<1><<<static_cast<unsigned>(grid), xtc::kNumThreads, xtc::kSmemBytes, st>>>(h->tmap_in, prm);
+    else
+        xtc::xengine_direct_kernel<2><<<static_cast<unsigned>(grid), xtc::kNumThreads, xtc::kSmemBytes, st>>>(h->tmap_in, prm);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(h, e, "xengine_direct_kernel launch");
+    h->last_launches += 1;
+    return CORR_OK;
+}
+
+int launch_simt(corr_plan* h, const void* in, void* out, int accumulate, cudaStream_t st) {
+    xsimt::Params prm;
+    prm.in = in;
+    prm.out = out;
+    prm.n_station = h->N;
+    prm.n_pol = h->P;
+    prm.n_chan = h->C;
+    prm.n_time = h->T;
+    prm.n_baseline = h->B;
+    prm.n_vis = static_cast<long long>(h->C) * h->B * h->P * h->P;
+    prm.accumulate = accumulate ? 1 : 0;
+    long long blocks = (prm.n_vis + 127) / 128;
+    const long long cap = static_cast<long long>(h->sm_count) * 16;
+    if (blocks > cap) blocks = cap;
+    if (h->dtype == CORR_CI8)
+        xsimt::xengine_simt_kernel<false><<<static_cast<unsigned>(blocks), 128, 0, st>>>(prm);
+    else
+        xsimt::xengine_simt_kernel<true><<<static_cast<unsigned>(blocks), 128, 0, st>>>(prm);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(h, e, "xengine_simt_kernel launch");
+    h->last_launches += 1;
+    return CORR_OK;
+}
+
+int launch_corner_turn(corr_plan* h, const void* in, void* ws, cudaStream_t st) {
+    cturn::Params prm;
+    prm.in = in;
+    prm.ws = ws;
+    prm.ws_rot = static_cast<uint8_t*>(ws) + workspace_bytes(h) / 2;
+    prm.n_cm = static_cast<long long>(h->C) * h->M;
+    prm.n_time = h->T;
+    prm.n_time_pad = h->Tp;
+    const unsigned gx = static_cast<unsigned>((prm.n_cm + cturn::kTileCm - 1) / cturn::kTileCm);
+    if (h->dtype == CORR_CI8) {
+        dim3 grid(gx, static_cast<unsigned>(h->Tp / 64));
+        cturn::corner_turn_kernel<2><<<grid, cturn::kThreads, 0, st>>>(prm);
+    } else {
+        dim3 grid(gx, static_cast<unsigned>(h->Tp / 32));
+        cturn::corner_turn_kernel<4><<<grid, cturn::kThreads, 0, st>>>(prm);
+    }
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(h, e, "corner_turn_kernel launch");
+    h->last_launches += 1;
+    return CORR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+long long corr_baseline_index(int i, int j) {
+    if (j < 0 || j > i) return -1;
+    return static_cast<long long>(i) * (i + 1) / 2 + j;
+}
+
+int corr_tile_schedule(int n_station, int n_pol, int dtype, int feed, int* tiles3, int max_tiles) {
+    if (!valid_geometry(n_station, n_pol, dtype) || max_tiles < 0 || (max_tiles > 0 && !tiles3)) return CORR_EINVAL;
+    if (feed != CORR_FEED_DIRECT) return CORR_EUNSUPPORTED;
+    std::vector<xtc::TileDesc> v;
+    build_schedule_direct(n_station, n_pol, v);
+    for (size_t k = 0; k < v.size() && static_cast<int>(k) < max_tiles; ++k) {
+        tiles3[3 * k + 0] = v[k].row0;
+        tiles3[3 * k + 1] = v[k].col0;
+        tiles3[3 * k + 2] = v[k].ncols;
+    }
+    return static_cast<int>(v.size());
+}
+
+corr_handle corr_create(int n_station, int n_pol, int n_chan, int n_time, int dtype) {
+    g_create_error[0] = 0;
+    if (!valid_geometry(n_station, n_pol, dtype) || n_chan < 1 || n_time < 1) {
+        fail(nullptr, CORR_EINVAL, "corr_create: invalid geometry N=%d P=%d C=%d T=%d dtype=%d", n_station, n_pol,
+             n_chan, n_time, dtype);
+        return nullptr;
+    }
+    const long long M = static_cast<long long>(n_station) * n_pol;
+    const long long W = static_cast<long long>(n_chan) * 2 * M;
+    if (M > (1 << 20) || W > (1ll << 31) - 1024 || n_time > (1 << 24)) {
+        fail(nullptr, CORR_EINVAL, "corr_create: geometry too large (N*P=%lld, C*2*N*P=%lld, T=%d)", M, W, n_time);
+        return nullptr;
+    }
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) {
+        fail(nullptr, CORR_EUNSUPPORTED, "corr_create: no usable CUDA device (%s)", cudaGetErrorString(e));
+        return nullptr;
+    }
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, dev);
+    if (e != cudaSuccess) {
+        fail(nullptr, CORR_EUNSUPPORTED, "corr_create: cudaGetDeviceProperties: %s", cudaGetErrorString(e));
+        return nullptr;
+    }
+    if (prop.major != 10) {
+        fail(nullptr, CORR_EUNSUPPORTED, "corr_create: device %d (%s) is sm_%d%d; this library is built for sm_100a only",
+             dev, prop.name, prop.major, prop.minor);
+        return nullptr;
+    }
+    corr_plan* h = new (std::nothrow) corr_plan();
+    if (!h) {
+        fail(nullptr, CORR_ENOMEM, "corr_create: out of host memory");
+        return nullptr;
+    }
+    h->N = n_station;
+    h->P = n_pol;
+    h->C = n_chan;
+    h->T = n_time;
+    h->dtype = dtype;
+    h->M = static_cast<int>(M);
+    h->B = static_cast<long long>(n_station) * (n_station + 1) / 2;
+    h->sample_bytes = dtype == CORR_CI8 ? 2 : 4;
+    h->device = dev;
+    h->sm_count = prop.multiProcessorCount;
+    h->feed = CORR_FEED_DIRECT;
+    h->tma_ok = (static_cast<long long>(n_chan) * M * h->sample_bytes) % 16 == 0;
+    h->t_total = 0;
+    h->last_launches = 0;
+    h->d_tiles = nullptr;
+    h->encode = nullptr;
+    h->tmap_in_ptr = nullptr;
+    h->Tp = (n_time + 63) / 64 * 64;
+    h->d_ws = nullptr;
+    h->d_in_stage = nullptr;
+    h->d_out_stage = nullptr;
+    h->own_stream = nullptr;
+    h->err[0] = 0;
+
+    build_schedule_direct(h->N, h->P, h->h_tiles);
+    e = cudaMalloc(&h->d_tiles, h->h_tiles.size() * sizeof(xtc::TileDesc));
+    if (e == cudaSuccess)
+        e = cudaMemcpy(h->d_tiles, h->h_tiles.data(), h->h_tiles.size() * sizeof(xtc::TileDesc), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+        fail(nullptr, e == cudaErrorMemoryAllocation ? CORR_ENOMEM : CORR_ECUDA, "corr_create: tile table: %s",
+             cudaGetErrorString(e));
+        corr_destroy(h);
+        return nullptr;
+    }
+    if (h->tma_ok) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+        if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn) {
+            fail(nullptr, CORR_ECUDA, "corr_create: cuTensorMapEncodeTiled entry point unavailable (%s)",
+                 cudaGetErrorString(e));
+            corr_destroy(h);
+            return nullptr;
+        }
+        h->encode = reinterpret_cast<EncodeTiledFn>(fn);
+        e = cudaFuncSetAttribute(xtc::xengine_direct_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, xtc::kSmemBytes);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(xtc::xengine_direct_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, xtc::kSmemBytes);
+        if (e != cudaSuccess) {
+            fail(nullptr, CORR_ECUDA, "corr_create: cudaFuncSetAttribute(smem): %s", cudaGetErrorString(e));
+            corr_destroy(h);
+            return nullptr;
+        }
+    }
+    return h;
+}
+
+void corr_destroy(corr_handle h) {
+    if (!h) return;
+    if (h->d_tiles) cudaFree(h->d_tiles);
+    if (h->d_ws) cudaFree(h->d_ws);
+    if (h->d_in_stage) cudaFree(h->d_in_stage);
+    if (h->d_out_stage) cudaFree(h->d_out_stage);
+    if (h->own_stream) cudaStreamDestroy(h->own_stream);
+    delete h;
+}
+
+size_t corr_input_bytes(corr_handle h) { return h ? input_bytes(h) : 0; }
+size_t corr_output_bytes(corr_handle h) { return h ? output_bytes(h) : 0; }
+size_t corr_workspace_bytes(corr_handle h) { return h ? workspace_bytes(h) : 0; }
+int corr_workspace_time(corr_handle h) { return h ? h->Tp : 0; }
+const char* corr_last_error(corr_handle h) { return h ? h->err : g_create_error; }
+int corr_get_feed(corr_handle h) { return h ? h->feed : CORR_EINVAL; }
+int corr_uses_tensor_cores(corr_handle h) { return h ? (h->tma_ok ? 1 : 0) : CORR_EINVAL; }
+int corr_last_launch_count(corr_handle h) { return h ? h->last_launches : CORR_EINVAL; }
+
+int corr_set_feed(corr_handle h, int feed) {
+    if (!h) return CORR_EINVAL;
+    if (feed == CORR_FEED_DIRECT) {
+        h->feed = feed;
+        return CORR_OK;
+    }
+    if (feed == CORR_FEED_CORNER_TURN)
+        return fail(h, CORR_EUNSUPPORTED, "corr_set_feed: the corner-turn feeder of the tensor-core kernel is not built yet");
+    return fail(h, CORR_EINVAL, "corr_set_feed: unknown feed %d", feed);
+}
+
+int corr_corner_turn(corr_handle h, const void* in, void* ws, void* stream) {
+    if (!h) return CORR_EINVAL;
+    if (!in || !ws) return fail(h, CORR_EINVAL, "corr_corner_turn: NULL pointer");
+    if ((reinterpret_cast<uintptr_t>(in) & 15) || (reinterpret_cast<uintptr_t>(ws) & 1023))
+        return fail(h, CORR_EINVAL, "corr_corner_turn: `in` must be 16-byte and `ws` 1024-byte aligned");
+    if (!h->tma_ok)
+        return fail(h, CORR_EUNSUPPORTED, "corr_corner_turn: input row pitch %lld B is not a multiple of 16",
+                    static_cast<long long>(h->C) * h->M * h->sample_bytes);
+    h->last_launches = 0;
+    return launch_corner_turn(h, in, ws, static_cast<cudaStream_t>(stream));
+}
+
+int corr_xengine(corr_handle h, const void* in, void* out, int accumulate, void* stream) {
+    if (!h) return CORR_EINVAL;
+    if (!in || !out) return fail(h, CORR_EINVAL, "corr_xengine: NULL pointer");
+    if ((reinterpret_cast<uintptr_t>(in) & 15) || (reinterpret_cast<uintptr_t>(out) & 15))
+        return fail(h, CORR_EINVAL, "corr_xengine: `in` and `out` must be 16-byte aligned");
+    const long long t_next = accumulate ? h->t_total + h->T : h->T;
+    if (h->dtype == CORR_CI8 && t_next > kMaxIntegrationCi8)
+        return fail(h, CORR_EOVERFLOW, "corr_xengine: integrating %lld samples would overflow int32 (limit %lld)", t_next,
+                    kMaxIntegrationCi8);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    h->last_launches = 0;
+    int rc;
+    if (h->tma_ok && !getenv("CORR_FORCE_SIMT"))
+        rc = launch_direct(h, in, out, accumulate, st);
+    else
+        rc = launch_simt(h, in, out, accumulate, st);
+    if (rc == CORR_OK) h->t_total = t_next;
+    return rc;
+}
+
+int corr_xengine_host(corr_handle h, const void* in_host, void* out_host, int accumulate) {
+    if (!h) return CORR_EINVAL;
+    if (!in_host || !out_host) return fail(h, CORR_EINVAL, "corr_xengine_host: NULL pointer");
+    cudaError_t e;
+    if (!h->own_stream) {
+        e = cudaStreamCreateWithFlags(&h->own_stream, cudaStreamNonBlocking);
+        if (e != cudaSuccess) return fail_cuda(h, e, "cudaStreamCreate");
+    }
+    if (!h->d_in_stage) {
+        e = cudaMalloc(&h->d_in_stage, input_bytes(h));
+        if (e != cudaSuccess) return fail(h, CORR_ENOMEM, "corr_xengine_host: input staging: %s", cudaGetErrorString(e));
+    }
+    if (!h->d_out_stage) {
+        if (accumulate) return fail(h, CORR_EINVAL, "corr_xengine_host: accumulate without a previous call");
+        e = cudaMalloc(&h->d_out_stage, output_bytes(h));
+        if (e != cudaSuccess) return fail(h, CORR_ENOMEM, "corr_xengine_host: output staging: %s", cudaGetErrorString(e));
+    }
+    e = cudaMemcpyAsync(h->d_in_stage, in_host, input_bytes(h), cudaMemcpyHostToDevice, h->own_stream);
+    if (e != cudaSuccess) return fail_cuda(h, e, "H2D copy");
+    const int rc = corr_xengine(h, h->d_in_stage, h->d_out_stage, accumulate, h->own_stream);
+    if (rc != CORR_OK) return rc;
+    e = cudaMemcpyAsync(out_host, h->d_out_stage, output_bytes(h), cudaMemcpyDeviceToHost, h->own_stream);
+    if (e != cudaSuccess) return fail_cuda(h, e, "D2H copy");
+    e = cudaStreamSynchronize(h->own_stream);
+    if (e != cudaSuccess) return fail_cuda(h, e, "corr_xengine_host: stream synchronize");
+    return CORR_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,73 @@
+// xengine_simt.cuh -- plain CUDA-core X-engine for geometries TMA cannot address (input row pitch
+// C*N*P*sample_bytes not a multiple of 16 bytes).  One thread per stored visibility, Eq. 2
+// evaluated term by term.  Not a performance path.
+#pragma once
+#include <cuda_fp16.h>
+#include <cstdint>
+
+namespace xsimt {
+
+struct Params {
+    const void* in;
+    void* out;
+    int n_station, n_pol, n_chan, n_time;
+    long long n_baseline;
+    long long n_vis;     // n_chan * n_baseline * n_pol * n_pol
+    int accumulate;
+};
+
+__device__ __forceinline__ void decode_baseline(long long b, int& i, int& j) {
+    // largest i with i(i+1)/2 <= b
+    long long r = static_cast<long long>((sqrt(8.0 * static_cast<double>(b) + 1.0) - 1.0) * 0.5);
+    while (r * (r + 1) / 2 > b) --r;
+    while ((r + 1) * (r + 2) / 2 <= b) ++r;
+    i = static_cast<int>(r);
+    j = static_cast<int>(b - r * (r + 1) / 2);
+}
+
+template <bool kFloat>
+__global__ void xengine_simt_kernel(const Params prm) {
+    const int P = prm.n_pol, N = prm.n_station, C = prm.n_chan;
+    for (long long v = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; v < prm.n_vis;
+         v += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const int q = static_cast<int>(v % P);
+        const int p = static_cast<int>((v / P) % P);
+        const long long cb = v / (P * P);
+        const long long b = cb % prm.n_baseline;
+        const int c = static_cast<int>(cb / prm.n_baseline);
+        int i, j;
+        decode_baseline(b, i, j);
+        const long long pitch = static_cast<long long>(C) * N * P;          // samples per time step
+        const long long ia = (static_cast<long long>(c) * N + i) * P + p;
+        const long long ib = (static_cast<long long>(c) * N + j) * P + q;
+        if constexpr (kFloat) {
+            const __half2* x = static_cast<const __half2*>(prm.in);
+            double re = 0.0, im = 0.0;
+            for (int t = 0; t < prm.n_time; ++t) {
+                const float2 a = __half22float2(x[t * pitch + ia]);
+                const float2 bb = __half22float2(x[t * pitch + ib]);
+                re += static_cast<double>(a.x) * bb.x + static_cast<double>(a.y) * bb.y;
+                im += static_cast<double>(a.x) * bb.y - static_cast<double>(a.y) * bb.x;
+            }
+            float2* o = static_cast<float2*>(prm.out) + v;
+            float2 r = make_float2(static_cast<float>(re), static_cast<float>(im));
+            if (prm.accumulate) { r.x += o->x; r.y += o->y; }
+            *o = r;
+        } else {
+            const char2* x = static_cast<const char2*>(prm.in);
+            int re = 0, im = 0;
+            for (int t = 0; t < prm.n_time; ++t) {
+                const char2 a = x[t * pitch + ia];
+                const char2 bb = x[t * pitch + ib];
+                re += a.x * bb.x + a.y * bb.y;
+                im += a.x * bb.y - a.y * bb.x;
+            }
+            int2* o = static_cast<int2*>(prm.out) + v;
+            int2 r = make_int2(re, im);
+            if (prm.accumulate) { r.x += o->x; r.y += o->y; }
+            *o = r;
+        }
+    }
+}
+
+}  // namespace xsimt

@@ -1,0 +1,264 @@
+// xengine_tc.cuh -- the X-engine as a per-channel Hermitian rank-T update on tcgen05 tensor cores.
+//
+// Computes PAPER.md:54-57 (Sec. 2, Eq. 2)  V_ij[c] = sum_t conj(x_i[t][c]) x_j[t][c]  for the lower
+// station triangle incl. autocorrelations and writes the packed-baseline output.
+//
+// DIRECT feed ("Gram of components"): for a fixed channel the input is a real matrix
+// Y[t][u], u = 2*m + {0: re, 1: im}, m = s*P + p, contiguous in u.  The real Gram matrix
+// G = Y^T Y (contraction over time) holds every product Eq. 2 needs:
+//     Re V_mn = G[2m][2n]   + G[2m+1][2n+1]
+//     Im V_mn = G[2m][2n+1] - G[2m+1][2n]                       (conj on the first index m)
+// Both MMA operands are MN-major (u contiguous, K = time strided), so TMA boxes
+// [KSTAGE time rows] x [128 bytes of u] are cut straight out of in[t][c][s][p] -- no corner turn,
+// no staging copy.  One CTA tile is 128 rows (u) x up to 256 columns (u) of G for one channel;
+// the accumulator lives in TMEM (256 columns, double buffered), and the epilogue forms Re/Im with
+// one shuffle between adjacent TMEM lanes and streams the packed triangle to HBM.
+//
+// Warp roles (192 threads, 1 CTA / SM, persistent over a static round-robin of tiles):
+//   warp 0      TMA producer  (one lane)
+//   warp 1      TMEM allocator + tcgen05.mma issuer (one lane)
+//   warps 2..5  epilogue: tcgen05.ld -> combine -> packed-baseline store (+= when accumulating)
+#pragma once
+#include "ptx.cuh"
+
+namespace xtc {
+
+constexpr int kNumStages = 8;
+constexpr int kStageBytes = 24 * 1024;
+constexpr int kTileRows = 128;        // G rows per tile   (TMEM lanes)
+constexpr int kTileCols = 256;        // G columns per tile (TMEM columns per accumulator stage)
+constexpr int kNumThreads = 192;
+constexpr int kSmemBytes = kNumStages * kStageBytes + 1024 /*alignment slack*/ + 256 /*barriers*/;
+
+struct TileDesc {
+    int row0;    // first G row   of the tile, in real components u within the channel (multiple of 128)
+    int col0;    // first G column of the tile (multiple of 256)
+    int ncols;   // columns to compute: multiple of 16, <= 256 (triangular cut and channel edge)
+    int pad;
+};
+
+struct Params {
+    const TileDesc* tiles;   // DEVICE: per-channel tile table
+    int tiles_per_chan;
+    long long n_tiles;       // tiles_per_chan * n_chan
+    int n_station, n_pol, n_chan, n_time;
+    int M;                   // n_station * n_pol  (inputs per channel)
+    long long n_baseline;    // N(N+1)/2
+    void* out;               // DEVICE: packed output
+    int accumulate;
+};
+
+template <int kElt> struct Cfg;
+template <> struct Cfg<1> {                      // complex int8 -> int32
+    static constexpr int kKStage = 64;           // time samples per pipeline stage
+    static constexpr int kMmaK = 32;             // time samples per tcgen05.mma (kind::i8)
+    static constexpr bool kFloat = false;
+    // instruction descriptor: D = S32 (2<<4), A = B = signed 8 bit (1<<7, 1<<10), A and B MN-major
+    // (1<<15, 1<<16), M = 128 (8<<24); N is OR-ed in per tile ((N>>3) << 17).
+    static constexpr uint32_t kIdesc = (2u << 4) | (1u << 7) | (1u << 10) | (1u << 15) | (1u << 16) | (8u << 24);
+};
+template <> struct Cfg<2> {                      // complex fp16 -> fp32
+    static constexpr int kKStage = 32;
+    static constexpr int kMmaK = 16;
+    static constexpr bool kFloat = true;
+    // D = F32 (1<<4), A = B = F16 (0), MN-major both, M = 128.
+    static constexpr uint32_t kIdesc = (1u << 4) | (1u << 15) | (1u << 16) | (8u << 24);
+};
+
+template <bool kFloat> __device__ __forceinline__ uint32_t add_bits(uint32_t a, uint32_t b) {
+    if constexpr (kFloat) return __float_as_uint(__uint_as_float(a) + __uint_as_float(b));
+    else return a + b;
+}
+template <bool kFloat> __device__ __forceinline__ uint32_t sub_bits(uint32_t a, uint32_t b) {
+    if constexpr (kFloat) return __float_as_uint(__uint_as_float(a) - __uint_as_float(b));
+    else return a - b;
+}
+
+template <int kElt>
+__global__ void __launch_bounds__(kNumThreads, 1)
+xengine_direct_kernel(const __grid_constant__ CUtensorMap tmap_in, const Params prm) {
+    using C = Cfg<kElt>;
+    constexpr int kChunkElems = 128 / kElt;                 // u per 128-byte chunk
+    constexpr int kChunkBytes = C::kKStage * 128;           // one TMA box: [KSTAGE rows][128 B]
+    constexpr int kAChunks = kTileRows / kChunkElems;       // 1 (ci8) / 2 (cf16)
+    constexpr int kBChunksMax = kTileCols / kChunkElems;    // 2 (ci8) / 4 (cf16)
+    constexpr int kKStepBytes = C::kMmaK * 128;             // smem advance per MMA k-step
+    constexpr int kKSteps = C::kKStage / C::kMmaK;          // 2
+    static_assert((kAChunks + kBChunksMax) * kChunkBytes == kStageBytes, "stage size");
+
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;   // SWIZZLE_128B atoms: 1024-B aligned
+    const uint32_t bar_base = smem_base + kNumStages * kStageBytes;
+    // barrier slots (8 bytes each): full[S], empty[S], tmem_full[2], tmem_empty[2], then the TMEM base word
+    auto full_bar = [&](int s) { return bar_base + 8u * s; };
+    auto empty_bar = [&](int s) { return bar_base + 8u * (kNumStages + s); };
+    auto tfull_bar = [&](int a) { return bar_base + 8u * (2 * kNumStages + a); };
+    auto tempty_bar = [&](int a) { return bar_base + 8u * (2 * kNumStages + 2 + a); };
+    const uint32_t tmem_slot = bar_base + 8u * (2 * kNumStages + 4);
+    uint32_t* tmem_slot_ptr =
+        reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - ptx::smem_u32(smem_raw)));
+
+    const int warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+
+    if (threadIdx.x == 0) {
+        ptx::prefetch_tensormap(&tmap_in);
+        for (int s = 0; s < kNumStages; ++s) {
+            ptx::mbar_init(full_bar(s), 1);
+            ptx::mbar_init(empty_bar(s), 1);
+        }
+        for (int a = 0; a < 2; ++a) {
+            ptx::mbar_init(tfull_bar(a), 1);
+            ptx::mbar_init(tempty_bar(a), 4);      // one arrive per epilogue warp
+        }
+        ptx::fence_mbar_init();
+    }
+    if (warp == 1) {
+        ptx::tmem_alloc(tmem_slot, 512);
+        ptx::tmem_relinquish();
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    const int num_kb = (prm.n_time + C::kKStage - 1) / C::kKStage;
+    const int M2 = 2 * prm.M;
+
+    if (warp == 0) {
+        // ===================== TMA producer =====================
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            for (long long tile = blockIdx.x; tile < prm.n_tiles; tile += gridDim.x) {
+                const int c = static_cast<int>(tile / prm.tiles_per_chan);
+                const TileDesc td = prm.tiles[tile - static_cast<long long>(c) * prm.tiles_per_chan];
+                const int w_row = c * M2 + td.row0;        // element coordinate in the [T][C*2M] view
+                const int w_col = c * M2 + td.col0;
+                const int nb = (td.ncols + kChunkElems - 1) / kChunkElems;
+                const uint32_t tx = static_cast<uint32_t>((kAChunks + nb) * kChunkBytes);
+                for (int kb = 0; kb < num_kb; ++kb) {
+                    ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
+                    const uint32_t sa = smem_base + stage * kStageBytes;
+                    ptx::mbar_arrive_expect_tx(full_bar(stage), tx);
+#pragma unroll
+                    for (int a = 0; a < kAChunks; ++a)
+                        ptx::tma_load_2d(sa + a * kChunkBytes, &tmap_in, full_bar(stage),
+                                         w_row + a * kChunkElems, kb * C::kKStage);
+#pragma unroll
+                    for (int b = 0; b < kBChunksMax; ++b)
+                        if (b < nb)
+                            ptx::tma_load_2d(sa + (kAChunks + b) * kChunkBytes, &tmap_in, full_bar(stage),
+                                             w_col + b * kChunkElems, kb * C::kKStage);
+                    if (++stage == kNumStages) { stage = 0; phase ^= 1u; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===================== MMA issuer =====================
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            int acc = 0;
+            uint32_t acc_phase = 0;
+            for (long long tile = blockIdx.x; tile < prm.n_tiles; tile += gridDim.x) {
+                const int c = static_cast<int>(tile / prm.tiles_per_chan);
+                const TileDesc td = prm.tiles[tile - static_cast<long long>(c) * prm.tiles_per_chan];
+                const uint32_t idesc = C::kIdesc | (static_cast<uint32_t>(td.ncols >> 3) << 17);
+                const uint32_t d_tmem = tmem_base + acc * kTileCols;
+                ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1u);     // epilogue has drained this accumulator
+                ptx::tc_fence_after();
+                for (int kb = 0; kb < num_kb; ++kb) {
+                    ptx::mbar_wait(full_bar(stage), phase);          // TMA bytes have landed
+                    ptx::tc_fence_after();
+                    const uint32_t sa = smem_base + stage * kStageBytes;
+                    const uint32_t sb = sa + kAChunks * kChunkBytes;
+#pragma unroll
+                    for (int k = 0; k < kKSteps; ++k) {
+                        // MN-major SWIZZLE_128B: LBO = distance between 128-byte-wide chunks (one TMA box),
+                        // SBO = distance between 8-row groups along K (8 * 128 B).
+                        const uint64_t adesc = ptx::smem_desc_sw128(sa + k * kKStepBytes, kChunkBytes, 1024);
+                        const uint64_t bdesc = ptx::smem_desc_sw128(sb + k * kKStepBytes, kChunkBytes, 1024);
+                        if constexpr (C::kFloat) ptx::mma_f16(d_tmem, adesc, bdesc, idesc, (kb | k) != 0);
+                        else ptx::mma_i8(d_tmem, adesc, bdesc, idesc, (kb | k) != 0);
+                    }
+                    ptx::mma_commit(empty_bar(stage));               // frees the smem slot when the MMAs retire
+                    if (++stage == kNumStages) { stage = 0; phase ^= 1u; }
+                }
+                ptx::mma_commit(tfull_bar(acc));                     // accumulator complete -> epilogue
+                if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+            }
+        }
+    } else {
+        // ===================== epilogue: combine + packed-baseline writer =====================
+        const int quarter = warp & 3;                // TMEM lanes [32*quarter, 32*quarter+32) belong to this warp
+        const int ri = lane & 1;                     // row parity: 0 = re row (u even), 1 = im row
+        const int P = prm.n_pol;
+        int acc = 0;
+        uint32_t acc_phase = 0;
+        for (long long tile = blockIdx.x; tile < prm.n_tiles; tile += gridDim.x) {
+            const int c = static_cast<int>(tile / prm.tiles_per_chan);
+            const TileDesc td = prm.tiles[tile - static_cast<long long>(c) * prm.tiles_per_chan];
+            const int m = (td.row0 + quarter * 32 + lane) >> 1;      // conjugated input of this lane pair
+            const int i = m / P, p = m - i * P;
+            const bool row_ok = m < prm.M;
+            // word offset of (c, b(i,0), p, q=0); b(i,j) = i(i+1)/2 + j
+            const long long row_base =
+                ((static_cast<long long>(c) * prm.n_baseline + static_cast<long long>(i) * (i + 1) / 2) * P + p) * P * 2;
+            uint32_t* out = static_cast<uint32_t*>(prm.out);
+
+            ptx::mbar_wait(tfull_bar(acc), acc_phase);
+            ptx::tc_fence_after();
+            const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + acc * kTileCols;
+            for (int h0 = 0; h0 < td.ncols; h0 += 32) {
+                uint32_t v[32];
+                ptx::tmem_ld_32x32(taddr + h0, v);
+                ptx::tmem_ld_wait();
+                if (h0 + 32 >= td.ncols) {           // last chunk is in registers: hand the accumulator back
+                    ptx::tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
+                }
+                // step 1: columns (2x, 2x+1) = (re, im) of input n.  Even lane (re row) forms
+                //         Re = G[2m][2n] + G[2m+1][2n+1]; odd lane (im row) forms Im = G[2m][2n+1] - G[2m+1][2n].
+                uint32_t w[16];
+#pragma unroll
+                for (int x = 0; x < 16; ++x) {
+                    const uint32_t other = __shfl_xor_sync(0xffffffffu, v[2 * x + 1], 1);
+                    w[x] = ri ? sub_bits<C::kFloat>(other, v[2 * x]) : add_bits<C::kFloat>(v[2 * x], other);
+                }
+                // step 2: pair (Re, Im) in one lane: even lane keeps inputs n = n0 + 2y, odd lane n0 + 2y + 1.
+                const int n0 = (td.col0 + h0) >> 1;
+#pragma unroll
+                for (int y = 0; y < 8; ++y) {
+                    const uint32_t send = ri ? w[2 * y] : w[2 * y + 1];
+                    const uint32_t recv = __shfl_xor_sync(0xffffffffu, send, 1);
+                    const uint32_t re = ri ? recv : w[2 * y];
+                    const uint32_t im = ri ? w[2 * y + 1] : recv;
+                    const int n = n0 + 2 * y + ri;
+                    const int j = n / P, q = n - j * P;
+                    if (row_ok && n < prm.M && j <= i) {
+                        uint2* dst = reinterpret_cast<uint2*>(out + row_base + (static_cast<long long>(j) * P * P + q) * 2);
+                        uint2 val = make_uint2(re, im);
+                        if (prm.accumulate) {
+                            const uint2 old = *dst;
+                            val.x = add_bits<C::kFloat>(old.x, val.x);
+                            val.y = add_bits<C::kFloat>(old.y, val.y);
+                        }
+                        *dst = val;
+                    }
+                }
+            }
+            if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+        }
+    }
+
+    ptx::tc_fence_before();
+    __syncthreads();
+    if (warp == 1) {
+        ptx::tc_fence_after();
+        ptx::tmem_dealloc(tmem_base, 512);
+    }
+}
+
+}  // namespace xtc
