@@ -109,8 +109,8 @@ int corr_set_feed(corr_handle h, int feed);
 int corr_get_feed(corr_handle h);
 
 /* Which kernel corr_xengine will launch for this geometry: 1 = tcgen05 tensor-core kernel,
- * 0 = SIMT kernel (geometries whose input row pitch C*N*P*sample_bytes is not a multiple of 16,
- * which TMA cannot address). */
+ * 0 = SIMT kernel (geometries whose per-channel sample row N*P*sample_bytes is not a multiple of 16
+ * bytes -- N*P not a multiple of 8 (CI8) / 4 (CF16) -- where TMA box starts would be misaligned). */
 int corr_uses_tensor_cores(corr_handle h);
 
 /*

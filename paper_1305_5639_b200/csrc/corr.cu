@@ -38,7 +38,8 @@ struct corr_plan {
     int device;
     int sm_count;
     int feed;
-    bool tma_ok;           // input row pitch is a multiple of 16 bytes
+    bool tma_ok;           // one channel's row of components (2*M*elt bytes) is a multiple of 16 bytes, so every
+                           // TMA box start (c*2M + tile offset) is 16-byte aligned
     long long t_total;     // samples integrated since the last accumulate == 0 call
     int last_launches;
 
@@ -270,7 +271,7 @@ corr_handle corr_create(int n_station, int n_pol, int n_chan, int n_time, int dt
     h->device = dev;
     h->sm_count = prop.multiProcessorCount;
     h->feed = CORR_FEED_DIRECT;
-    h->tma_ok = (static_cast<long long>(n_chan) * M * h->sample_bytes) % 16 == 0;
+    h->tma_ok = (M * h->sample_bytes) % 16 == 0;
     h->t_total = 0;
     h->last_launches = 0;
     h->d_tiles = nullptr;
@@ -352,8 +353,8 @@ int corr_corner_turn(corr_handle h, const void* in, void* ws, void* stream) {
     if ((reinterpret_cast<uintptr_t>(in) & 15) || (reinterpret_cast<uintptr_t>(ws) & 1023))
         return fail(h, CORR_EINVAL, "corr_corner_turn: `in` must be 16-byte and `ws` 1024-byte aligned");
     if (!h->tma_ok)
-        return fail(h, CORR_EUNSUPPORTED, "corr_corner_turn: input row pitch %lld B is not a multiple of 16",
-                    static_cast<long long>(h->C) * h->M * h->sample_bytes);
+        return fail(h, CORR_EUNSUPPORTED, "corr_corner_turn: per-channel row of %lld B is not a multiple of 16",
+                    static_cast<long long>(h->M) * h->sample_bytes);
     h->last_launches = 0;
     return launch_corner_turn(h, in, ws, static_cast<cudaStream_t>(stream));
 }
