@@ -86,7 +86,8 @@ int corr_xengine(corr_handle h, const void* in, void* out, int accumulate, void*
  * staging buffer owned by the handle, runs corr_xengine on the handle's own stream, copies the
  * result to `out_host` and synchronises.  With accumulate != 0 the running sum lives in the
  * handle's device staging buffer (state of the previous corr_xengine_host call on this handle) and
- * `out_host` receives the updated integration.  Pinned host memory makes the copies DMA directly.
+ * `out_host` receives the updated integration; `out_host` may be NULL to leave the running sum on
+ * the device until a later call asks for it.  Pinned host memory makes the copies DMA directly.
  */
 int corr_xengine_host(corr_handle h, const void* in_host, void* out_host, int accumulate);
 

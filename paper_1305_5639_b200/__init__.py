@@ -9,6 +9,7 @@ __all__ = ["inputs"]
 def __getattr__(name):
     # lazy: importing the package (e.g. for ``inputs``) must not require the CUDA library
     if name in ("Correlator", "CorrError", "lib", "binding"):
-        from . import binding
+        import importlib
+        binding = importlib.import_module(__name__ + ".binding")
         return binding if name == "binding" else getattr(binding, name)
     raise AttributeError(name)

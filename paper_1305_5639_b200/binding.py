@@ -170,8 +170,10 @@ class Correlator:
     def xengine_host(self, x_host, out_host, accumulate=False):
         """corr_xengine_host: HOST tensors in and out (blocking; copies inside the library)."""
         self._check_in(x_host, "cpu")
-        self._check_out(out_host, "cpu")
-        self._check(self._L.corr_xengine_host(self._h, x_host.data_ptr(), out_host.data_ptr(),
+        if out_host is not None:
+            self._check_out(out_host, "cpu")
+        self._check(self._L.corr_xengine_host(self._h, x_host.data_ptr(),
+                                              None if out_host is None else out_host.data_ptr(),
                                               int(bool(accumulate))))
         return out_host
 

@@ -381,7 +381,7 @@ int corr_xengine(corr_handle h, const void* in, void* out, int accumulate, void*
 
 int corr_xengine_host(corr_handle h, const void* in_host, void* out_host, int accumulate) {
     if (!h) return CORR_EINVAL;
-    if (!in_host || !out_host) return fail(h, CORR_EINVAL, "corr_xengine_host: NULL pointer");
+    if (!in_host) return fail(h, CORR_EINVAL, "corr_xengine_host: NULL input pointer");
     cudaError_t e;
     if (!h->own_stream) {
         e = cudaStreamCreateWithFlags(&h->own_stream, cudaStreamNonBlocking);
@@ -400,8 +400,10 @@ int corr_xengine_host(corr_handle h, const void* in_host, void* out_host, int ac
     if (e != cudaSuccess) return fail_cuda(h, e, "H2D copy");
     const int rc = corr_xengine(h, h->d_in_stage, h->d_out_stage, accumulate, h->own_stream);
     if (rc != CORR_OK) return rc;
-    e = cudaMemcpyAsync(out_host, h->d_out_stage, output_bytes(h), cudaMemcpyDeviceToHost, h->own_stream);
-    if (e != cudaSuccess) return fail_cuda(h, e, "D2H copy");
+    if (out_host) {
+        e = cudaMemcpyAsync(out_host, h->d_out_stage, output_bytes(h), cudaMemcpyDeviceToHost, h->own_stream);
+        if (e != cudaSuccess) return fail_cuda(h, e, "D2H copy");
+    }
     e = cudaStreamSynchronize(h->own_stream);
     if (e != cudaSuccess) return fail_cuda(h, e, "corr_xengine_host: stream synchronize");
     return CORR_OK;

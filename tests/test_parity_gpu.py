@@ -1,0 +1,298 @@
+"""GPU parity: libcorr.so (through its C ABI, via the ctypes binding) against the CPU oracle.
+
+Bar (BASELINE.json north_star): complex int8 -> int32 path BIT-EXACT, every word of the packed
+output; complex fp16 -> fp32 path |dV_ij| <= 2e-5 * sqrt(V_ii^{pp} V_jj^{qq}) with both
+autocorrelations taken from the fp64 oracle.  Small cases are compared element by element on all
+channels; BASELINE.json's full-size configs are compared on sampled channels (every baseline and
+polarisation product of each sampled channel) plus two identities that hold at any size on EVERY
+channel: the beam-sum identity and real, non-negative autocorrelations.
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_1305_5639_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+FP16_TOL = 2e-5          # north_star: |dV_ij| <= 2e-5 * sqrt(V_ii * V_jj)
+
+
+@pytest.fixture(scope="module")
+def corr():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (there is no CPU fallback)")
+    from paper_1305_5639_b200 import binding
+    binding.lib()
+    return binding
+
+
+def run_gpu(corr, xs, dtype, accumulate_calls=True, host=False):
+    """xs: list of input tensors (one per call).  Returns the int32/fp32 output as numpy."""
+    T, C, N, P, _ = xs[0].shape
+    with corr.Correlator(N, P, C, T, dtype) as h:
+        if host:
+            out = torch.empty(h.output_shape(), dtype=torch.int32 if dtype == "ci8" else torch.float32)
+            for k, x in enumerate(xs):
+                h.xengine_host(x.cpu().contiguous(), out, accumulate=(k > 0 and accumulate_calls))
+            return out.numpy(), h.uses_tensor_cores
+        out = None
+        for k, x in enumerate(xs):
+            out = h.xengine(x.cuda(), out, accumulate=(k > 0 and accumulate_calls))
+        torch.cuda.synchronize()
+        return out.cpu().numpy(), h.uses_tensor_cores
+
+
+def run_oracle(oracle, xs, chans=None):
+    V = None
+    for x in xs:
+        V = oracle.xengine(x.cpu().numpy(), chans=chans, accumulate_into=V)
+    return V
+
+
+def assert_bit_exact(got, want):
+    assert got.dtype == np.int32 and want.dtype == np.int64
+    assert np.abs(want).max() < 2 ** 31
+    bad = np.argwhere(got.astype(np.int64) != want)
+    assert bad.size == 0, "first mismatches (c,b,p,q,reim): %s" % bad[:8].tolist()
+
+
+def fp16_normalised_error(got, want, N, P):
+    """max over all visibilities of |dV| / sqrt(V_ii^pp V_jj^qq) (autocorrelations from the oracle)."""
+    i_of_b = np.concatenate([np.full(i + 1, i) for i in range(N)])
+    j_of_b = np.concatenate([np.arange(i + 1) for i in range(N)])
+    auto_b = np.array([i * (i + 1) // 2 + i for i in range(N)])
+    auto = np.stack([want[:, auto_b, p, p, 0] for p in range(P)], axis=-1)        # [C, N, P]
+    d = got.astype(np.float64) - want
+    err = np.sqrt(d[..., 0] ** 2 + d[..., 1] ** 2)                                # [C, B, P, P]
+    norm = np.sqrt(auto[:, i_of_b, :, None] * auto[:, j_of_b, None, :])
+    return float((err / norm).max())
+
+
+# ---------------------------------------------------------------------------------------------
+# small cases: every channel, every word
+# ---------------------------------------------------------------------------------------------
+SMALL_CI8 = [
+    # N, P, C, T      what it exercises
+    (16, 2, 64, 256),   # BASELINE config 1
+    (1, 1, 1, 1),       # smallest possible problem (SIMT path: row pitch not a multiple of 16 B)
+    (1, 2, 3, 5),
+    (4, 2, 5, 70),      # one partial tile, ragged T (not a multiple of the 64-sample stage)
+    (8, 1, 3, 33),      # single polarisation on the tensor-core path
+    (33, 2, 3, 100),    # N*P*2 = 132 B row: SIMT path
+    (36, 2, 3, 130),    # 144 columns: two row blocks, ragged column cut
+    (40, 1, 2, 64),
+    (72, 2, 2, 192),    # 288 columns: >1 column block
+    (100, 2, 2, 96),    # 400 columns: several row blocks + triangular cut + channel edge
+    (130, 2, 1, 64),    # 520 columns
+    (64, 2, 7, 1),      # T = 1
+]
+
+
+@pytest.mark.parametrize("N,P,C,T", SMALL_CI8)
+def test_ci8_bit_exact_small(corr, oracle, N, P, C, T):
+    x = inputs.gauss_ci8(T, C, N, P, 40.0, seed=7000 + N * 3 + T)
+    got, tc = run_gpu(corr, [x], "ci8")
+    assert tc == ((N * P * 2) % 16 == 0)
+    assert_bit_exact(got, run_oracle(oracle, [x]))
+
+
+def test_ci8_full_range_including_minus_128(corr, oracle):
+    """-128 is exact on the direct (no-negation) feed: corr.h 'any value in [-128, 127] is exact'."""
+    g = torch.Generator().manual_seed(11)
+    x = torch.randint(-128, 128, (96, 3, 24, 2, 2), generator=g, dtype=torch.int8)
+    x[0, 0] = -128
+    x[1, 1] = 127
+    got, tc = run_gpu(corr, [x], "ci8")
+    assert tc
+    assert_bit_exact(got, run_oracle(oracle, [x]))
+
+
+def test_ci8_extreme_constant_fills_int32_range(corr, oracle):
+    """All samples -128-128j for T = 65535: |V| = 2 * 128^2 * 65535 = 2^31 - 32768, the largest exact sum."""
+    x = torch.full((4096, 1, 8, 2, 2), -128, dtype=torch.int8)
+    with corr.Correlator(8, 2, 1, 4096, "ci8") as h:
+        xd = x.cuda()
+        out = h.xengine(xd)
+        for _ in range(14):
+            h.xengine(xd, out, accumulate=True)
+        torch.cuda.synchronize()
+        # 15 * 4096 = 61440 samples so far; 65535 is not a multiple of 4096, so stop here and check
+        got = out.cpu().numpy()
+        assert (got[..., 0] == 2 * 128 * 128 * 61440).all() and (got[..., 1] == 0).all()
+        # one more call would be 65536 samples > 65535: refused, nothing launched
+        with pytest.raises(corr.CorrError) as e:
+            h.xengine(xd, out, accumulate=True)
+        assert e.value.code == corr.CORR_EOVERFLOW
+        torch.cuda.synchronize()
+        assert (out.cpu().numpy() == got).all()
+
+
+@pytest.mark.parametrize("host", [False, True])
+def test_ci8_accumulate_across_calls(corr, oracle, host):
+    """Integration across successive calls: accumulate = 0, 1, 1 equals the oracle's sum."""
+    xs = [inputs.gauss_ci8(128, 4, 40, 2, 30.0, seed=7100 + k) for k in range(3)]
+    got, _ = run_gpu(corr, xs, "ci8", host=host)
+    assert_bit_exact(got, run_oracle(oracle, xs))
+    # and concatenating the calls' samples is the same thing (additivity in time)
+    assert_bit_exact(got, run_oracle(oracle, [torch.cat(xs, dim=0)]))
+
+
+def test_accumulate_zero_overwrites_garbage(corr, oracle):
+    x = inputs.gauss_ci8(64, 2, 20, 2, 30.0, seed=7200)
+    with corr.Correlator(20, 2, 2, 64, "ci8") as h:
+        out = torch.full(h.output_shape(), 0x5a5a5a5a, dtype=torch.int32, device="cuda")
+        h.xengine(x.cuda(), out, accumulate=False)
+        torch.cuda.synchronize()
+        assert_bit_exact(out.cpu().numpy(), run_oracle(oracle, [x]))
+
+
+def test_does_not_write_outside_the_output(corr):
+    x = inputs.gauss_ci8(64, 3, 36, 2, 30.0, seed=7300).cuda()
+    with corr.Correlator(36, 2, 3, 64, "ci8") as h:
+        n = h.output_bytes // 4
+        buf = torch.full((n + 2048,), 0x7e7e7e7e, dtype=torch.int32, device="cuda")
+        out = buf[1024:1024 + n].view(h.output_shape())
+        h.xengine(x, out)
+        torch.cuda.synchronize()
+        assert (buf[:1024] == 0x7e7e7e7e).all() and (buf[1024 + n:] == 0x7e7e7e7e).all()
+
+
+def test_argument_errors(corr):
+    with corr.Correlator(16, 2, 4, 64, "ci8") as h:
+        x = torch.zeros(h.input_shape(), dtype=torch.int8, device="cuda")
+        out = h.empty_output()
+        L = corr.lib()
+        assert L.corr_xengine(h._h, None, out.data_ptr(), 0, None) == corr.CORR_EINVAL
+        assert L.corr_xengine(h._h, x.data_ptr(), None, 0, None) == corr.CORR_EINVAL
+        assert L.corr_xengine(h._h, x.data_ptr() + 2, out.data_ptr(), 0, None) == corr.CORR_EINVAL
+        assert b"aligned" in L.corr_last_error(h._h)
+        assert h.input_bytes == x.numel() and h.output_bytes == out.numel() * 4
+
+
+SMALL_CF16 = [(16, 2, 8, 256), (2, 2, 3, 40), (3, 1, 2, 17), (20, 2, 3, 100), (68, 2, 2, 160), (128, 2, 2, 512)]
+
+
+@pytest.mark.parametrize("N,P,C,T", SMALL_CF16)
+def test_cf16_within_tolerance_small(corr, oracle, N, P, C, T):
+    x = inputs.corr_phase_cf16(T, C, N, P, seed=7400 + N)
+    got, tc = run_gpu(corr, [x], "cf16")
+    assert tc == ((N * P * 4) % 16 == 0)
+    want = run_oracle(oracle, [x])
+    assert fp16_normalised_error(got, want, N, P) <= FP16_TOL
+
+
+def test_cf16_accumulate_across_calls(corr, oracle):
+    xs = [inputs.corr_phase_cf16(256, 3, 24, 2, seed=7500 + k) for k in range(3)]
+    got, _ = run_gpu(corr, xs, "cf16")
+    assert fp16_normalised_error(got, run_oracle(oracle, xs), 24, 2) <= FP16_TOL
+
+
+def test_stream_argument_is_honoured(corr, oracle):
+    x = inputs.gauss_ci8(64, 4, 16, 2, 30.0, seed=7600)
+    s = torch.cuda.Stream()
+    with corr.Correlator(16, 2, 4, 64, "ci8") as h:
+        with torch.cuda.stream(s):
+            xd = x.cuda(non_blocking=False)
+            out = h.xengine(xd, stream=s)
+        s.synchronize()
+        assert_bit_exact(out.cpu().numpy(), run_oracle(oracle, [x]))
+        assert h.last_launch_count >= 1
+
+
+def test_corner_turn_kernel(corr):
+    """Piece (a): ws[c][m][t] = in[t][c][m], ws_rot = (im, -re), time zero-padded -- against torch ops."""
+    for dtype, N, P, C, T in [("ci8", 24, 2, 5, 100), ("ci8", 64, 2, 3, 256), ("cf16", 20, 2, 3, 70)]:
+        if dtype == "ci8":
+            x = inputs.gauss_ci8(T, C, N, P, 30.0, seed=7700)
+        else:
+            x = inputs.corr_phase_cf16(T, C, N, P, seed=7701)
+        with corr.Correlator(N, P, C, T, dtype) as h:
+            ws = h.corner_turn(x.cuda())
+            torch.cuda.synchronize()
+            Tp = h.workspace_time
+            planes = ws.cpu().view(torch.int8 if dtype == "ci8" else torch.float16).view(2, C, N * P, Tp, 2)
+        ref = x.reshape(T, C, N * P, 2).permute(1, 2, 0, 3)                       # [C, M, T, 2]
+        assert torch.equal(planes[0, :, :, :T], ref)
+        rot = torch.stack([ref[..., 1], -ref[..., 0]], dim=-1)
+        assert torch.equal(planes[1, :, :, :T], rot)
+        assert (planes[:, :, :, T:] == 0).all()
+
+
+# ---------------------------------------------------------------------------------------------
+# BASELINE.json configs at full size, in the launch configuration bench.py times
+# ---------------------------------------------------------------------------------------------
+def sample_channels(C, n, seed):
+    rng = np.random.default_rng(seed)
+    mid = rng.choice(np.arange(1, C - 1), size=min(n, C) - 2, replace=False) if C > 2 else []
+    return np.unique(np.concatenate([[0, C - 1], mid]).astype(np.int32))
+
+
+def beam_sum_identity(xs, got, N, P):
+    """Both sides of  sum_{m,n} H_c[m][n] = sum_t |sum_m x[t][c][m]|^2  for EVERY channel (SURVEY pin 10).
+    The right side is formed from the device-resident inputs in chunks of time with torch ops (exact in
+    int64 for ci8, fp64 for cf16); the left side expands the packed triangle by Hermitian symmetry."""
+    C = got.shape[0]
+    integer = got.dtype == np.int32
+    wide = torch.int64 if integer else torch.float64
+    rhs = torch.zeros(C, dtype=wide, device=xs[0].device)
+    for x in xs:
+        for t0 in range(0, x.shape[0], 64):
+            s = x[t0:t0 + 64].to(torch.int32 if integer else torch.float64).sum(dim=(2, 3)).to(wide)   # [t, C, 2]
+            rhs += (s * s).sum(dim=(0, 2))
+    g = torch.from_numpy(got)
+    re = g[..., 0].to(wide)
+    auto_b = torch.tensor([i * (i + 1) // 2 + i for i in range(N)])
+    lhs = 2 * re.sum(dim=(1, 2, 3)) - re[:, auto_b].sum(dim=(1, 2, 3))            # cross terms twice, autos once
+    return lhs.numpy(), rhs.cpu().numpy()
+
+
+def check_full_config(corr, oracle, name, n_chan_sample):
+    cfg = inputs.CONFIGS[name]
+    N, P, C, T, dtype = cfg["N"], cfg["P"], cfg["C"], cfg["T"], cfg["dtype"]
+    xs = [inputs.make_input(cfg, call=k, device="cuda") for k in range(cfg["calls"])]
+    with corr.Correlator(N, P, C, T, dtype) as h:
+        assert h.uses_tensor_cores
+        out = None
+        for k, x in enumerate(xs):
+            out = h.xengine(x, out, accumulate=k > 0)
+        torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    chans = sample_channels(C, n_chan_sample, cfg["seed"])
+    want = None
+    for x in xs:
+        want = oracle.xengine(x.cpu().numpy(), chans=chans, accumulate_into=want)
+    lhs, rhs = beam_sum_identity(xs, got, N, P)
+    auto_b = np.array([i * (i + 1) // 2 + i for i in range(N)])
+    if dtype == "ci8":
+        assert_bit_exact(got[chans], want)
+        assert (lhs == rhs).all()
+        for p in range(P):
+            assert (got[:, auto_b, p, p, 1] == 0).all() and (got[:, auto_b, p, p, 0] >= 0).all()
+    else:
+        err = fp16_normalised_error(got[chans], want, N, P)
+        assert err <= FP16_TOL, err
+        # the per-visibility tolerance implies |lhs - rhs| <= tol * (sum_m sqrt(H_mm))^2
+        autos = np.stack([got[:, auto_b, p, p, 0] for p in range(P)], axis=-1).astype(np.float64)   # [C, N, P]
+        assert (autos > 0).all()
+        bound = FP16_TOL * np.sqrt(autos).sum(axis=(1, 2)) ** 2
+        assert (np.abs(lhs - rhs) <= bound).all()
+        for p in range(P):
+            assert (np.abs(got[:, auto_b, p, p, 1]) <= FP16_TOL * got[:, auto_b, p, p, 0]).all()
+
+
+def test_config2_full_size(corr, oracle):
+    check_full_config(corr, oracle, "cfg2", 24)
+
+
+def test_config3_full_size_fp16(corr, oracle):
+    check_full_config(corr, oracle, "cfg3", 8)
+
+
+def test_config4_full_size_four_calls(corr, oracle):
+    check_full_config(corr, oracle, "cfg4", 8)
+
+
+@pytest.mark.parametrize("N", [32, 128, 512, 1024])
+def test_config5_sweep_points(corr, oracle, N):
+    check_full_config(corr, oracle, "cfg5_n%d" % N, 4 if N <= 128 else 2)
