@@ -121,7 +121,7 @@ int corr_uses_tensor_cores(corr_handle h);
  *     ws_rot[c][m][t] = (im, -re) of the same sample           (feeds the imaginary part)
  * with the time axis padded to corr_workspace_time(h) samples (zero filled).
  *   in      DEVICE pointer as for corr_xengine.
- *   ws      DEVICE pointer, corr_workspace_bytes(h) bytes, 1024-byte aligned: the two planes,
+ *   ws      DEVICE pointer, corr_workspace_bytes(h) bytes, 128-byte aligned: the two planes,
  *           ws then ws_rot, each n_chan * M * corr_workspace_time(h) samples.
  * Asynchronous on `stream`.  corr_xengine with CORR_FEED_CORNER_TURN runs this internally.
  */

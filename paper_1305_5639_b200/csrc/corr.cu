@@ -350,8 +350,8 @@ int corr_set_feed(corr_handle h, int feed) {
 int corr_corner_turn(corr_handle h, const void* in, void* ws, void* stream) {
     if (!h) return CORR_EINVAL;
     if (!in || !ws) return fail(h, CORR_EINVAL, "corr_corner_turn: NULL pointer");
-    if ((reinterpret_cast<uintptr_t>(in) & 15) || (reinterpret_cast<uintptr_t>(ws) & 1023))
-        return fail(h, CORR_EINVAL, "corr_corner_turn: `in` must be 16-byte and `ws` 1024-byte aligned");
+    if ((reinterpret_cast<uintptr_t>(in) & 15) || (reinterpret_cast<uintptr_t>(ws) & 127))
+        return fail(h, CORR_EINVAL, "corr_corner_turn: `in` must be 16-byte and `ws` 128-byte aligned");
     if (!h->tma_ok)
         return fail(h, CORR_EUNSUPPORTED, "corr_corner_turn: per-channel row of %lld B is not a multiple of 16",
                     static_cast<long long>(h->M) * h->sample_bytes);
