@@ -146,6 +146,9 @@ int launch_direct(corr_plan* h, const void* in, void* out, int accumulate, cudaS
     prm.n_baseline = h->B;
     prm.out = out;
     prm.accumulate = accumulate ? 1 : 0;
+    // samples per TMEM accumulation pass: everything for int32 (exact); 1024 for fp32 (see xengine_tc.cuh)
+    const int kstage = h->dtype == CORR_CI8 ? xtc::Cfg<1>::kKStage : xtc::Cfg<2>::kKStage;
+    prm.k_chunk = h->dtype == CORR_CI8 ? (h->T + kstage - 1) / kstage * kstage : xtc::kFloatChunk;
     const long long grid = prm.n_tiles < h->sm_count ? prm.n_tiles : h->sm_count;
     if (h->dtype == CORR_CI8)
         xtc::xengine_direct_kernel<1><<<static_cast<unsigned>(grid), xtc::kNumThreads, xtc::kSmemBytes, st>>>(h->tmap_in, prm);

@@ -14,21 +14,39 @@
 // the accumulator lives in TMEM (256 columns, double buffered), and the epilogue forms Re/Im with
 // one shuffle between adjacent TMEM lanes and streams the packed triangle to HBM.
 //
-// Warp roles (192 threads, 1 CTA / SM, persistent over a static round-robin of tiles):
+// Warp roles (320 threads, 1 CTA / SM, persistent over a static round-robin of tiles):
 //   warp 0      TMA producer  (one lane)
 //   warp 1      TMEM allocator + tcgen05.mma issuer (one lane)
-//   warps 2..5  epilogue: tcgen05.ld -> combine -> packed-baseline store (+= when accumulating)
+//   warps 2..9  epilogue: tcgen05.ld -> combine -> shared-memory staging in packed-baseline order ->
+//               bulk async store (or bulk reduce-add when accumulating) of whole station-row segments.
+//               Warp w owns TMEM lanes 32 (w % 4) .. +31 and the column half (w - 2) / 4 of the tile.
+//
+// Integration in time is cut into K-chunks of `k_chunk` samples per TMEM accumulation pass: the int8
+// path uses one chunk (int32 sums are exact); the fp16 path uses 1024 samples so that the tensor
+// core's fp32 accumulator (which truncates when it aligns addends)
+// never integrates more than 64 MMAs before its content is folded into the output with an IEEE
+// round-to-nearest fp32 add (the L2's reduce-add).  Chunk 0 stores (or reduce-adds if the call
+// accumulates), chunks >= 1 reduce-add.
 #pragma once
 #include "ptx.cuh"
 
 namespace xtc {
 
-constexpr int kNumStages = 8;
+constexpr int kNumStages = 6;
 constexpr int kStageBytes = 24 * 1024;
 constexpr int kTileRows = 128;        // G rows per tile   (TMEM lanes)
 constexpr int kTileCols = 256;        // G columns per tile (TMEM columns per accumulator stage)
-constexpr int kNumThreads = 192;
-constexpr int kSmemBytes = kNumStages * kStageBytes + 1024 /*alignment slack*/ + 256 /*barriers*/;
+constexpr int kNumEpiWarps = 8;
+constexpr int kNumThreads = 64 + 32 * kNumEpiWarps;
+// epilogue staging (n_pol == 2): one pass = 64 G columns = 16 stations j; a warp's 32 TMEM lanes are
+// 8 stations i; one station-row segment is 16 x 32 B = 512 B, padded to 544 B (bank spread, 16-B aligned)
+constexpr int kFloatChunk = 1024;   // fp16 path: samples per TMEM accumulation pass
+constexpr int kEpiCols = 64;
+constexpr int kEpiRowBytes = 544;
+constexpr int kEpiBufBytes = 8 * kEpiRowBytes;
+constexpr int kEpiWarpBytes = 2 * kEpiBufBytes;                       // double buffered
+constexpr int kEpiBytes = kNumEpiWarps * kEpiWarpBytes;
+constexpr int kSmemBytes = kNumStages * kStageBytes + kEpiBytes + 1024 /*alignment slack*/ + 256 /*barriers*/;
 
 struct TileDesc {
     int row0;    // first G row   of the tile, in real components u within the channel (multiple of 128)
@@ -46,6 +64,7 @@ struct Params {
     long long n_baseline;    // N(N+1)/2
     void* out;               // DEVICE: packed output
     int accumulate;
+    int k_chunk;             // samples per TMEM accumulation pass (multiple of the pipeline stage)
 };
 
 template <int kElt> struct Cfg;
@@ -74,6 +93,27 @@ template <bool kFloat> __device__ __forceinline__ uint32_t sub_bits(uint32_t a, 
     else return a - b;
 }
 
+// Re/Im of eight (m, n) products from one 32-column TMEM chunk.  Lane pair (2k, 2k+1) holds G rows
+// (2m, 2m+1); columns (2x, 2x+1) are (re, im) of input n0 + x.  On return the even lane (ri = 0) holds
+// (re, im) of inputs n0 + 2y, the odd lane of inputs n0 + 2y + 1, y = 0..7.
+template <bool kFloat>
+__device__ __forceinline__ void combine_chunk(const uint32_t (&v)[32], int ri, uint32_t (&re)[8], uint32_t (&im)[8]) {
+    uint32_t w[16];
+#pragma unroll
+    for (int x = 0; x < 16; ++x) {
+        // even lane: Re = G[2m][2n] + G[2m+1][2n+1];  odd lane: Im = G[2m][2n+1] - G[2m+1][2n]
+        const uint32_t other = __shfl_xor_sync(0xffffffffu, v[2 * x + 1], 1);
+        w[x] = ri ? sub_bits<kFloat>(other, v[2 * x]) : add_bits<kFloat>(v[2 * x], other);
+    }
+#pragma unroll
+    for (int y = 0; y < 8; ++y) {
+        const uint32_t send = ri ? w[2 * y] : w[2 * y + 1];
+        const uint32_t recv = __shfl_xor_sync(0xffffffffu, send, 1);
+        re[y] = ri ? recv : w[2 * y];
+        im[y] = ri ? w[2 * y + 1] : recv;
+    }
+}
+
 template <int kElt>
 __global__ void __launch_bounds__(kNumThreads, 1)
 xengine_direct_kernel(const __grid_constant__ CUtensorMap tmap_in, const Params prm) {
@@ -88,7 +128,8 @@ xengine_direct_kernel(const __grid_constant__ CUtensorMap tmap_in, const Params 
 
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;   // SWIZZLE_128B atoms: 1024-B aligned
-    const uint32_t bar_base = smem_base + kNumStages * kStageBytes;
+    const uint32_t epi_base = smem_base + kNumStages * kStageBytes;
+    const uint32_t bar_base = epi_base + kEpiBytes;
     // barrier slots (8 bytes each): full[S], empty[S], tmem_full[2], tmem_empty[2], then the TMEM base word
     auto full_bar = [&](int s) { return bar_base + 8u * s; };
     auto empty_bar = [&](int s) { return bar_base + 8u * (kNumStages + s); };
@@ -109,7 +150,7 @@ xengine_direct_kernel(const __grid_constant__ CUtensorMap tmap_in, const Params 
         }
         for (int a = 0; a < 2; ++a) {
             ptx::mbar_init(tfull_bar(a), 1);
-            ptx::mbar_init(tempty_bar(a), 4);      // one arrive per epilogue warp
+            ptx::mbar_init(tempty_bar(a), kNumEpiWarps);      // one arrive per epilogue warp
         }
         ptx::fence_mbar_init();
     }
@@ -122,7 +163,9 @@ xengine_direct_kernel(const __grid_constant__ CUtensorMap tmap_in, const Params 
     ptx::tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
 
-    const int num_kb = (prm.n_time + C::kKStage - 1) / C::kKStage;
+    const int num_kb = (prm.n_time + C::kKStage - 1) / C::kKStage;     // pipeline stages over the whole integration
+    const int kb_per_chunk = prm.k_chunk / C::kKStage;
+    const int n_kchunks = (num_kb + kb_per_chunk - 1) / kb_per_chunk;
     const int M2 = 2 * prm.M;
 
     if (warp == 0) {
@@ -165,92 +208,160 @@ xengine_direct_kernel(const __grid_constant__ CUtensorMap tmap_in, const Params 
                 const int c = static_cast<int>(tile / prm.tiles_per_chan);
                 const TileDesc td = prm.tiles[tile - static_cast<long long>(c) * prm.tiles_per_chan];
                 const uint32_t idesc = C::kIdesc | (static_cast<uint32_t>(td.ncols >> 3) << 17);
-                const uint32_t d_tmem = tmem_base + acc * kTileCols;
-                ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1u);     // epilogue has drained this accumulator
-                ptx::tc_fence_after();
-                for (int kb = 0; kb < num_kb; ++kb) {
-                    ptx::mbar_wait(full_bar(stage), phase);          // TMA bytes have landed
+                for (int kb0 = 0; kb0 < num_kb; kb0 += kb_per_chunk) {
+                    const int kb1 = kb0 + kb_per_chunk < num_kb ? kb0 + kb_per_chunk : num_kb;
+                    const uint32_t d_tmem = tmem_base + acc * kTileCols;
+                    ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1u);     // epilogue has drained this accumulator
                     ptx::tc_fence_after();
-                    const uint32_t sa = smem_base + stage * kStageBytes;
-                    const uint32_t sb = sa + kAChunks * kChunkBytes;
+                    for (int kb = kb0; kb < kb1; ++kb) {
+                        ptx::mbar_wait(full_bar(stage), phase);          // TMA bytes have landed
+                        ptx::tc_fence_after();
+                        const uint32_t sa = smem_base + stage * kStageBytes;
+                        const uint32_t sb = sa + kAChunks * kChunkBytes;
 #pragma unroll
-                    for (int k = 0; k < kKSteps; ++k) {
-                        // MN-major SWIZZLE_128B: LBO = distance between 128-byte-wide chunks (one TMA box),
-                        // SBO = distance between 8-row groups along K (8 * 128 B).
-                        const uint64_t adesc = ptx::smem_desc_sw128(sa + k * kKStepBytes, kChunkBytes, 1024);
-                        const uint64_t bdesc = ptx::smem_desc_sw128(sb + k * kKStepBytes, kChunkBytes, 1024);
-                        if constexpr (C::kFloat) ptx::mma_f16(d_tmem, adesc, bdesc, idesc, (kb | k) != 0);
-                        else ptx::mma_i8(d_tmem, adesc, bdesc, idesc, (kb | k) != 0);
+                        for (int k = 0; k < kKSteps; ++k) {
+                            // MN-major SWIZZLE_128B: LBO = distance between 128-byte-wide chunks (one TMA box),
+                            // SBO = distance between 8-row groups along K (8 * 128 B).
+                            const uint64_t adesc = ptx::smem_desc_sw128(sa + k * kKStepBytes, kChunkBytes, 1024);
+                            const uint64_t bdesc = ptx::smem_desc_sw128(sb + k * kKStepBytes, kChunkBytes, 1024);
+                            const uint32_t accum = (kb != kb0 || k != 0) ? 1u : 0u;
+                            if constexpr (C::kFloat) ptx::mma_f16(d_tmem, adesc, bdesc, idesc, accum);
+                            else ptx::mma_i8(d_tmem, adesc, bdesc, idesc, accum);
+                        }
+                        ptx::mma_commit(empty_bar(stage));               // frees the smem slot when the MMAs retire
+                        if (++stage == kNumStages) { stage = 0; phase ^= 1u; }
                     }
-                    ptx::mma_commit(empty_bar(stage));               // frees the smem slot when the MMAs retire
-                    if (++stage == kNumStages) { stage = 0; phase ^= 1u; }
+                    ptx::mma_commit(tfull_bar(acc));                     // accumulator complete -> epilogue
+                    if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
                 }
-                ptx::mma_commit(tfull_bar(acc));                     // accumulator complete -> epilogue
-                if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
             }
         }
     } else {
         // ===================== epilogue: combine + packed-baseline writer =====================
+        const int ew = warp - 2;
         const int quarter = warp & 3;                // TMEM lanes [32*quarter, 32*quarter+32) belong to this warp
+        const int chalf = ew >> 2;                   // column half of the tile handled by this warp
         const int ri = lane & 1;                     // row parity: 0 = re row (u even), 1 = im row
         const int P = prm.n_pol;
+        const uint32_t stage_smem = epi_base + ew * kEpiWarpBytes;
+        uint8_t* out8 = static_cast<uint8_t*>(prm.out);
         int acc = 0;
         uint32_t acc_phase = 0;
+        int buf = 0;
         for (long long tile = blockIdx.x; tile < prm.n_tiles; tile += gridDim.x) {
             const int c = static_cast<int>(tile / prm.tiles_per_chan);
             const TileDesc td = prm.tiles[tile - static_cast<long long>(c) * prm.tiles_per_chan];
-            const int m = (td.row0 + quarter * 32 + lane) >> 1;      // conjugated input of this lane pair
-            const int i = m / P, p = m - i * P;
-            const bool row_ok = m < prm.M;
-            // word offset of (c, b(i,0), p, q=0); b(i,j) = i(i+1)/2 + j
-            const long long row_base =
-                ((static_cast<long long>(c) * prm.n_baseline + static_cast<long long>(i) * (i + 1) / 2) * P + p) * P * 2;
-            uint32_t* out = static_cast<uint32_t*>(prm.out);
-
-            ptx::mbar_wait(tfull_bar(acc), acc_phase);
-            ptx::tc_fence_after();
-            const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + acc * kTileCols;
-            for (int h0 = 0; h0 < td.ncols; h0 += 32) {
-                uint32_t v[32];
-                ptx::tmem_ld_32x32(taddr + h0, v);
-                ptx::tmem_ld_wait();
-                if (h0 + 32 >= td.ncols) {           // last chunk is in registers: hand the accumulator back
-                    ptx::tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
-                }
-                // step 1: columns (2x, 2x+1) = (re, im) of input n.  Even lane (re row) forms
-                //         Re = G[2m][2n] + G[2m+1][2n+1]; odd lane (im row) forms Im = G[2m][2n+1] - G[2m+1][2n].
-                uint32_t w[16];
+            const int u0 = td.row0 + quarter * 32;                 // first G row of this warp
+            const int h_begin = chalf * (kTileCols / 2);
+            const int h_end = td.ncols < h_begin + kTileCols / 2 ? td.ncols : h_begin + kTileCols / 2;
+            for (int kc = 0; kc < n_kchunks; ++kc) {
+                const bool reduce = prm.accumulate != 0 || kc != 0;
+                ptx::mbar_wait(tfull_bar(acc), acc_phase);
+                ptx::tc_fence_after();
+                const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + acc * kTileCols;
+                if (P == 2) {
+                    // ---- fast path: station rows are 32-byte aligned runs; bulk async store / reduce-add ----
+                    const int il = lane >> 2;                        // station within the warp's 8
+                    const int p = (lane >> 1) & 1;
+                    const int i_row = (u0 >> 2) + lane;              // lanes 0..7: the station row this lane ships
+                    // chunk kc - 1 wrote the same addresses: its bulk operations must be complete (not just read)
+                    if (kc != 0 && lane < 8) ptx::bulk_wait<0>();
+                    if (h_begin >= h_end) {                          // nothing in this column half: just release
+                        ptx::tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
+                    }
+                    for (int h0 = h_begin; h0 < h_end; h0 += kEpiCols) {
+                        if (lane < 8) ptx::bulk_wait_read<1>();      // staging[buf] (two passes ago) has been read
+                        __syncwarp();
+                        const uint32_t sbuf = stage_smem + buf * kEpiBufBytes;
 #pragma unroll
-                for (int x = 0; x < 16; ++x) {
-                    const uint32_t other = __shfl_xor_sync(0xffffffffu, v[2 * x + 1], 1);
-                    w[x] = ri ? sub_bits<C::kFloat>(other, v[2 * x]) : add_bits<C::kFloat>(v[2 * x], other);
-                }
-                // step 2: pair (Re, Im) in one lane: even lane keeps inputs n = n0 + 2y, odd lane n0 + 2y + 1.
-                const int n0 = (td.col0 + h0) >> 1;
+                        for (int half = 0; half < kEpiCols / 32; ++half) {
+                            const int hh = h0 + 32 * half;
+                            if (hh < h_end) {
+                                uint32_t v[32];
+                                ptx::tmem_ld_32x32(taddr + hh, v);
+                                ptx::tmem_ld_wait();
+                                if (hh + 32 >= h_end) {              // all of this warp's columns are in registers
+                                    ptx::tc_fence_before();
+                                    __syncwarp();
+                                    if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
+                                }
+                                uint32_t re[8], im[8];
+                                combine_chunk<C::kFloat>(v, ri, re, im);
+                                // (i, p) x (j = j0 + 8 half + y, q = ri): byte offset j*32 + p*16 + q*8 in the station row
+                                const uint32_t dst = sbuf + il * kEpiRowBytes + half * 256 + p * 16 + ri * 8;
 #pragma unroll
-                for (int y = 0; y < 8; ++y) {
-                    const uint32_t send = ri ? w[2 * y] : w[2 * y + 1];
-                    const uint32_t recv = __shfl_xor_sync(0xffffffffu, send, 1);
-                    const uint32_t re = ri ? recv : w[2 * y];
-                    const uint32_t im = ri ? w[2 * y + 1] : recv;
-                    const int n = n0 + 2 * y + ri;
-                    const int j = n / P, q = n - j * P;
-                    if (row_ok && n < prm.M && j <= i) {
-                        uint2* dst = reinterpret_cast<uint2*>(out + row_base + (static_cast<long long>(j) * P * P + q) * 2);
-                        uint2 val = make_uint2(re, im);
-                        if (prm.accumulate) {
-                            const uint2 old = *dst;
-                            val.x = add_bits<C::kFloat>(old.x, val.x);
-                            val.y = add_bits<C::kFloat>(old.y, val.y);
+                                for (int y = 0; y < 8; ++y) ptx::st_shared_v2(dst + y * 32, re[y], im[y]);
+                            }
                         }
-                        *dst = val;
+                        ptx::fence_proxy_async_smem();               // generic-proxy writes -> visible to the bulk copy
+                        __syncwarp();
+                        if (lane < 8) {
+                            const int j0 = (td.col0 + h0) >> 2;                       // first station of this pass
+                            int cnt = (h_end - h0) >> 2;                              // stations staged in this pass
+                            if (cnt > kEpiCols / 4) cnt = kEpiCols / 4;
+                            if (cnt > i_row - j0 + 1) cnt = i_row - j0 + 1;           // triangle: j <= i
+                            if (i_row < prm.n_station && cnt > 0) {
+                                uint8_t* dst = out8 + ((static_cast<long long>(c) * prm.n_baseline +
+                                                        static_cast<long long>(i_row) * (i_row + 1) / 2 + j0) << 5);
+                                const uint32_t src = sbuf + lane * kEpiRowBytes;
+                                const uint32_t bytes = static_cast<uint32_t>(cnt) << 5;
+                                if (!reduce) ptx::bulk_store(dst, src, bytes);
+                                else if constexpr (C::kFloat) ptx::bulk_reduce_add_f32(dst, src, bytes);
+                                else ptx::bulk_reduce_add_s32(dst, src, bytes);
+                            }
+                            ptx::bulk_commit();
+                        }
+                        buf ^= 1;
+                    }
+                } else {
+                    // ---- general path (n_pol == 1): per-visibility 8-byte stores ----
+                    const int m = (u0 + lane) >> 1;                  // conjugated input of this lane pair
+                    const int i = m / P, p = m - i * P;
+                    const bool row_ok = m < prm.M;
+                    // word offset of (c, b(i,0), p, q=0); b(i,j) = i(i+1)/2 + j
+                    const long long row_base =
+                        ((static_cast<long long>(c) * prm.n_baseline + static_cast<long long>(i) * (i + 1) / 2) * P + p) * P * 2;
+                    uint32_t* out = static_cast<uint32_t*>(prm.out);
+                    if (h_begin >= h_end) {
+                        ptx::tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
+                    }
+                    for (int h0 = h_begin; h0 < h_end; h0 += 32) {
+                        uint32_t v[32];
+                        ptx::tmem_ld_32x32(taddr + h0, v);
+                        ptx::tmem_ld_wait();
+                        if (h0 + 32 >= h_end) {
+                            ptx::tc_fence_before();
+                            __syncwarp();
+                            if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
+                        }
+                        uint32_t re[8], im[8];
+                        combine_chunk<C::kFloat>(v, ri, re, im);
+                        const int n0 = (td.col0 + h0) >> 1;
+#pragma unroll
+                        for (int y = 0; y < 8; ++y) {
+                            const int n = n0 + 2 * y + ri;
+                            const int j = n / P, q = n - j * P;
+                            if (row_ok && n < prm.M && j <= i) {
+                                uint2* dst = reinterpret_cast<uint2*>(out + row_base + (static_cast<long long>(j) * P * P + q) * 2);
+                                uint2 val = make_uint2(re[y], im[y]);
+                                if (reduce) {
+                                    const uint2 old = *dst;
+                                    val.x = add_bits<C::kFloat>(old.x, val.x);
+                                    val.y = add_bits<C::kFloat>(old.y, val.y);
+                                }
+                                *dst = val;
+                            }
+                        }
                     }
                 }
+                if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
             }
-            if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
         }
+        if (lane < 8) ptx::bulk_wait<0>();           // all bulk stores performed before the CTA retires
     }
 
     ptx::tc_fence_before();
