@@ -50,6 +50,8 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="cfg4")
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "single", "pair", "quad", "simt"],
+                    help="force a kernel variant (default: the library's own choice)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=0, help="steps of the host-buffer leg (default min(K, 5))")
@@ -228,7 +230,10 @@ def run_native(args):
     # every rank is an independent replica on its own seeded inputs (replicas only; no sharding)
     xs = [inputs.make_input(cfg, call=k, device="cuda") for k in range(calls)]
     h = binding.Correlator(N, P, C, T, dtype)
-    if not h.uses_tensor_cores:
+    if args.kernel != "auto":
+        h.set_kernel(args.kernel)
+    kernel = h.kernel
+    if not h.uses_tensor_cores and args.kernel != "simt":
         raise RuntimeError("workload %s does not run on the tcgen05 kernel" % cfg["name"])
     out = h.empty_output()
     # inputs smaller than L2 (126 MB) are re-read from DRAM only if L2 is flushed between steps
@@ -319,7 +324,9 @@ def run_native(args):
     roofline = {
         "bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TOPS" if dtype == "ci8" else "TFLOP/s",
         "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg["name"]),
-        "kernel": "xtc::xengine_direct_kernel<%d>" % (1 if dtype == "ci8" else 2), "kernel_ms": kernel_ms,
+        "kernel": {"single": "xtc::xengine_direct_kernel<%d>", "pair": "xtc::xengine_pair_kernel<%d, 1>",
+                   "quad": "xtc::xengine_pair_kernel<%d, 2>", "simt": "xsimt::xengine_simt_kernel<%d>"}[kernel]
+                  % (1 if dtype == "ci8" else 2), "kernel_ms": kernel_ms,
         "peak_source": "%s bf16 burst %.1f TFLOP/s x nominal %s/bf16 ratio %.0f" % (pk["source"], pk["bf16"], dtype, ratio),
         "frac_of_sustained": achieved / (pk["bf16_sustained"] * ratio),
         "frac_of_nominal": achieved / (2250.0 * ratio),

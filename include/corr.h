@@ -58,6 +58,15 @@ enum {
     CORR_FEED_CORNER_TURN = 1   /* corner-turn kernel -> channel-major, time-inner workspace (K-major) */
 };
 
+/* which kernel corr_xengine launches (corr_set_kernel); all compute the same result */
+enum {
+    CORR_KERNEL_AUTO = 0,    /* default: chosen from the geometry (see corr_get_kernel)                              */
+    CORR_KERNEL_SINGLE = 1,  /* tcgen05, one CTA per 128 x 256 tile of the per-channel Gram matrix                   */
+    CORR_KERNEL_PAIR = 2,    /* tcgen05 cta_group::2: a CTA pair per 256 x 256 tile (half the L2 bytes per MAC of B)  */
+    CORR_KERNEL_QUAD = 3,    /* two CTA pairs per 4-CTA cluster, the operand their tiles share fetched once (multicast) */
+    CORR_KERNEL_SIMT = 4     /* CUDA-core kernel for geometries TMA cannot address (and a cross-check)                */
+};
+
 /*
  * corr_create -- plan for one problem geometry on the CURRENT CUDA device (host call).
  *   n_station >= 1, n_pol in {1, 2}, n_chan >= 1, n_time >= 1, dtype in {CORR_CI8, CORR_CF16}.
@@ -109,6 +118,13 @@ const char* corr_last_error(corr_handle h);
 int corr_set_feed(corr_handle h, int feed);
 int corr_get_feed(corr_handle h);
 
+/* Force one of the CORR_KERNEL_* variants for subsequent corr_xengine calls (CORR_KERNEL_AUTO restores the
+ * default choice).  CORR_EUNSUPPORTED if the geometry / device cannot run it.  corr_get_kernel returns the
+ * kernel that WILL run (never CORR_KERNEL_AUTO): SIMT when TMA cannot address the geometry, else QUAD for
+ * 2*N*P >= 512 real components per channel, PAIR for >= 256, SINGLE below. */
+int corr_set_kernel(corr_handle h, int kernel);
+int corr_get_kernel(corr_handle h);
+
 /* Which kernel corr_xengine will launch for this geometry: 1 = tcgen05 tensor-core kernel,
  * 0 = SIMT kernel (geometries whose per-channel sample row N*P*sample_bytes is not a multiple of 16
  * bytes -- N*P not a multiple of 8 (CI8) / 4 (CF16) -- where TMA box starts would be misaligned). */
@@ -133,9 +149,12 @@ int corr_workspace_time(corr_handle h);
  * Introspection of the triangular tile schedule (host logic, no GPU work): writes up to `max_tiles`
  * entries of {row0, col0, ncols} (units: real components u = 2*m + {re:0, im:1} within a channel,
  * rows = conjugated side) for ONE channel and returns the number of tiles per channel.
- * Usable without a handle or a GPU.  `feed` selects the feeder whose schedule is reported.
+ * Usable without a handle or a GPU.  `kernel` is CORR_KERNEL_SINGLE (128-row tiles, ncols <= 256),
+ * CORR_KERNEL_PAIR (256 x 256 tiles) or CORR_KERNEL_QUAD (256 x 256 tiles in cluster order: entries 2k and
+ * 2k+1 run on the two pairs of one cluster and share their rows or their columns; ncols == 0 marks the
+ * duplicate of an odd tile out, which is computed but not written).
  */
-int corr_tile_schedule(int n_station, int n_pol, int dtype, int feed, int* tiles3, int max_tiles);
+int corr_tile_schedule(int n_station, int n_pol, int dtype, int kernel, int* tiles3, int max_tiles);
 
 /* Number of kernels launched by the last corr_xengine / corr_xengine_host call on this handle. */
 int corr_last_launch_count(corr_handle h);

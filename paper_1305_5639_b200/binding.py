@@ -14,6 +14,8 @@ LIB_PATH = os.path.join(HERE, "libcorr.so")
 CORR_CI8, CORR_CF16 = 0, 1
 CORR_OK, CORR_EINVAL, CORR_EUNSUPPORTED, CORR_ENOMEM, CORR_ECUDA, CORR_EOVERFLOW = 0, -1, -2, -3, -4, -5
 CORR_FEED_DIRECT, CORR_FEED_CORNER_TURN = 0, 1
+KERNELS = {"auto": 0, "single": 1, "pair": 2, "quad": 3, "simt": 4}      # CORR_KERNEL_*
+KERNEL_NAMES = {v: k for k, v in KERNELS.items()}
 DTYPES = {"ci8": CORR_CI8, "cf16": CORR_CF16}
 
 # name -> (restype, argtypes): every symbol include/corr.h declares
@@ -29,6 +31,8 @@ SYMBOLS = {
     "corr_last_error": (_cp, [_vp]),
     "corr_set_feed": (_i, [_vp, _i]),
     "corr_get_feed": (_i, [_vp]),
+    "corr_set_kernel": (_i, [_vp, _i]),
+    "corr_get_kernel": (_i, [_vp]),
     "corr_uses_tensor_cores": (_i, [_vp]),
     "corr_corner_turn": (_i, [_vp, _vp, _vp, _vp]),
     "corr_workspace_bytes": (_sz, [_vp]),
@@ -64,9 +68,10 @@ def baseline_index(i, j):
     return int(lib().corr_baseline_index(int(i), int(j)))
 
 
-def tile_schedule(n_station, n_pol, dtype="ci8", feed=CORR_FEED_DIRECT):
+def tile_schedule(n_station, n_pol, dtype="ci8", kernel="single"):
     """Per-channel triangular tile schedule as a list of (row0, col0, ncols); host logic only."""
     L = lib()
+    feed = KERNELS[kernel]
     n = L.corr_tile_schedule(n_station, n_pol, DTYPES[dtype], feed, None, 0)
     if n < 0:
         raise CorrError(n, "corr_tile_schedule")
@@ -118,6 +123,14 @@ class Correlator:
     @property
     def last_launch_count(self):
         return int(self._L.corr_last_launch_count(self._h))
+
+    @property
+    def kernel(self):
+        """Name of the kernel corr_xengine will launch: single / pair / quad / simt."""
+        return KERNEL_NAMES[int(self._L.corr_get_kernel(self._h))]
+
+    def set_kernel(self, kernel):
+        self._check(self._L.corr_set_kernel(self._h, KERNELS[kernel]))
 
     def set_feed(self, feed):
         self._check(self._L.corr_set_feed(self._h, int(feed)))

@@ -17,6 +17,7 @@
 #include "corner_turn.cuh"
 #include "xengine_simt.cuh"
 #include "xengine_tc.cuh"
+#include "xengine_pair.cuh"
 
 namespace {
 
@@ -43,8 +44,12 @@ struct corr_plan {
     long long t_total;     // samples integrated since the last accumulate == 0 call
     int last_launches;
 
+    int kernel;            // requested CORR_KERNEL_*
     std::vector<xtc::TileDesc> h_tiles;
     xtc::TileDesc* d_tiles;
+    std::vector<xtc::PairGroup> h_groups[2];   // [0]: one pair per cluster, [1]: two pairs per cluster (multicast)
+    xtc::PairGroup* d_groups[2];
+    int max_clusters[2];                       // co-resident clusters of 2 / 4 CTAs (cudaOccupancyMaxActiveClusters)
     EncodeTiledFn encode;
 
     CUtensorMap tmap_in;
@@ -98,6 +103,50 @@ void build_schedule_direct(int N, int P, std::vector<xtc::TileDesc>& v) {
             v.push_back(xtc::TileDesc{row0, col0, ncols, 0});
         }
     }
+}
+
+// Pair tiles of ONE channel: 256 x 256 blocks of G touching the lower station triangle, column-block major
+// (tiles of one column block are adjacent, so clusters working at the same time share operands in L2).
+void build_pair_tiles(int N, int P, std::vector<xtc::PairTile>& v) {
+    v.clear();
+    const int M2 = 2 * N * P;
+    const int R = (M2 + xtc::kPairRows - 1) / xtc::kPairRows;
+    for (int cb = 0; cb < R; ++cb)
+        for (int rb = cb; rb < R; ++rb) v.push_back(xtc::PairTile{rb * xtc::kPairRows, cb * xtc::kPairRows});
+}
+
+// Groups of ONE channel.  pairs_per_cluster == 1: one tile per group.  == 2: two tiles sharing their column
+// block (B multicast); the odd tile out of each column block lies in the last row block, and those are joined
+// two by two (A multicast); a last single tile is duplicated (computed twice, written once).
+void build_groups(int N, int P, int pairs_per_cluster, std::vector<xtc::PairGroup>& g) {
+    g.clear();
+    const int M2 = 2 * N * P;
+    const int R = (M2 + xtc::kPairRows - 1) / xtc::kPairRows;
+    if (pairs_per_cluster == 1) {
+        std::vector<xtc::PairTile> t;
+        build_pair_tiles(N, P, t);
+        for (const xtc::PairTile& x : t) g.push_back(xtc::PairGroup{{x, x}, 0, 0});
+        return;
+    }
+    std::vector<xtc::PairTile> odd;
+    for (int cb = 0; cb < R; ++cb) {
+        int rb = cb;
+        for (; rb + 1 < R; rb += 2)
+            g.push_back(xtc::PairGroup{{{rb * xtc::kPairRows, cb * xtc::kPairRows}, {(rb + 1) * xtc::kPairRows, cb * xtc::kPairRows}}, 2, 0});
+        if (rb < R) odd.push_back(xtc::PairTile{rb * xtc::kPairRows, cb * xtc::kPairRows});
+    }
+    size_t k = 0;
+    for (; k + 1 < odd.size(); k += 2) g.push_back(xtc::PairGroup{{odd[k], odd[k + 1]}, 1, 0});
+    if (k < odd.size()) g.push_back(xtc::PairGroup{{odd[k], odd[k]}, 3, 0});
+}
+
+int resolve_kernel(const corr_plan* h) {
+    if (!h->tma_ok) return CORR_KERNEL_SIMT;
+    if (h->kernel != CORR_KERNEL_AUTO) return h->kernel;
+    const int M2 = 2 * h->M;
+    if (M2 >= 512 && h->max_clusters[1] > 0) return CORR_KERNEL_QUAD;
+    if (M2 >= 256 && h->max_clusters[0] > 0) return CORR_KERNEL_PAIR;
+    return CORR_KERNEL_SINGLE;
 }
 
 size_t input_bytes(const corr_plan* h) {
@@ -160,6 +209,55 @@ int launch_direct(corr_plan* h, const void* in, void* out, int accumulate, cudaS
     return CORR_OK;
 }
 
+template <int kElt, int kPairs>
+cudaError_t launch_pair_kernel(const CUtensorMap& tmap, const xtc::PairParams& pp, unsigned clusters, cudaStream_t st) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(clusters * 2 * kPairs);
+    cfg.blockDim = dim3(xtc::kNumThreads);
+    cfg.dynamicSmemBytes = xtc::kPairSmemBytes;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = 2 * kPairs;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, xtc::xengine_pair_kernel<kElt, kPairs>, tmap, pp);
+}
+
+int launch_pair(corr_plan* h, const void* in, void* out, int accumulate, cudaStream_t st, int pairs_per_cluster) {
+    int rc = encode_input_map(h, in);
+    if (rc != CORR_OK) return rc;
+    const int v = pairs_per_cluster - 1;
+    xtc::PairParams pp;
+    pp.base.tiles = nullptr;
+    pp.base.tiles_per_chan = 0;
+    pp.base.n_tiles = 0;
+    pp.base.n_station = h->N;
+    pp.base.n_pol = h->P;
+    pp.base.n_chan = h->C;
+    pp.base.n_time = h->T;
+    pp.base.M = h->M;
+    pp.base.n_baseline = h->B;
+    pp.base.out = out;
+    pp.base.accumulate = accumulate ? 1 : 0;
+    const int kstage = h->dtype == CORR_CI8 ? xtc::Cfg<1>::kKStage : xtc::Cfg<2>::kKStage;
+    pp.base.k_chunk = h->dtype == CORR_CI8 ? (h->T + kstage - 1) / kstage * kstage : xtc::kFloatChunk;
+    pp.groups = h->d_groups[v];
+    pp.groups_per_chan = static_cast<int>(h->h_groups[v].size());
+    pp.n_groups = static_cast<long long>(pp.groups_per_chan) * h->C;
+    const unsigned clusters = static_cast<unsigned>(pp.n_groups < h->max_clusters[v] ? pp.n_groups : h->max_clusters[v]);
+    cudaError_t e;
+    if (h->dtype == CORR_CI8)
+        e = v ? launch_pair_kernel<1, 2>(h->tmap_in, pp, clusters, st) : launch_pair_kernel<1, 1>(h->tmap_in, pp, clusters, st);
+    else
+        e = v ? launch_pair_kernel<2, 2>(h->tmap_in, pp, clusters, st) : launch_pair_kernel<2, 1>(h->tmap_in, pp, clusters, st);
+    if (e != cudaSuccess) return fail_cuda(h, e, "xengine_pair_kernel launch");
+    h->last_launches += 1;
+    return CORR_OK;
+}
+
 int launch_simt(corr_plan* h, const void* in, void* out, int accumulate, cudaStream_t st) {
     xsimt::Params prm;
     prm.in = in;
@@ -215,17 +313,29 @@ long long corr_baseline_index(int i, int j) {
     return static_cast<long long>(i) * (i + 1) / 2 + j;
 }
 
-int corr_tile_schedule(int n_station, int n_pol, int dtype, int feed, int* tiles3, int max_tiles) {
+int corr_tile_schedule(int n_station, int n_pol, int dtype, int kernel, int* tiles3, int max_tiles) {
     if (!valid_geometry(n_station, n_pol, dtype) || max_tiles < 0 || (max_tiles > 0 && !tiles3)) return CORR_EINVAL;
-    if (feed != CORR_FEED_DIRECT) return CORR_EUNSUPPORTED;
-    std::vector<xtc::TileDesc> v;
-    build_schedule_direct(n_station, n_pol, v);
-    for (size_t k = 0; k < v.size() && static_cast<int>(k) < max_tiles; ++k) {
-        tiles3[3 * k + 0] = v[k].row0;
-        tiles3[3 * k + 1] = v[k].col0;
-        tiles3[3 * k + 2] = v[k].ncols;
+    std::vector<int> flat;
+    if (kernel == CORR_KERNEL_SINGLE) {
+        std::vector<xtc::TileDesc> v;
+        build_schedule_direct(n_station, n_pol, v);
+        for (const xtc::TileDesc& t : v) { flat.push_back(t.row0); flat.push_back(t.col0); flat.push_back(t.ncols); }
+    } else if (kernel == CORR_KERNEL_PAIR || kernel == CORR_KERNEL_QUAD) {
+        std::vector<xtc::PairGroup> g;
+        build_groups(n_station, n_pol, kernel == CORR_KERNEL_QUAD ? 2 : 1, g);
+        for (const xtc::PairGroup& x : g)
+            for (int k = 0; k < (kernel == CORR_KERNEL_QUAD ? 2 : 1); ++k) {
+                flat.push_back(x.t[k].row0);
+                flat.push_back(x.t[k].col0);
+                flat.push_back(k == 1 && x.share == 3 ? 0 : xtc::kTileCols);     // 0: duplicate, computed but not written
+            }
+    } else {
+        return CORR_EINVAL;
     }
-    return static_cast<int>(v.size());
+    const int n = static_cast<int>(flat.size() / 3);
+    for (int k = 0; k < n && k < max_tiles; ++k)
+        for (int q = 0; q < 3; ++q) tiles3[3 * k + q] = flat[3 * k + q];
+    return n;
 }
 
 corr_handle corr_create(int n_station, int n_pol, int n_chan, int n_time, int dtype) {
@@ -278,6 +388,9 @@ corr_handle corr_create(int n_station, int n_pol, int n_chan, int n_time, int dt
     h->t_total = 0;
     h->last_launches = 0;
     h->d_tiles = nullptr;
+    h->kernel = CORR_KERNEL_AUTO;
+    h->d_groups[0] = h->d_groups[1] = nullptr;
+    h->max_clusters[0] = h->max_clusters[1] = 0;
     h->encode = nullptr;
     h->tmap_in_ptr = nullptr;
     h->Tp = (n_time + 63) / 64 * 64;
@@ -316,6 +429,39 @@ corr_handle corr_create(int n_station, int n_pol, int n_chan, int n_time, int dt
             corr_destroy(h);
             return nullptr;
         }
+        // CTA-pair kernels: group tables and the number of co-resident clusters (the persistent grid)
+        for (int v = 0; v < 2 && e == cudaSuccess; ++v) {
+            build_groups(h->N, h->P, v + 1, h->h_groups[v]);
+            const size_t bytes = h->h_groups[v].size() * sizeof(xtc::PairGroup);
+            e = cudaMalloc(&h->d_groups[v], bytes);
+            if (e == cudaSuccess) e = cudaMemcpy(h->d_groups[v], h->h_groups[v].data(), bytes, cudaMemcpyHostToDevice);
+            const void* fn_ptr = h->dtype == CORR_CI8
+                                     ? (v ? (const void*)xtc::xengine_pair_kernel<1, 2> : (const void*)xtc::xengine_pair_kernel<1, 1>)
+                                     : (v ? (const void*)xtc::xengine_pair_kernel<2, 2> : (const void*)xtc::xengine_pair_kernel<2, 1>);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(fn_ptr, cudaFuncAttributeMaxDynamicSharedMemorySize, xtc::kPairSmemBytes);
+            if (e == cudaSuccess) {
+                cudaLaunchConfig_t cfg = {};
+                cfg.gridDim = dim3(static_cast<unsigned>(h->sm_count / (2 * (v + 1)) * (2 * (v + 1))));
+                cfg.blockDim = dim3(xtc::kNumThreads);
+                cfg.dynamicSmemBytes = xtc::kPairSmemBytes;
+                cudaLaunchAttribute at[1];
+                at[0].id = cudaLaunchAttributeClusterDimension;
+                at[0].val.clusterDim.x = 2 * (v + 1);
+                at[0].val.clusterDim.y = 1;
+                at[0].val.clusterDim.z = 1;
+                cfg.attrs = at;
+                cfg.numAttrs = 1;
+                int n = 0;
+                if (cudaOccupancyMaxActiveClusters(&n, fn_ptr, &cfg) == cudaSuccess) h->max_clusters[v] = n;
+                else cudaGetLastError();          // pair kernels unavailable: resolve_kernel falls back
+            }
+        }
+        if (e != cudaSuccess) {
+            fail(nullptr, e == cudaErrorMemoryAllocation ? CORR_ENOMEM : CORR_ECUDA, "corr_create: pair kernel setup: %s",
+                 cudaGetErrorString(e));
+            corr_destroy(h);
+            return nullptr;
+        }
     }
     return h;
 }
@@ -323,6 +469,8 @@ corr_handle corr_create(int n_station, int n_pol, int n_chan, int n_time, int dt
 void corr_destroy(corr_handle h) {
     if (!h) return;
     if (h->d_tiles) cudaFree(h->d_tiles);
+    if (h->d_groups[0]) cudaFree(h->d_groups[0]);
+    if (h->d_groups[1]) cudaFree(h->d_groups[1]);
     if (h->d_ws) cudaFree(h->d_ws);
     if (h->d_in_stage) cudaFree(h->d_in_stage);
     if (h->d_out_stage) cudaFree(h->d_out_stage);
@@ -336,7 +484,20 @@ size_t corr_workspace_bytes(corr_handle h) { return h ? workspace_bytes(h) : 0; 
 int corr_workspace_time(corr_handle h) { return h ? h->Tp : 0; }
 const char* corr_last_error(corr_handle h) { return h ? h->err : g_create_error; }
 int corr_get_feed(corr_handle h) { return h ? h->feed : CORR_EINVAL; }
-int corr_uses_tensor_cores(corr_handle h) { return h ? (h->tma_ok ? 1 : 0) : CORR_EINVAL; }
+int corr_uses_tensor_cores(corr_handle h) { return h ? (resolve_kernel(h) != CORR_KERNEL_SIMT ? 1 : 0) : CORR_EINVAL; }
+int corr_get_kernel(corr_handle h) { return h ? resolve_kernel(h) : CORR_EINVAL; }
+
+int corr_set_kernel(corr_handle h, int kernel) {
+    if (!h) return CORR_EINVAL;
+    if (kernel < CORR_KERNEL_AUTO || kernel > CORR_KERNEL_SIMT) return fail(h, CORR_EINVAL, "corr_set_kernel: unknown kernel %d", kernel);
+    if (kernel != CORR_KERNEL_AUTO && kernel != CORR_KERNEL_SIMT && !h->tma_ok)
+        return fail(h, CORR_EUNSUPPORTED, "corr_set_kernel: per-channel row of %lld B is not a multiple of 16, only the SIMT kernel applies",
+                    static_cast<long long>(h->M) * h->sample_bytes);
+    if ((kernel == CORR_KERNEL_PAIR && h->max_clusters[0] <= 0) || (kernel == CORR_KERNEL_QUAD && h->max_clusters[1] <= 0))
+        return fail(h, CORR_EUNSUPPORTED, "corr_set_kernel: no co-resident clusters for kernel %d on this device", kernel);
+    h->kernel = kernel;
+    return CORR_OK;
+}
 int corr_last_launch_count(corr_handle h) { return h ? h->last_launches : CORR_EINVAL; }
 
 int corr_set_feed(corr_handle h, int feed) {
@@ -374,10 +535,12 @@ int corr_xengine(corr_handle h, const void* in, void* out, int accumulate, void*
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     h->last_launches = 0;
     int rc;
-    if (h->tma_ok && !getenv("CORR_FORCE_SIMT"))
-        rc = launch_direct(h, in, out, accumulate, st);
-    else
-        rc = launch_simt(h, in, out, accumulate, st);
+    switch (resolve_kernel(h)) {
+        case CORR_KERNEL_QUAD: rc = launch_pair(h, in, out, accumulate, st, 2); break;
+        case CORR_KERNEL_PAIR: rc = launch_pair(h, in, out, accumulate, st, 1); break;
+        case CORR_KERNEL_SINGLE: rc = launch_direct(h, in, out, accumulate, st); break;
+        default: rc = launch_simt(h, in, out, accumulate, st); break;
+    }
     if (rc == CORR_OK) h->t_total = t_next;
     return rc;
 }

@@ -1,0 +1,240 @@
+// xengine_pair.cuh -- the X-engine HERK on CTA PAIRS (tcgen05 cta_group::2) with optional TMA multicast
+// between two pairs of a 4-CTA cluster.  Same mathematics and same direct feed as xengine_tc.cuh
+// (Sec. 2 Eq. 2; lower station triangle incl. autocorrelations PAPER.md:79, 144).
+//
+// Why (profiles/r1a_cfg4_ncu_1cta_kernel.md): with 128 x 256 tiles per CTA every time sample costs
+// 128 + 256 operand bytes from L2 per 32768 MACs, and at config 4 that is 15 GB of L2 -> SM traffic per
+// call = the L2 slice throughput cap; the tensor pipe idles 60 % of the time.  A CTA pair computes a
+// 256 x 256 tile of G with one M = 256 instruction: each CTA holds 128 rows of A and only HALF of B's
+// columns (the hardware feeds both halves to both tensor cores), so a sample costs 128 + 128 bytes per CTA
+// for the same 32768 MACs (and half the shared-memory operand reads).  Two pairs that work on tiles of one
+// channel sharing a column block (or a row block) form a 4-CTA cluster and fetch the shared operand ONCE
+// with a multicast TMA load: 128 + 64 bytes per CTA and sample.
+//
+// Roles per CTA (320 threads, one CTA per SM, persistent; both CTAs of a pair walk the same tile list):
+//   warp 0      TMA producer (one lane): its 128 A rows and its 128 B columns of every pipeline stage; completion
+//               bytes of both CTAs are counted on the pair LEADER's `full` barrier
+//   warp 1      TMEM allocator (both CTAs) + tcgen05.mma.cta_group::2 issuer (one lane of the leader CTA);
+//               tcgen05.commit multicasts the `empty` (all CTAs of the cluster) and `tmem full` (the pair) arrivals
+//   warps 2..9  epilogue of this CTA's 128 TMEM lanes (drain_accumulator in xengine_tc.cuh); they release the
+//               accumulator by arriving on the leader's `tmem empty` barrier through shared::cluster
+#pragma once
+#include "xengine_tc.cuh"
+
+namespace xtc {
+
+constexpr int kPairRows = 256;                 // G rows per pair tile
+constexpr int kPairStageBytes = 16 * 1024;     // per CTA and stage: A 128 components + B 128 components, KSTAGE samples
+constexpr int kPairStages = 9;
+constexpr int kPairSmemBytes = kPairStages * kPairStageBytes + kEpiBytes + 1024 /*alignment slack*/ + 256 /*barriers*/;
+static_assert(kPairSmemBytes <= 227 * 1024, "shared memory");
+
+struct PairTile {
+    int row0;   // first G row    (multiple of 256), real components u within the channel
+    int col0;   // first G column (multiple of 256)
+};
+// Work item of one cluster: one tile per pair, all of the same channel.
+struct PairGroup {
+    PairTile t[2];
+    int share;   // bit 0: both tiles have the same rows (A multicast), bit 1: the same columns (B multicast);
+                 // 3: t[1] duplicates t[0] (odd tile out) and is computed but not written
+    int pad;
+};
+
+struct PairParams {
+    Params base;                 // geometry, output, accumulate, k_chunk (tiles/tiles_per_chan/n_tiles unused)
+    const PairGroup* groups;     // DEVICE: per-channel group table
+    int groups_per_chan;
+    long long n_groups;          // groups_per_chan * n_chan
+};
+
+template <int kElt, int kPairs>
+__global__ void __launch_bounds__(kNumThreads, 1)
+xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const PairParams pp) {
+    using C = Cfg<kElt>;
+    const Params& prm = pp.base;
+    constexpr int kChunkElems = 128 / kElt;                 // u per 128-byte chunk
+    constexpr int kChunkBytes = C::kKStage * 128;           // one TMA box: [KSTAGE rows][128 B]
+    constexpr int kOpChunks = 128 / kChunkElems;            // chunks per operand and CTA: 1 (ci8) / 2 (cf16)
+    constexpr int kKStepBytes = C::kMmaK * 128;
+    constexpr int kKSteps = C::kKStage / C::kMmaK;
+    static_assert(2 * kOpChunks * kChunkBytes == kPairStageBytes, "stage size");
+    // M = 256 (16 << 24), N = 256 (32 << 17); formats and MN-major bits as for the 1-CTA kernel
+    constexpr uint32_t kIdesc = (C::kIdesc & ~(0x1fu << 24)) | (16u << 24) | (32u << 17);
+    constexpr uint16_t kAllMask = static_cast<uint16_t>((1u << (2 * kPairs)) - 1u);
+
+    extern __shared__ uint8_t smem_raw[];
+    // the SAME offsets in every CTA of the cluster (multicast and cta_group::2 address by offset): the dynamic
+    // shared memory window starts at the same offset in all CTAs of a launch, so the rounding is identical
+    const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t epi_base = smem_base + kPairStages * kPairStageBytes;
+    const uint32_t bar_base = epi_base + kEpiBytes;
+    auto full_bar = [&](int s) { return bar_base + 8u * s; };
+    auto empty_bar = [&](int s) { return bar_base + 8u * (kPairStages + s); };
+    auto tfull_bar = [&](int a) { return bar_base + 8u * (2 * kPairStages + a); };
+    auto tempty_bar = [&](int a) { return bar_base + 8u * (2 * kPairStages + 2 + a); };
+    const uint32_t tmem_slot = bar_base + 8u * (2 * kPairStages + 4);
+    uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - ptx::smem_u32(smem_raw)));
+
+    const int warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+    const uint32_t rank = ptx::cluster_ctarank();          // 0 .. 2 kPairs - 1
+    const int pair = static_cast<int>(rank >> 1);
+    const int half = static_cast<int>(rank & 1u);          // 0 = pair leader (issues the MMAs)
+    const uint16_t pair_mask = static_cast<uint16_t>(3u << (2 * pair));
+    const long long cluster_id = ptx::cluster_id_x();
+    const long long n_clusters = ptx::cluster_count_x();
+
+    if (threadIdx.x == 0) {
+        ptx::prefetch_tensormap(&tmap_in);
+        for (int s = 0; s < kPairStages; ++s) {
+            ptx::mbar_init(full_bar(s), 1);                  // leader: its own arrive.expect_tx
+            ptx::mbar_init(empty_bar(s), kPairs);            // one tcgen05.commit arrival per pair of the cluster
+        }
+        for (int a = 0; a < 2; ++a) {
+            ptx::mbar_init(tfull_bar(a), 1);
+            ptx::mbar_init(tempty_bar(a), 2 * kNumEpiWarps); // leader: every epilogue warp of both CTAs
+        }
+        ptx::fence_mbar_init();
+    }
+    if (warp == 1) {
+        ptx::tmem_alloc_pair(tmem_slot, 512);
+        ptx::tmem_relinquish_pair();
+    }
+    ptx::tc_fence_before();
+    ptx::cluster_sync();                 // barriers of every CTA initialised before anyone signals them
+    ptx::tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    const int num_kb = (prm.n_time + C::kKStage - 1) / C::kKStage;
+    const int kb_per_chunk = prm.k_chunk / C::kKStage;
+    const int n_kchunks = (num_kb + kb_per_chunk - 1) / kb_per_chunk;
+    const int M2 = 2 * prm.M;
+
+    if (warp == 0) {
+        // ===================== TMA producer =====================
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            for (long long g = cluster_id; g < pp.n_groups; g += n_clusters) {
+                const int c = static_cast<int>(g / pp.groups_per_chan);
+                const PairGroup gd = pp.groups[g - static_cast<long long>(c) * pp.groups_per_chan];
+                const PairTile td = (kPairs == 2 && pair == 1) ? gd.t[1] : gd.t[0];
+                const int w_a = c * M2 + td.row0 + 128 * half;      // this CTA's A rows in the [T][C*2M] view
+                const int w_b = c * M2 + td.col0 + 128 * half;      // this CTA's half of the B columns
+                // a shared operand is fetched once, by pair 0's CTA, and multicast to the same-half CTA of pair 1
+                const bool mc_a = kPairs == 2 && (gd.share & 1);
+                const bool mc_b = kPairs == 2 && (gd.share & 2);
+                const uint16_t mc_mask = static_cast<uint16_t>((1u << half) | (4u << half));
+                for (int kb = 0; kb < num_kb; ++kb) {
+                    ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
+                    const uint32_t sa = smem_base + stage * kPairStageBytes;
+                    const uint32_t sb = sa + kOpChunks * kChunkBytes;
+                    if (half == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), 2u * kPairStageBytes);
+#pragma unroll
+                    for (int ch = 0; ch < kOpChunks; ++ch) {
+                        if (!mc_a)
+                            ptx::tma_load_2d_pair(sa + ch * kChunkBytes, &tmap_in, full_bar(stage),
+                                                  w_a + ch * kChunkElems, kb * C::kKStage);
+                        else if (pair == 0)
+                            ptx::tma_load_2d_pair_mc(sa + ch * kChunkBytes, &tmap_in, full_bar(stage),
+                                                     w_a + ch * kChunkElems, kb * C::kKStage, mc_mask);
+                    }
+#pragma unroll
+                    for (int ch = 0; ch < kOpChunks; ++ch) {
+                        if (!mc_b)
+                            ptx::tma_load_2d_pair(sb + ch * kChunkBytes, &tmap_in, full_bar(stage),
+                                                  w_b + ch * kChunkElems, kb * C::kKStage);
+                        else if (pair == 0)
+                            ptx::tma_load_2d_pair_mc(sb + ch * kChunkBytes, &tmap_in, full_bar(stage),
+                                                     w_b + ch * kChunkElems, kb * C::kKStage, mc_mask);
+                    }
+                    if (++stage == kPairStages) { stage = 0; phase ^= 1u; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===================== MMA issuer (pair leader only) =====================
+        if (lane == 0 && half == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            int acc = 0;
+            uint32_t acc_phase = 0;
+            for (long long g = cluster_id; g < pp.n_groups; g += n_clusters) {
+                for (int kb0 = 0; kb0 < num_kb; kb0 += kb_per_chunk) {
+                    const int kb1 = kb0 + kb_per_chunk < num_kb ? kb0 + kb_per_chunk : num_kb;
+                    const uint32_t d_tmem = tmem_base + acc * kTileCols;
+                    ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1u);     // both CTAs' epilogues have drained it
+                    ptx::tc_fence_after();
+                    for (int kb = kb0; kb < kb1; ++kb) {
+                        ptx::mbar_wait(full_bar(stage), phase);          // both CTAs' operand bytes have landed
+                        ptx::tc_fence_after();
+                        const uint32_t sa = smem_base + stage * kPairStageBytes;
+                        const uint32_t sb = sa + kOpChunks * kChunkBytes;
+#pragma unroll
+                        for (int k = 0; k < kKSteps; ++k) {
+                            const uint64_t adesc = ptx::smem_desc_sw128(sa + k * kKStepBytes, kChunkBytes, 1024);
+                            const uint64_t bdesc = ptx::smem_desc_sw128(sb + k * kKStepBytes, kChunkBytes, 1024);
+                            const uint32_t accum = (kb != kb0 || k != 0) ? 1u : 0u;
+                            if constexpr (C::kFloat) ptx::mma_f16_pair(d_tmem, adesc, bdesc, kIdesc, accum);
+                            else ptx::mma_i8_pair(d_tmem, adesc, bdesc, kIdesc, accum);
+                        }
+                        ptx::mma_commit_pair_mc(empty_bar(stage), kAllMask);   // slot free in every CTA that fills it
+                        if (++stage == kPairStages) { stage = 0; phase ^= 1u; }
+                    }
+                    ptx::mma_commit_pair_mc(tfull_bar(acc), pair_mask);        // accumulator complete in both CTAs
+                    if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+                }
+            }
+        }
+    } else {
+        // ===================== epilogue: this CTA's 128 rows of the pair tile =====================
+        const int ew = warp - 2;
+        const int quarter = warp & 3;                // TMEM lanes [32*quarter, 32*quarter+32) belong to this warp
+        const int chalf = ew >> 2;                   // column half of the tile handled by this warp
+        const uint32_t stage_smem = epi_base + ew * kEpiWarpBytes;
+        const uint32_t leader = rank & ~1u;
+        int acc = 0;
+        uint32_t acc_phase = 0;
+        int buf = 0;
+        for (long long g = cluster_id; g < pp.n_groups; g += n_clusters) {
+            const int c = static_cast<int>(g / pp.groups_per_chan);
+            const PairGroup gd = pp.groups[g - static_cast<long long>(c) * pp.groups_per_chan];
+            const PairTile td = (kPairs == 2 && pair == 1) ? gd.t[1] : gd.t[0];
+            const int r0 = td.row0 + 128 * half;                   // first G row of this CTA
+            const int u0 = r0 + quarter * 32;                      // first G row of this warp
+            // columns this CTA's rows need: up to the last station of its rows (s_j <= s_i), none for rows past the
+            // channel's 2M components or for the duplicate tile of an odd group
+            int need = 0;
+            if (r0 < M2 && !(kPairs == 2 && pair == 1 && gd.share == 3)) {
+                int i_max = (r0 + 127) / (2 * prm.n_pol);
+                if (i_max > prm.n_station - 1) i_max = prm.n_station - 1;
+                need = (i_max + 1) * 2 * prm.n_pol - td.col0;
+                if (need > kTileCols) need = kTileCols;
+                if (need < 0) need = 0;
+            }
+            const int h_begin = chalf * (kTileCols / 2);
+            const int h_end = need < h_begin + kTileCols / 2 ? need : h_begin + kTileCols / 2;
+            for (int kc = 0; kc < n_kchunks; ++kc) {
+                const bool reduce = prm.accumulate != 0 || kc != 0;
+                ptx::mbar_wait(tfull_bar(acc), acc_phase);
+                ptx::tc_fence_after();
+                const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + acc * kTileCols;
+                drain_accumulator<C::kFloat, true>(prm, c, u0, td.col0, h_begin, h_end, taddr,
+                                                   ptx::mapa(tempty_bar(acc), leader), reduce, kc == 0, stage_smem, buf, lane);
+                if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+            }
+        }
+        if (lane < 8) ptx::bulk_wait<0>();           // all bulk stores performed before the CTA retires
+    }
+
+    // no CTA may exit (or free TMEM) while a peer can still signal its barriers or read its operands
+    ptx::tc_fence_before();
+    ptx::cluster_sync();
+    if (warp == 1) {
+        ptx::tc_fence_after();
+        ptx::tmem_dealloc_pair(tmem_base, 512);
+    }
+}
+
+}  // namespace xtc

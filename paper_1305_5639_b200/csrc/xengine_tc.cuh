@@ -114,6 +114,126 @@ __device__ __forceinline__ void combine_chunk(const uint32_t (&v)[32], int ri, u
     }
 }
 
+// Drain one TMEM accumulator pass of one tile through this epilogue warp: tcgen05.ld -> Re/Im combine ->
+// packed-baseline writer (+ accumulate).  The warp owns TMEM lanes [32 quarter, +32) = G rows u0 .. u0 + 31 of
+// channel c and the tile columns [h_begin, h_end) (G columns col0 + h); `taddr` addresses lane 32 quarter,
+// column 0 of the accumulator.  `release_bar` is arrived on (by lane 0; `kRemote`: it lives in the pair leader
+// CTA and is a shared::cluster address) as soon as the warp's last TMEM column is in registers.
+// first_pass: no earlier pass of this tile wrote the same output addresses (else wait for those writes).
+template <bool kFloat, bool kRemote>
+__device__ __forceinline__ void drain_accumulator(const Params& prm, int c, int u0, int col0, int h_begin, int h_end,
+                                                  uint32_t taddr, uint32_t release_bar, bool reduce, bool first_pass,
+                                                  uint32_t stage_smem, int& buf, int lane) {
+    auto release = [](uint32_t bar) {
+        if constexpr (kRemote) ptx::mbar_arrive_cluster(bar);
+        else ptx::mbar_arrive(bar);
+    };
+    const int P = prm.n_pol;
+    const int ri = lane & 1;                     // row parity: 0 = re row (u even), 1 = im row
+    uint8_t* out8 = static_cast<uint8_t*>(prm.out);
+    struct { int col0; } td{col0};
+    const int kc = first_pass ? 0 : 1;
+    if (P == 2) {
+        // ---- fast path: station rows are 32-byte aligned runs; bulk async store / reduce-add ----
+        const int il = lane >> 2;                        // station within the warp's 8
+        const int p = (lane >> 1) & 1;
+        const int i_row = (u0 >> 2) + lane;              // lanes 0..7: the station row this lane ships
+        // chunk kc - 1 wrote the same addresses: its bulk operations must be complete (not just read)
+        if (kc != 0 && lane < 8) ptx::bulk_wait<0>();
+        if (h_begin >= h_end) {                          // nothing in this column half: just release
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) release(release_bar);
+        }
+        for (int h0 = h_begin; h0 < h_end; h0 += kEpiCols) {
+            if (lane < 8) ptx::bulk_wait_read<1>();      // staging[buf] (two passes ago) has been read
+            __syncwarp();
+            const uint32_t sbuf = stage_smem + buf * kEpiBufBytes;
+#pragma unroll
+            for (int half = 0; half < kEpiCols / 32; ++half) {
+                const int hh = h0 + 32 * half;
+                if (hh < h_end) {
+                    uint32_t v[32];
+                    ptx::tmem_ld_32x32(taddr + hh, v);
+                    ptx::tmem_ld_wait();
+                    if (hh + 32 >= h_end) {              // all of this warp's columns are in registers
+                        ptx::tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) release(release_bar);
+                    }
+                    uint32_t re[8], im[8];
+                    combine_chunk<kFloat>(v, ri, re, im);
+                    // (i, p) x (j = j0 + 8 half + y, q = ri): byte offset j*32 + p*16 + q*8 in the station row
+                    const uint32_t dst = sbuf + il * kEpiRowBytes + half * 256 + p * 16 + ri * 8;
+#pragma unroll
+                    for (int y = 0; y < 8; ++y) ptx::st_shared_v2(dst + y * 32, re[y], im[y]);
+                }
+            }
+            ptx::fence_proxy_async_smem();               // generic-proxy writes -> visible to the bulk copy
+            __syncwarp();
+            if (lane < 8) {
+                const int j0 = (td.col0 + h0) >> 2;                       // first station of this pass
+                int cnt = (h_end - h0) >> 2;                              // stations staged in this pass
+                if (cnt > kEpiCols / 4) cnt = kEpiCols / 4;
+                if (cnt > i_row - j0 + 1) cnt = i_row - j0 + 1;           // triangle: j <= i
+                if (i_row < prm.n_station && cnt > 0) {
+                    uint8_t* dst = out8 + ((static_cast<long long>(c) * prm.n_baseline +
+                                            static_cast<long long>(i_row) * (i_row + 1) / 2 + j0) << 5);
+                    const uint32_t src = sbuf + lane * kEpiRowBytes;
+                    const uint32_t bytes = static_cast<uint32_t>(cnt) << 5;
+                    if (!reduce) ptx::bulk_store(dst, src, bytes);
+                    else if constexpr (kFloat) ptx::bulk_reduce_add_f32(dst, src, bytes);
+                    else ptx::bulk_reduce_add_s32(dst, src, bytes);
+                }
+                ptx::bulk_commit();
+            }
+            buf ^= 1;
+        }
+    } else {
+        // ---- general path (n_pol == 1): per-visibility 8-byte stores ----
+        const int m = (u0 + lane) >> 1;                  // conjugated input of this lane pair
+        const int i = m / P, p = m - i * P;
+        const bool row_ok = m < prm.M;
+        // word offset of (c, b(i,0), p, q=0); b(i,j) = i(i+1)/2 + j
+        const long long row_base =
+            ((static_cast<long long>(c) * prm.n_baseline + static_cast<long long>(i) * (i + 1) / 2) * P + p) * P * 2;
+        uint32_t* out = static_cast<uint32_t*>(prm.out);
+        if (h_begin >= h_end) {
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) release(release_bar);
+        }
+        for (int h0 = h_begin; h0 < h_end; h0 += 32) {
+            uint32_t v[32];
+            ptx::tmem_ld_32x32(taddr + h0, v);
+            ptx::tmem_ld_wait();
+            if (h0 + 32 >= h_end) {
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) release(release_bar);
+            }
+            uint32_t re[8], im[8];
+            combine_chunk<kFloat>(v, ri, re, im);
+            const int n0 = (td.col0 + h0) >> 1;
+#pragma unroll
+            for (int y = 0; y < 8; ++y) {
+                const int n = n0 + 2 * y + ri;
+                const int j = n / P, q = n - j * P;
+                if (row_ok && n < prm.M && j <= i) {
+                    uint2* dst = reinterpret_cast<uint2*>(out + row_base + (static_cast<long long>(j) * P * P + q) * 2);
+                    uint2 val = make_uint2(re[y], im[y]);
+                    if (reduce) {
+                        const uint2 old = *dst;
+                        val.x = add_bits<kFloat>(old.x, val.x);
+                        val.y = add_bits<kFloat>(old.y, val.y);
+                    }
+                    *dst = val;
+                }
+            }
+        }
+    }
+}
+
 template <int kElt>
 __global__ void __launch_bounds__(kNumThreads, 1)
 xengine_direct_kernel(const __grid_constant__ CUtensorMap tmap_in, const Params prm) {
@@ -241,10 +361,7 @@ xengine_direct_kernel(const __grid_constant__ CUtensorMap tmap_in, const Params 
         const int ew = warp - 2;
         const int quarter = warp & 3;                // TMEM lanes [32*quarter, 32*quarter+32) belong to this warp
         const int chalf = ew >> 2;                   // column half of the tile handled by this warp
-        const int ri = lane & 1;                     // row parity: 0 = re row (u even), 1 = im row
-        const int P = prm.n_pol;
         const uint32_t stage_smem = epi_base + ew * kEpiWarpBytes;
-        uint8_t* out8 = static_cast<uint8_t*>(prm.out);
         int acc = 0;
         uint32_t acc_phase = 0;
         int buf = 0;
@@ -259,105 +376,8 @@ xengine_direct_kernel(const __grid_constant__ CUtensorMap tmap_in, const Params 
                 ptx::mbar_wait(tfull_bar(acc), acc_phase);
                 ptx::tc_fence_after();
                 const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + acc * kTileCols;
-                if (P == 2) {
-                    // ---- fast path: station rows are 32-byte aligned runs; bulk async store / reduce-add ----
-                    const int il = lane >> 2;                        // station within the warp's 8
-                    const int p = (lane >> 1) & 1;
-                    const int i_row = (u0 >> 2) + lane;              // lanes 0..7: the station row this lane ships
-                    // chunk kc - 1 wrote the same addresses: its bulk operations must be complete (not just read)
-                    if (kc != 0 && lane < 8) ptx::bulk_wait<0>();
-                    if (h_begin >= h_end) {                          // nothing in this column half: just release
-                        ptx::tc_fence_before();
-                        __syncwarp();
-                        if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
-                    }
-                    for (int h0 = h_begin; h0 < h_end; h0 += kEpiCols) {
-                        if (lane < 8) ptx::bulk_wait_read<1>();      // staging[buf] (two passes ago) has been read
-                        __syncwarp();
-                        const uint32_t sbuf = stage_smem + buf * kEpiBufBytes;
-#pragma unroll
-                        for (int half = 0; half < kEpiCols / 32; ++half) {
-                            const int hh = h0 + 32 * half;
-                            if (hh < h_end) {
-                                uint32_t v[32];
-                                ptx::tmem_ld_32x32(taddr + hh, v);
-                                ptx::tmem_ld_wait();
-                                if (hh + 32 >= h_end) {              // all of this warp's columns are in registers
-                                    ptx::tc_fence_before();
-                                    __syncwarp();
-                                    if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
-                                }
-                                uint32_t re[8], im[8];
-                                combine_chunk<C::kFloat>(v, ri, re, im);
-                                // (i, p) x (j = j0 + 8 half + y, q = ri): byte offset j*32 + p*16 + q*8 in the station row
-                                const uint32_t dst = sbuf + il * kEpiRowBytes + half * 256 + p * 16 + ri * 8;
-#pragma unroll
-                                for (int y = 0; y < 8; ++y) ptx::st_shared_v2(dst + y * 32, re[y], im[y]);
-                            }
-                        }
-                        ptx::fence_proxy_async_smem();               // generic-proxy writes -> visible to the bulk copy
-                        __syncwarp();
-                        if (lane < 8) {
-                            const int j0 = (td.col0 + h0) >> 2;                       // first station of this pass
-                            int cnt = (h_end - h0) >> 2;                              // stations staged in this pass
-                            if (cnt > kEpiCols / 4) cnt = kEpiCols / 4;
-                            if (cnt > i_row - j0 + 1) cnt = i_row - j0 + 1;           // triangle: j <= i
-                            if (i_row < prm.n_station && cnt > 0) {
-                                uint8_t* dst = out8 + ((static_cast<long long>(c) * prm.n_baseline +
-                                                        static_cast<long long>(i_row) * (i_row + 1) / 2 + j0) << 5);
-                                const uint32_t src = sbuf + lane * kEpiRowBytes;
-                                const uint32_t bytes = static_cast<uint32_t>(cnt) << 5;
-                                if (!reduce) ptx::bulk_store(dst, src, bytes);
-                                else if constexpr (C::kFloat) ptx::bulk_reduce_add_f32(dst, src, bytes);
-                                else ptx::bulk_reduce_add_s32(dst, src, bytes);
-                            }
-                            ptx::bulk_commit();
-                        }
-                        buf ^= 1;
-                    }
-                } else {
-                    // ---- general path (n_pol == 1): per-visibility 8-byte stores ----
-                    const int m = (u0 + lane) >> 1;                  // conjugated input of this lane pair
-                    const int i = m / P, p = m - i * P;
-                    const bool row_ok = m < prm.M;
-                    // word offset of (c, b(i,0), p, q=0); b(i,j) = i(i+1)/2 + j
-                    const long long row_base =
-                        ((static_cast<long long>(c) * prm.n_baseline + static_cast<long long>(i) * (i + 1) / 2) * P + p) * P * 2;
-                    uint32_t* out = static_cast<uint32_t*>(prm.out);
-                    if (h_begin >= h_end) {
-                        ptx::tc_fence_before();
-                        __syncwarp();
-                        if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
-                    }
-                    for (int h0 = h_begin; h0 < h_end; h0 += 32) {
-                        uint32_t v[32];
-                        ptx::tmem_ld_32x32(taddr + h0, v);
-                        ptx::tmem_ld_wait();
-                        if (h0 + 32 >= h_end) {
-                            ptx::tc_fence_before();
-                            __syncwarp();
-                            if (lane == 0) ptx::mbar_arrive(tempty_bar(acc));
-                        }
-                        uint32_t re[8], im[8];
-                        combine_chunk<C::kFloat>(v, ri, re, im);
-                        const int n0 = (td.col0 + h0) >> 1;
-#pragma unroll
-                        for (int y = 0; y < 8; ++y) {
-                            const int n = n0 + 2 * y + ri;
-                            const int j = n / P, q = n - j * P;
-                            if (row_ok && n < prm.M && j <= i) {
-                                uint2* dst = reinterpret_cast<uint2*>(out + row_base + (static_cast<long long>(j) * P * P + q) * 2);
-                                uint2 val = make_uint2(re[y], im[y]);
-                                if (reduce) {
-                                    const uint2 old = *dst;
-                                    val.x = add_bits<C::kFloat>(old.x, val.x);
-                                    val.y = add_bits<C::kFloat>(old.y, val.y);
-                                }
-                                *dst = val;
-                            }
-                        }
-                    }
-                }
+                drain_accumulator<C::kFloat, false>(prm, c, u0, td.col0, h_begin, h_end, taddr, tempty_bar(acc), reduce,
+                                                    kc == 0, stage_smem, buf, lane);
                 if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
             }
         }

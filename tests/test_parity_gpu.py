@@ -27,10 +27,13 @@ def corr():
     return binding
 
 
-def run_gpu(corr, xs, dtype, accumulate_calls=True, host=False):
+def run_gpu(corr, xs, dtype, accumulate_calls=True, host=False, kernel=None):
     """xs: list of input tensors (one per call).  Returns the int32/fp32 output as numpy."""
     T, C, N, P, _ = xs[0].shape
     with corr.Correlator(N, P, C, T, dtype) as h:
+        if kernel is not None:
+            h.set_kernel(kernel)
+            assert h.kernel == kernel
         if host:
             out = torch.empty(h.output_shape(), dtype=torch.int32 if dtype == "ci8" else torch.float32)
             for k, x in enumerate(xs):
@@ -95,6 +98,30 @@ def test_ci8_bit_exact_small(corr, oracle, N, P, C, T):
     got, tc = run_gpu(corr, [x], "ci8")
     assert tc == ((N * P * 2) % 16 == 0)
     assert_bit_exact(got, run_oracle(oracle, [x]))
+
+
+# every tensor-core kernel variant on geometries that span ragged pair tiles, several row / column blocks,
+# odd group counts (duplicate tile of the quad kernel), ragged T and both polarisation counts
+KERNEL_CASES = [(16, 2, 5, 100), (64, 2, 9, 200), (72, 2, 3, 130), (96, 2, 4, 64), (128, 2, 5, 257),
+                (136, 1, 3, 96), (200, 2, 2, 128), (256, 2, 3, 192), (320, 2, 2, 64)]
+
+
+@pytest.mark.parametrize("kernel", ["single", "pair", "quad", "simt"])
+@pytest.mark.parametrize("N,P,C,T", KERNEL_CASES)
+def test_ci8_bit_exact_every_kernel(corr, oracle, kernel, N, P, C, T):
+    x = inputs.gauss_ci8(T, C, N, P, 40.0, seed=7100 + N + T)
+    got, _ = run_gpu(corr, [x, x], "ci8", kernel=kernel)          # two calls: store, then reduce-add
+    want = run_oracle(oracle, [x, x])
+    assert_bit_exact(got, want)
+
+
+@pytest.mark.parametrize("kernel", ["single", "pair", "quad", "simt"])
+@pytest.mark.parametrize("N,P,C,T", [(24, 2, 3, 100), (64, 2, 3, 1100), (96, 1, 2, 64), (160, 2, 2, 2100)])
+def test_cf16_within_tolerance_every_kernel(corr, oracle, kernel, N, P, C, T):
+    x = inputs.corr_phase_cf16(T, C, N, P, seed=7200 + N)
+    got, _ = run_gpu(corr, [x], "cf16", kernel=kernel)
+    err = fp16_normalised_error(got, run_oracle(oracle, [x]), N, P)
+    assert err <= FP16_TOL, "normalised error %.3g" % err
 
 
 def test_ci8_full_range_including_minus_128(corr, oracle):
