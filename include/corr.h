@@ -120,8 +120,8 @@ int corr_get_feed(corr_handle h);
 
 /* Force one of the CORR_KERNEL_* variants for subsequent corr_xengine calls (CORR_KERNEL_AUTO restores the
  * default choice).  CORR_EUNSUPPORTED if the geometry / device cannot run it.  corr_get_kernel returns the
- * kernel that WILL run (never CORR_KERNEL_AUTO): SIMT when TMA cannot address the geometry, else QUAD for
- * 2*N*P >= 512 real components per channel, PAIR for >= 256, SINGLE below. */
+ * kernel that WILL run (never CORR_KERNEL_AUTO): SIMT when TMA cannot address the geometry, else PAIR for
+ * 2*N*P >= 256 real components per channel, SINGLE below (QUAD only on request: it measured slower). */
 int corr_set_kernel(corr_handle h, int kernel);
 int corr_get_kernel(corr_handle h);
 

@@ -49,6 +49,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     cmd = [_nvcc()] + NVCC_FLAGS + ["-I", INCLUDE]
     if verbose:
         cmd += ["-Xptxas", "-v"]
+    if os.environ.get("CORR_STATS"):          # developer build: per-role stall counters (clock64) in the pair kernel
+        cmd += ["-DCORR_STATS"]
     cmd += _sources() + ["-o", LIB + ".tmp"]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if res.returncode != 0:

@@ -144,7 +144,8 @@ int resolve_kernel(const corr_plan* h) {
     if (!h->tma_ok) return CORR_KERNEL_SIMT;
     if (h->kernel != CORR_KERNEL_AUTO) return h->kernel;
     const int M2 = 2 * h->M;
-    if (M2 >= 512 && h->max_clusters[1] > 0) return CORR_KERNEL_QUAD;
+    // CORR_KERNEL_QUAD (multicast between two pairs) is never chosen: measured 12 % slower than PAIR at config 4
+    // (profiles/): the multicast saves L2 reads but not delivered bytes, and couples the two pairs' pipelines
     if (M2 >= 256 && h->max_clusters[0] > 0) return CORR_KERNEL_PAIR;
     return CORR_KERNEL_SINGLE;
 }
@@ -244,6 +245,12 @@ int launch_pair(corr_plan* h, const void* in, void* out, int accumulate, cudaStr
     pp.base.accumulate = accumulate ? 1 : 0;
     const int kstage = h->dtype == CORR_CI8 ? xtc::Cfg<1>::kKStage : xtc::Cfg<2>::kKStage;
     pp.base.k_chunk = h->dtype == CORR_CI8 ? (h->T + kstage - 1) / kstage * kstage : xtc::kFloatChunk;
+#ifdef CORR_STATS
+    static unsigned long long* d_stats = nullptr;
+    if (!d_stats) cudaMalloc(&d_stats, 8 * 160 * sizeof(unsigned long long));
+    cudaMemsetAsync(d_stats, 0, 8 * 160 * sizeof(unsigned long long), st);
+    pp.base.stats = d_stats;
+#endif
     pp.groups = h->d_groups[v];
     pp.groups_per_chan = static_cast<int>(h->h_groups[v].size());
     pp.n_groups = static_cast<long long>(pp.groups_per_chan) * h->C;
@@ -254,6 +261,20 @@ int launch_pair(corr_plan* h, const void* in, void* out, int accumulate, cudaStr
     else
         e = v ? launch_pair_kernel<2, 2>(h->tmap_in, pp, clusters, st) : launch_pair_kernel<2, 1>(h->tmap_in, pp, clusters, st);
     if (e != cudaSuccess) return fail_cuda(h, e, "xengine_pair_kernel launch");
+#ifdef CORR_STATS
+    if (getenv("CORR_STATS_PRINT")) {
+        static unsigned long long hs[8 * 160];
+        cudaStreamSynchronize(st);
+        cudaMemcpy(hs, d_stats, sizeof(hs), cudaMemcpyDeviceToHost);
+        const int nb = static_cast<int>(clusters) * 2 * pairs_per_cluster;
+        double a[8] = {0};
+        for (int b = 0; b < nb; ++b) for (int k = 0; k < 8; ++k) a[k] += static_cast<double>(hs[b * 8 + k]) / nb;
+        double lead_tempty = 0, lead_full = 0;
+        for (int b = 0; b < nb; b += 2) { lead_tempty += hs[b * 8 + 2] / (nb / 2.0); lead_full += hs[b * 8 + 3] / (nb / 2.0); }
+        fprintf(stderr, "[corr stats] clk/CTA: total %.0f | producer wait empty %.0f | mma wait tmem-empty %.0f, wait full %.0f | epi(warp2) wait tmem-full %.0f, drain %.0f\n",
+                a[0], a[1], lead_tempty, lead_full, a[4], a[5]);
+    }
+#endif
     h->last_launches += 1;
     return CORR_OK;
 }

@@ -24,9 +24,15 @@
 namespace xtc {
 
 constexpr int kPairRows = 256;                 // G rows per pair tile
-constexpr int kPairStageBytes = 16 * 1024;     // per CTA and stage: A 128 components + B 128 components, KSTAGE samples
-constexpr int kPairStages = 9;
-constexpr int kPairSmemBytes = kPairStages * kPairStageBytes + kEpiBytes + 1024 /*alignment slack*/ + 256 /*barriers*/;
+constexpr int kPairBoxes = 2;                  // TMA boxes (of Cfg::kKStage samples) stacked along time per pipeline stage
+constexpr int kPairStageBytes = kPairBoxes * 16 * 1024;   // per CTA and stage: A 128 components + B 128 components
+constexpr int kPairEpiBufs = 1;                // staging buffers per epilogue warp
+constexpr int kPairEpiWarpBytes = kPairEpiBufs * kEpiBufBytes;
+constexpr int kPairEpiBytes = kNumEpiWarps * kPairEpiWarpBytes;
+constexpr int kPairStages = 6;
+// the dynamic shared memory window of a kernel without static shared memory starts 1024-byte aligned (checked
+// in the kernel), so no alignment slack is reserved
+constexpr int kPairSmemBytes = kPairStages * kPairStageBytes + kPairEpiBytes + 256 /*barriers*/;
 static_assert(kPairSmemBytes <= 227 * 1024, "shared memory");
 
 struct PairTile {
@@ -54,10 +60,13 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const PairParam
     using C = Cfg<kElt>;
     const Params& prm = pp.base;
     constexpr int kChunkElems = 128 / kElt;                 // u per 128-byte chunk
-    constexpr int kChunkBytes = C::kKStage * 128;           // one TMA box: [KSTAGE rows][128 B]
+    constexpr int kBoxRows = C::kKStage;                    // one TMA box: [kBoxRows samples][128 B]
+    constexpr int kBoxBytes = kBoxRows * 128;
+    constexpr int kStageK = kPairBoxes * kBoxRows;          // samples per pipeline stage
+    constexpr int kChunkBytes = kStageK * 128;              // one 128-byte-wide chunk of a stage (boxes stacked along K)
     constexpr int kOpChunks = 128 / kChunkElems;            // chunks per operand and CTA: 1 (ci8) / 2 (cf16)
     constexpr int kKStepBytes = C::kMmaK * 128;
-    constexpr int kKSteps = C::kKStage / C::kMmaK;
+    constexpr int kKSteps = kStageK / C::kMmaK;
     static_assert(2 * kOpChunks * kChunkBytes == kPairStageBytes, "stage size");
     // M = 256 (16 << 24), N = 256 (32 << 17); formats and MN-major bits as for the 1-CTA kernel
     constexpr uint32_t kIdesc = (C::kIdesc & ~(0x1fu << 24)) | (16u << 24) | (32u << 17);
@@ -66,9 +75,10 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const PairParam
     extern __shared__ uint8_t smem_raw[];
     // the SAME offsets in every CTA of the cluster (multicast and cta_group::2 address by offset): the dynamic
     // shared memory window starts at the same offset in all CTAs of a launch, so the rounding is identical
-    const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t smem_base = ptx::smem_u32(smem_raw);
+    if (smem_base & 1023u) __trap();
     const uint32_t epi_base = smem_base + kPairStages * kPairStageBytes;
-    const uint32_t bar_base = epi_base + kEpiBytes;
+    const uint32_t bar_base = epi_base + kPairEpiBytes;
     auto full_bar = [&](int s) { return bar_base + 8u * s; };
     auto empty_bar = [&](int s) { return bar_base + 8u * (kPairStages + s); };
     auto tfull_bar = [&](int a) { return bar_base + 8u * (2 * kPairStages + a); };
@@ -106,8 +116,8 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const PairParam
     ptx::tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
 
-    const int num_kb = (prm.n_time + C::kKStage - 1) / C::kKStage;
-    const int kb_per_chunk = prm.k_chunk / C::kKStage;
+    const int num_kb = (prm.n_time + kStageK - 1) / kStageK;
+    const int kb_per_chunk = prm.k_chunk / kStageK > 0 ? prm.k_chunk / kStageK : 1;
     const int n_kchunks = (num_kb + kb_per_chunk - 1) / kb_per_chunk;
     const int M2 = 2 * prm.M;
 
@@ -116,6 +126,8 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const PairParam
         if (lane == 0) {
             int stage = 0;
             uint32_t phase = 0;
+            [[maybe_unused]] long long st_empty = 0;
+            [[maybe_unused]] const long long st_begin = clock64();
             for (long long g = cluster_id; g < pp.n_groups; g += n_clusters) {
                 const int c = static_cast<int>(g / pp.groups_per_chan);
                 const PairGroup gd = pp.groups[g - static_cast<long long>(c) * pp.groups_per_chan];
@@ -125,33 +137,51 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const PairParam
                 // a shared operand is fetched once, by pair 0's CTA, and multicast to the same-half CTA of pair 1
                 const bool mc_a = kPairs == 2 && (gd.share & 1);
                 const bool mc_b = kPairs == 2 && (gd.share & 2);
+                // diagonal tile: this CTA's half of the B columns IS its 128 A rows -> one load serves both operands
+                const bool diag = kPairs == 1 && td.row0 == td.col0;
                 const uint16_t mc_mask = static_cast<uint16_t>((1u << half) | (4u << half));
                 for (int kb = 0; kb < num_kb; ++kb) {
-                    ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
+                    {
+                        CORR_STAT_T0();
+                        ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
+                        CORR_STAT_ADD(st_empty);
+                    }
                     const uint32_t sa = smem_base + stage * kPairStageBytes;
                     const uint32_t sb = sa + kOpChunks * kChunkBytes;
-                    if (half == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), 2u * kPairStageBytes);
+                    if (half == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), diag ? kPairStageBytes : 2u * kPairStageBytes);
 #pragma unroll
-                    for (int ch = 0; ch < kOpChunks; ++ch) {
-                        if (!mc_a)
-                            ptx::tma_load_2d_pair(sa + ch * kChunkBytes, &tmap_in, full_bar(stage),
-                                                  w_a + ch * kChunkElems, kb * C::kKStage);
-                        else if (pair == 0)
-                            ptx::tma_load_2d_pair_mc(sa + ch * kChunkBytes, &tmap_in, full_bar(stage),
-                                                     w_a + ch * kChunkElems, kb * C::kKStage, mc_mask);
+                    for (int ch = 0; ch < kOpChunks; ++ch)
+#pragma unroll
+                        for (int b = 0; b < kPairBoxes; ++b) {
+                            if (!mc_a)
+                                ptx::tma_load_2d_pair(sa + ch * kChunkBytes + b * kBoxBytes, &tmap_in, full_bar(stage),
+                                                      w_a + ch * kChunkElems, kb * kStageK + b * kBoxRows);
+                            else if (pair == 0)
+                                ptx::tma_load_2d_pair_mc(sa + ch * kChunkBytes + b * kBoxBytes, &tmap_in, full_bar(stage),
+                                                         w_a + ch * kChunkElems, kb * kStageK + b * kBoxRows, mc_mask);
+                        }
+                    if (diag) {
+                        if (++stage == kPairStages) { stage = 0; phase ^= 1u; }
+                        continue;
                     }
 #pragma unroll
-                    for (int ch = 0; ch < kOpChunks; ++ch) {
-                        if (!mc_b)
-                            ptx::tma_load_2d_pair(sb + ch * kChunkBytes, &tmap_in, full_bar(stage),
-                                                  w_b + ch * kChunkElems, kb * C::kKStage);
-                        else if (pair == 0)
-                            ptx::tma_load_2d_pair_mc(sb + ch * kChunkBytes, &tmap_in, full_bar(stage),
-                                                     w_b + ch * kChunkElems, kb * C::kKStage, mc_mask);
-                    }
+                    for (int ch = 0; ch < kOpChunks; ++ch)
+#pragma unroll
+                        for (int b = 0; b < kPairBoxes; ++b) {
+                            if (!mc_b)
+                                ptx::tma_load_2d_pair(sb + ch * kChunkBytes + b * kBoxBytes, &tmap_in, full_bar(stage),
+                                                      w_b + ch * kChunkElems, kb * kStageK + b * kBoxRows);
+                            else if (pair == 0)
+                                ptx::tma_load_2d_pair_mc(sb + ch * kChunkBytes + b * kBoxBytes, &tmap_in, full_bar(stage),
+                                                         w_b + ch * kChunkElems, kb * kStageK + b * kBoxRows, mc_mask);
+                        }
                     if (++stage == kPairStages) { stage = 0; phase ^= 1u; }
                 }
             }
+#ifdef CORR_STATS
+            prm.stats[blockIdx.x * 8 + 0] = clock64() - st_begin;
+            prm.stats[blockIdx.x * 8 + 1] = st_empty;
+#endif
         }
     } else if (warp == 1) {
         // ===================== MMA issuer (pair leader only) =====================
@@ -160,17 +190,28 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const PairParam
             uint32_t phase = 0;
             int acc = 0;
             uint32_t acc_phase = 0;
+            [[maybe_unused]] long long st_tempty = 0, st_full = 0;
             for (long long g = cluster_id; g < pp.n_groups; g += n_clusters) {
+                const PairGroup gd = pp.groups[g % pp.groups_per_chan];
+                const bool diag = kPairs == 1 && gd.t[0].row0 == gd.t[0].col0;      // B operand = the A buffer
                 for (int kb0 = 0; kb0 < num_kb; kb0 += kb_per_chunk) {
                     const int kb1 = kb0 + kb_per_chunk < num_kb ? kb0 + kb_per_chunk : num_kb;
                     const uint32_t d_tmem = tmem_base + acc * kTileCols;
-                    ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1u);     // both CTAs' epilogues have drained it
+                    {
+                        CORR_STAT_T0();
+                        ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1u);     // both CTAs' epilogues have drained it
+                        CORR_STAT_ADD(st_tempty);
+                    }
                     ptx::tc_fence_after();
                     for (int kb = kb0; kb < kb1; ++kb) {
-                        ptx::mbar_wait(full_bar(stage), phase);          // both CTAs' operand bytes have landed
+                        {
+                            CORR_STAT_T0();
+                            ptx::mbar_wait(full_bar(stage), phase);          // both CTAs' operand bytes have landed
+                            CORR_STAT_ADD(st_full);
+                        }
                         ptx::tc_fence_after();
                         const uint32_t sa = smem_base + stage * kPairStageBytes;
-                        const uint32_t sb = sa + kOpChunks * kChunkBytes;
+                        const uint32_t sb = diag ? sa : sa + kOpChunks * kChunkBytes;
 #pragma unroll
                         for (int k = 0; k < kKSteps; ++k) {
                             const uint64_t adesc = ptx::smem_desc_sw128(sa + k * kKStepBytes, kChunkBytes, 1024);
@@ -186,17 +227,22 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const PairParam
                     if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
                 }
             }
+#ifdef CORR_STATS
+            prm.stats[blockIdx.x * 8 + 2] = st_tempty;
+            prm.stats[blockIdx.x * 8 + 3] = st_full;
+#endif
         }
     } else {
         // ===================== epilogue: this CTA's 128 rows of the pair tile =====================
         const int ew = warp - 2;
         const int quarter = warp & 3;                // TMEM lanes [32*quarter, 32*quarter+32) belong to this warp
         const int chalf = ew >> 2;                   // column half of the tile handled by this warp
-        const uint32_t stage_smem = epi_base + ew * kEpiWarpBytes;
+        const uint32_t stage_smem = epi_base + ew * kPairEpiWarpBytes;
         const uint32_t leader = rank & ~1u;
         int acc = 0;
         uint32_t acc_phase = 0;
         int buf = 0;
+        [[maybe_unused]] long long st_tfull = 0, st_drain = 0;
         for (long long g = cluster_id; g < pp.n_groups; g += n_clusters) {
             const int c = static_cast<int>(g / pp.groups_per_chan);
             const PairGroup gd = pp.groups[g - static_cast<long long>(c) * pp.groups_per_chan];
@@ -217,15 +263,29 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const PairParam
             const int h_end = need < h_begin + kTileCols / 2 ? need : h_begin + kTileCols / 2;
             for (int kc = 0; kc < n_kchunks; ++kc) {
                 const bool reduce = prm.accumulate != 0 || kc != 0;
-                ptx::mbar_wait(tfull_bar(acc), acc_phase);
+                {
+                    CORR_STAT_T0();
+                    ptx::mbar_wait(tfull_bar(acc), acc_phase);
+                    CORR_STAT_ADD(st_tfull);
+                }
                 ptx::tc_fence_after();
                 const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + acc * kTileCols;
-                drain_accumulator<C::kFloat, true>(prm, c, u0, td.col0, h_begin, h_end, taddr,
-                                                   ptx::mapa(tempty_bar(acc), leader), reduce, kc == 0, stage_smem, buf, lane);
+                {
+                    CORR_STAT_T0();
+                    drain_accumulator<C::kFloat, true, kPairEpiBufs>(prm, c, u0, td.col0, h_begin, h_end, taddr,
+                                                       ptx::mapa(tempty_bar(acc), leader), reduce, kc == 0, stage_smem, buf, lane);
+                    CORR_STAT_ADD(st_drain);
+                }
                 if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
             }
         }
         if (lane < 8) ptx::bulk_wait<0>();           // all bulk stores performed before the CTA retires
+#ifdef CORR_STATS
+        if (warp == 2 && lane == 0) {
+            prm.stats[blockIdx.x * 8 + 4] = st_tfull;
+            prm.stats[blockIdx.x * 8 + 5] = st_drain;
+        }
+#endif
     }
 
     // no CTA may exit (or free TMEM) while a peer can still signal its barriers or read its operands

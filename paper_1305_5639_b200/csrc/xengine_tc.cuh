@@ -65,7 +65,18 @@ struct Params {
     void* out;               // DEVICE: packed output
     int accumulate;
     int k_chunk;             // samples per TMEM accumulation pass (multiple of the pipeline stage)
+#ifdef CORR_STATS
+    unsigned long long* stats;   // DEVICE, 8 counters per CTA (developer build only: python -m ...build with CORR_STATS=1)
+#endif
 };
+
+#ifdef CORR_STATS
+#define CORR_STAT_T0() const long long stat_t0_ = clock64()
+#define CORR_STAT_ADD(var) (var) += clock64() - stat_t0_
+#else
+#define CORR_STAT_T0() do {} while (0)
+#define CORR_STAT_ADD(var) do {} while (0)
+#endif
 
 template <int kElt> struct Cfg;
 template <> struct Cfg<1> {                      // complex int8 -> int32
@@ -120,7 +131,7 @@ __device__ __forceinline__ void combine_chunk(const uint32_t (&v)[32], int ri, u
 // column 0 of the accumulator.  `release_bar` is arrived on (by lane 0; `kRemote`: it lives in the pair leader
 // CTA and is a shared::cluster address) as soon as the warp's last TMEM column is in registers.
 // first_pass: no earlier pass of this tile wrote the same output addresses (else wait for those writes).
-template <bool kFloat, bool kRemote>
+template <bool kFloat, bool kRemote, int kBufs = 2>
 __device__ __forceinline__ void drain_accumulator(const Params& prm, int c, int u0, int col0, int h_begin, int h_end,
                                                   uint32_t taddr, uint32_t release_bar, bool reduce, bool first_pass,
                                                   uint32_t stage_smem, int& buf, int lane) {
@@ -146,7 +157,7 @@ __device__ __forceinline__ void drain_accumulator(const Params& prm, int c, int 
             if (lane == 0) release(release_bar);
         }
         for (int h0 = h_begin; h0 < h_end; h0 += kEpiCols) {
-            if (lane < 8) ptx::bulk_wait_read<1>();      // staging[buf] (two passes ago) has been read
+            if (lane < 8) ptx::bulk_wait_read<kBufs - 1>();   // staging[buf] (kBufs passes ago) has been read
             __syncwarp();
             const uint32_t sbuf = stage_smem + buf * kEpiBufBytes;
 #pragma unroll
@@ -187,7 +198,7 @@ __device__ __forceinline__ void drain_accumulator(const Params& prm, int c, int 
                 }
                 ptx::bulk_commit();
             }
-            buf ^= 1;
+            if (kBufs == 2) buf ^= 1;
         }
     } else {
         // ---- general path (n_pol == 1): per-visibility 8-byte stores ----
