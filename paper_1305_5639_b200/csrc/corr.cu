@@ -52,7 +52,8 @@ struct corr_plan {
     int max_clusters[2];                       // co-resident clusters of 2 / 4 CTAs (cudaOccupancyMaxActiveClusters)
     EncodeTiledFn encode;
 
-    CUtensorMap tmap_in;
+    CUtensorMap tmap_in;     // 1-CTA kernel: box [128 B][Cfg::kKStage samples]
+    CUtensorMap tmap_pair;   // pair kernels: box [128 B][kPairStageK / kPairBoxes samples]
     const void* tmap_in_ptr;
 
     // corner-turn feed
@@ -173,9 +174,14 @@ int encode_input_map(corr_plan* h, const void* in) {
                                  2, const_cast<void*>(in), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                                  CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) {
+    cuuint32_t box2[2] = {box[0], static_cast<cuuint32_t>((elt == 1 ? xtc::kPairStageK<1> : xtc::kPairStageK<2>) / xtc::kPairBoxes)};
+    const CUresult r2 = r != CUDA_SUCCESS ? r :
+        h->encode(&h->tmap_pair, elt == 1 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16,
+                  2, const_cast<void*>(in), dims, strides, box2, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                  CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r2 != CUDA_SUCCESS) {
         h->tmap_in_ptr = nullptr;
-        return fail(h, CORR_ECUDA, "cuTensorMapEncodeTiled(in) failed with CUresult %d", static_cast<int>(r));
+        return fail(h, CORR_ECUDA, "cuTensorMapEncodeTiled(in) failed with CUresult %d", static_cast<int>(r2));
     }
     h->tmap_in_ptr = in;
     return CORR_OK;
@@ -243,8 +249,7 @@ int launch_pair(corr_plan* h, const void* in, void* out, int accumulate, cudaStr
     pp.base.n_baseline = h->B;
     pp.base.out = out;
     pp.base.accumulate = accumulate ? 1 : 0;
-    const int kstage = h->dtype == CORR_CI8 ? xtc::Cfg<1>::kKStage : xtc::Cfg<2>::kKStage;
-    pp.base.k_chunk = h->dtype == CORR_CI8 ? (h->T + kstage - 1) / kstage * kstage : xtc::kFloatChunk;
+    pp.base.k_chunk = h->dtype == CORR_CI8 ? (1 << 30) : xtc::kFloatChunk;      // int32 sums are exact: one pass
 #ifdef CORR_STATS
     static unsigned long long* d_stats = nullptr;
     if (!d_stats) cudaMalloc(&d_stats, 8 * 160 * sizeof(unsigned long long));
@@ -257,9 +262,9 @@ int launch_pair(corr_plan* h, const void* in, void* out, int accumulate, cudaStr
     const unsigned clusters = static_cast<unsigned>(pp.n_groups < h->max_clusters[v] ? pp.n_groups : h->max_clusters[v]);
     cudaError_t e;
     if (h->dtype == CORR_CI8)
-        e = v ? launch_pair_kernel<1, 2>(h->tmap_in, pp, clusters, st) : launch_pair_kernel<1, 1>(h->tmap_in, pp, clusters, st);
+        e = v ? launch_pair_kernel<1, 2>(h->tmap_pair, pp, clusters, st) : launch_pair_kernel<1, 1>(h->tmap_pair, pp, clusters, st);
     else
-        e = v ? launch_pair_kernel<2, 2>(h->tmap_in, pp, clusters, st) : launch_pair_kernel<2, 1>(h->tmap_in, pp, clusters, st);
+        e = v ? launch_pair_kernel<2, 2>(h->tmap_pair, pp, clusters, st) : launch_pair_kernel<2, 1>(h->tmap_pair, pp, clusters, st);
     if (e != cudaSuccess) return fail_cuda(h, e, "xengine_pair_kernel launch");
 #ifdef CORR_STATS
     if (getenv("CORR_STATS_PRINT")) {

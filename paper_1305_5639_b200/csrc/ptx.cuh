@@ -72,19 +72,27 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst_smem, const CUtensorMap
 // ---- bulk async copies shared -> global (TMA unit, no tensor map) -------------------------
 // `bytes` is a multiple of 16; both addresses are 16-byte aligned.  Completion is tracked per issuing
 // thread in bulk groups (commit / wait).
-__device__ __forceinline__ void bulk_store(void* dst_gmem, uint32_t src_smem, uint32_t bytes) {
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem), "r"(src_smem), "r"(bytes)
+// L2 eviction policy for data touched once (the packed output): evict first, so that it does not push the
+// input tiles other CTAs are about to re-read out of L2
+__device__ __forceinline__ uint64_t policy_evict_first() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void bulk_store(void* dst_gmem, uint32_t src_smem, uint32_t bytes, uint64_t policy) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;" ::"l"(dst_gmem),
+                 "r"(src_smem), "r"(bytes), "l"(policy)
                  : "memory");
 }
 // dst[k] += src[k] performed by the memory system (L2), element type s32 / f32.
-__device__ __forceinline__ void bulk_reduce_add_s32(void* dst_gmem, uint32_t src_smem, uint32_t bytes) {
-    asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.s32 [%0], [%1], %2;" ::"l"(dst_gmem),
-                 "r"(src_smem), "r"(bytes)
+__device__ __forceinline__ void bulk_reduce_add_s32(void* dst_gmem, uint32_t src_smem, uint32_t bytes, uint64_t policy) {
+    asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.L2::cache_hint.add.s32 [%0], [%1], %2, %3;" ::"l"(dst_gmem),
+                 "r"(src_smem), "r"(bytes), "l"(policy)
                  : "memory");
 }
-__device__ __forceinline__ void bulk_reduce_add_f32(void* dst_gmem, uint32_t src_smem, uint32_t bytes) {
-    asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f32 [%0], [%1], %2;" ::"l"(dst_gmem),
-                 "r"(src_smem), "r"(bytes)
+__device__ __forceinline__ void bulk_reduce_add_f32(void* dst_gmem, uint32_t src_smem, uint32_t bytes, uint64_t policy) {
+    asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.L2::cache_hint.add.f32 [%0], [%1], %2, %3;" ::"l"(dst_gmem),
+                 "r"(src_smem), "r"(bytes), "l"(policy)
                  : "memory");
 }
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }

@@ -24,8 +24,9 @@
 namespace xtc {
 
 constexpr int kPairRows = 256;                 // G rows per pair tile
-constexpr int kPairBoxes = 2;                  // TMA boxes (of Cfg::kKStage samples) stacked along time per pipeline stage
-constexpr int kPairStageBytes = kPairBoxes * 16 * 1024;   // per CTA and stage: A 128 components + B 128 components
+constexpr int kPairBoxes = 1;                  // TMA boxes stacked along time per 128-byte chunk of a pipeline stage
+constexpr int kPairStageBytes = 32 * 1024;     // per CTA and stage: A 128 components + B 128 components, kPairStageK samples
+template <int kElt> constexpr int kPairStageK = kPairStageBytes / (2 * 128 * kElt);    // 128 (ci8) / 64 (cf16) samples
 constexpr int kPairEpiBufs = 1;                // staging buffers per epilogue warp
 constexpr int kPairEpiWarpBytes = kPairEpiBufs * kEpiBufBytes;
 constexpr int kPairEpiBytes = kNumEpiWarps * kPairEpiWarpBytes;
@@ -60,9 +61,9 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const PairParam
     using C = Cfg<kElt>;
     const Params& prm = pp.base;
     constexpr int kChunkElems = 128 / kElt;                 // u per 128-byte chunk
-    constexpr int kBoxRows = C::kKStage;                    // one TMA box: [kBoxRows samples][128 B]
+    constexpr int kStageK = kPairStageK<kElt>;              // samples per pipeline stage
+    constexpr int kBoxRows = kStageK / kPairBoxes;          // one TMA box: [kBoxRows samples][128 B] (tmap_pair)
     constexpr int kBoxBytes = kBoxRows * 128;
-    constexpr int kStageK = kPairBoxes * kBoxRows;          // samples per pipeline stage
     constexpr int kChunkBytes = kStageK * 128;              // one 128-byte-wide chunk of a stage (boxes stacked along K)
     constexpr int kOpChunks = 128 / kChunkElems;            // chunks per operand and CTA: 1 (ci8) / 2 (cf16)
     constexpr int kKStepBytes = C::kMmaK * 128;

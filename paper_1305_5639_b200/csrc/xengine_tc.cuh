@@ -144,6 +144,7 @@ __device__ __forceinline__ void drain_accumulator(const Params& prm, int c, int 
     uint8_t* out8 = static_cast<uint8_t*>(prm.out);
     struct { int col0; } td{col0};
     const int kc = first_pass ? 0 : 1;
+    const uint64_t policy = ptx::policy_evict_first();
     if (P == 2) {
         // ---- fast path: station rows are 32-byte aligned runs; bulk async store / reduce-add ----
         const int il = lane >> 2;                        // station within the warp's 8
@@ -192,9 +193,9 @@ __device__ __forceinline__ void drain_accumulator(const Params& prm, int c, int 
                                             static_cast<long long>(i_row) * (i_row + 1) / 2 + j0) << 5);
                     const uint32_t src = sbuf + lane * kEpiRowBytes;
                     const uint32_t bytes = static_cast<uint32_t>(cnt) << 5;
-                    if (!reduce) ptx::bulk_store(dst, src, bytes);
-                    else if constexpr (kFloat) ptx::bulk_reduce_add_f32(dst, src, bytes);
-                    else ptx::bulk_reduce_add_s32(dst, src, bytes);
+                    if (!reduce) ptx::bulk_store(dst, src, bytes, policy);
+                    else if constexpr (kFloat) ptx::bulk_reduce_add_f32(dst, src, bytes, policy);
+                    else ptx::bulk_reduce_add_s32(dst, src, bytes, policy);
                 }
                 ptx::bulk_commit();
             }
