@@ -40,7 +40,10 @@ FALLBACK_BF16_TFLOPS = 1590.0                  # B200_PROFILING.md fallback
 FALLBACK_HBM_GBS = 6650.0
 # DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum) of ONE xengine_direct_kernel launch from
 # the committed `ncu --set full` capture of this workload (profiles/), or None where not captured.
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {
+    # profiles/r1b_cfg4_ncu_pair_kernel.md: 4.09 GB (accumulate = 0) and 5.08 GB (accumulate = 1) -> mean of the step's 4 calls
+    "cfg4": (4.086e9 + 3 * 5.078e9) / 4,
+}
 
 
 def parse_args():
@@ -52,6 +55,8 @@ def parse_args():
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
     ap.add_argument("--kernel", default="auto", choices=["auto", "single", "pair", "quad", "simt"],
                     help="force a kernel variant (default: the library's own choice)")
+    ap.add_argument("--piece", default="xengine", choices=["xengine", "corner_turn"],
+                    help="corner_turn: time the standalone corner-turn kernel (SURVEY 8(a) a1) on the workload's input")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-gemm-peak", action="store_true",
@@ -237,6 +242,54 @@ def describe(cfg):
                                                     "int32" if cfg["dtype"] == "ci8" else "fp32"))
 
 
+def max_over_ranks(value, dist=None, world=1, device="cpu"):
+    """MAX over all ranks of a per-rank scalar (the contract's timing reduction); identity at world == 1."""
+    import torch
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(units_per_rank_step, steps, world, total_ms):
+    """Whole-job throughput: the units ALL ranks processed (replicas: world x the same count) / the slowest rank's time."""
+    return world * steps * units_per_rank_step / (total_ms * 1e-3)
+
+
+# ------------------------------------------------------------------------------------------------
+# piece (a): the standalone corner-turn kernel, HBM-bound (read in + write two planes)
+# ------------------------------------------------------------------------------------------------
+def run_corner_turn(args):
+    import torch
+    from paper_1305_5639_b200 import binding, inputs
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device")
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    cfg = workload(args.workload)
+    pk = peaks()
+    x = inputs.make_input(cfg, call=0, device="cuda")
+    h = binding.Correlator(cfg["N"], cfg["P"], cfg["C"], cfg["T"], cfg["dtype"])
+    ws = torch.empty((h.workspace_bytes,), dtype=torch.uint8, device="cuda")
+    K, W = args.steps, max(args.warmup, 3)
+    for _ in range(W):
+        h.corner_turn(x, ws)
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    for a, b in ev:
+        a.record(); h.corner_turn(x, ws); b.record()
+    torch.cuda.synchronize()
+    ms = sum(a.elapsed_time(b) for a, b in ev) / K
+    nbytes = cfg["in_bytes"] + h.workspace_bytes          # read the input once, write ws and ws_rot
+    gbs = nbytes / (ms * 1e-3) / 1e9
+    print(json.dumps({"metric": "corner_turn_gbs", "value": gbs, "unit": "GB/s", "n_gpus": 1, "steps": K, "warmup": W,
+                      "ms_per_step": ms, "higher_is_better": True, "dtype": "u8", "data": "synthetic",
+                      "config": {"workload": describe(cfg), "l2": "input + workspace (%.0f MiB) larger than L2" % (nbytes / 2 ** 20)},
+                      "gpu_launches": K,
+                      "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s", "frac": gbs / pk["hbm"],
+                                   "traffic": None, "kernel": "cturn::corner_turn_kernel", "kernel_ms": ms,
+                                   "algorithmic_bytes_per_launch": nbytes}}), flush=True)
+
+
 # ------------------------------------------------------------------------------------------------
 # native arm
 # ------------------------------------------------------------------------------------------------
@@ -313,12 +366,9 @@ def run_native(args):
     call_ms = [evs[s][2 * k].elapsed_time(evs[s][2 * k + 1]) for s in range(K) for k in range(calls)]
     step_ms = [sum(call_ms[s * calls:(s + 1) * calls]) for s in range(K)]
     total_ms = sum(step_ms)          # device time of exactly K steps (flush kernels excluded)
-    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, dist, world, "cuda")
     ops_step = cfg["ops_per_call"] * calls
-    value = world * K * ops_step / (total_ms * 1e-3) / 1e12
+    value = whole_job_value(ops_step, K, world, total_ms) / 1e12
     kernel_ms = sum(call_ms) / len(call_ms)          # average launch duration of the dominant (only) kernel
 
     # ---- e2e: HOST pinned buffers through corr_xengine_host --------------------------------------
@@ -414,6 +464,8 @@ def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.piece == "corner_turn":
+        run_corner_turn(args)
     else:
         run_native(args)
 

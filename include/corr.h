@@ -52,12 +52,6 @@ enum {
     CORR_EOVERFLOW = -5      /* CORR_CI8: integration would exceed the exact int32 range         */
 };
 
-/* operand feeder of the tensor-core kernel (corr_set_feed) */
-enum {
-    CORR_FEED_DIRECT = 0,       /* default: TMA reads `in` in place as MN-major operands (no staging)  */
-    CORR_FEED_CORNER_TURN = 1   /* corner-turn kernel -> channel-major, time-inner workspace (K-major) */
-};
-
 /* which kernel corr_xengine launches (corr_set_kernel); all compute the same result */
 enum {
     CORR_KERNEL_AUTO = 0,    /* default: chosen from the geometry (see corr_get_kernel)                              */
@@ -113,11 +107,6 @@ long long corr_baseline_index(int i, int j); /* i(i+1)/2 + j for 0 <= j <= i, el
  * thread).  The string is owned by the library and valid until the next call on the same handle. */
 const char* corr_last_error(corr_handle h);
 
-/* Choose the operand feeder for subsequent corr_xengine calls (see enum above).  The corner-turn
- * feeder allocates its workspace (corr_workspace_bytes) on first use. */
-int corr_set_feed(corr_handle h, int feed);
-int corr_get_feed(corr_handle h);
-
 /* Force one of the CORR_KERNEL_* variants for subsequent corr_xengine calls (CORR_KERNEL_AUTO restores the
  * default choice).  CORR_EUNSUPPORTED if the geometry / device cannot run it.  corr_get_kernel returns the
  * kernel that WILL run (never CORR_KERNEL_AUTO): SIMT when TMA cannot address the geometry, else PAIR for
@@ -139,7 +128,7 @@ int corr_uses_tensor_cores(corr_handle h);
  *   in      DEVICE pointer as for corr_xengine.
  *   ws      DEVICE pointer, corr_workspace_bytes(h) bytes, 128-byte aligned: the two planes,
  *           ws then ws_rot, each n_chan * M * corr_workspace_time(h) samples.
- * Asynchronous on `stream`.  corr_xengine with CORR_FEED_CORNER_TURN runs this internally.
+ * Asynchronous on `stream`.  corr_xengine does NOT run it: its TMA feed reads `in` in place.
  */
 int corr_corner_turn(corr_handle h, const void* in, void* ws, void* stream);
 size_t corr_workspace_bytes(corr_handle h);

@@ -13,7 +13,6 @@ LIB_PATH = os.path.join(HERE, "libcorr.so")
 
 CORR_CI8, CORR_CF16 = 0, 1
 CORR_OK, CORR_EINVAL, CORR_EUNSUPPORTED, CORR_ENOMEM, CORR_ECUDA, CORR_EOVERFLOW = 0, -1, -2, -3, -4, -5
-CORR_FEED_DIRECT, CORR_FEED_CORNER_TURN = 0, 1
 KERNELS = {"auto": 0, "single": 1, "pair": 2, "quad": 3, "simt": 4}      # CORR_KERNEL_*
 KERNEL_NAMES = {v: k for k, v in KERNELS.items()}
 DTYPES = {"ci8": CORR_CI8, "cf16": CORR_CF16}
@@ -29,8 +28,6 @@ SYMBOLS = {
     "corr_output_bytes": (_sz, [_vp]),
     "corr_baseline_index": (_ll, [_i, _i]),
     "corr_last_error": (_cp, [_vp]),
-    "corr_set_feed": (_i, [_vp, _i]),
-    "corr_get_feed": (_i, [_vp]),
     "corr_set_kernel": (_i, [_vp, _i]),
     "corr_get_kernel": (_i, [_vp]),
     "corr_uses_tensor_cores": (_i, [_vp]),
@@ -131,9 +128,6 @@ class Correlator:
 
     def set_kernel(self, kernel):
         self._check(self._L.corr_set_kernel(self._h, KERNELS[kernel]))
-
-    def set_feed(self, feed):
-        self._check(self._L.corr_set_feed(self._h, int(feed)))
 
     def _check(self, rc):
         if rc != CORR_OK:

@@ -38,7 +38,6 @@ struct corr_plan {
     int sample_bytes;      // 2 (ci8) or 4 (cf16)
     int device;
     int sm_count;
-    int feed;
     bool tma_ok;           // one channel's row of components (2*M*elt bytes) is a multiple of 16 bytes, so every
                            // TMA box start (c*2M + tile offset) is 16-byte aligned
     long long t_total;     // samples integrated since the last accumulate == 0 call
@@ -409,7 +408,6 @@ corr_handle corr_create(int n_station, int n_pol, int n_chan, int n_time, int dt
     h->sample_bytes = dtype == CORR_CI8 ? 2 : 4;
     h->device = dev;
     h->sm_count = prop.multiProcessorCount;
-    h->feed = CORR_FEED_DIRECT;
     h->tma_ok = (M * h->sample_bytes) % 16 == 0;
     h->t_total = 0;
     h->last_launches = 0;
@@ -509,7 +507,6 @@ size_t corr_output_bytes(corr_handle h) { return h ? output_bytes(h) : 0; }
 size_t corr_workspace_bytes(corr_handle h) { return h ? workspace_bytes(h) : 0; }
 int corr_workspace_time(corr_handle h) { return h ? h->Tp : 0; }
 const char* corr_last_error(corr_handle h) { return h ? h->err : g_create_error; }
-int corr_get_feed(corr_handle h) { return h ? h->feed : CORR_EINVAL; }
 int corr_uses_tensor_cores(corr_handle h) { return h ? (resolve_kernel(h) != CORR_KERNEL_SIMT ? 1 : 0) : CORR_EINVAL; }
 int corr_get_kernel(corr_handle h) { return h ? resolve_kernel(h) : CORR_EINVAL; }
 
@@ -525,17 +522,6 @@ int corr_set_kernel(corr_handle h, int kernel) {
     return CORR_OK;
 }
 int corr_last_launch_count(corr_handle h) { return h ? h->last_launches : CORR_EINVAL; }
-
-int corr_set_feed(corr_handle h, int feed) {
-    if (!h) return CORR_EINVAL;
-    if (feed == CORR_FEED_DIRECT) {
-        h->feed = feed;
-        return CORR_OK;
-    }
-    if (feed == CORR_FEED_CORNER_TURN)
-        return fail(h, CORR_EUNSUPPORTED, "corr_set_feed: the corner-turn feeder of the tensor-core kernel is not built yet");
-    return fail(h, CORR_EINVAL, "corr_set_feed: unknown feed %d", feed);
-}
 
 int corr_corner_turn(corr_handle h, const void* in, void* ws, void* stream) {
     if (!h) return CORR_EINVAL;

@@ -121,7 +121,6 @@ def test_null_handle_helpers_are_safe(binding):
     assert L.corr_workspace_bytes(None) == 0
     assert L.corr_xengine(None, None, None, 0, None) == binding.CORR_EINVAL
     assert L.corr_xengine_host(None, None, None, 0) == binding.CORR_EINVAL
-    assert L.corr_set_feed(None, 0) == binding.CORR_EINVAL
     assert L.corr_set_kernel(None, 0) == binding.CORR_EINVAL
     assert L.corr_get_kernel(None) == binding.CORR_EINVAL
     L.corr_destroy(None)     # no-op
