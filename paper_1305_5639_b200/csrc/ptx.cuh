@@ -199,8 +199,10 @@ __device__ __forceinline__ uint32_t mapa(uint32_t addr, uint32_t rank) {
     return r;
 }
 // arrive on an mbarrier that may live in another CTA of the cluster (address from mapa)
+// .relaxed: the arrival orders nothing in generic memory (a .release at cluster scope costs a GPU-wide membar); the
+// TMEM reads it publishes are ordered by tcgen05.wait::ld + tcgen05.fence::before_thread_sync issued before it.
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+    asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
 // In a CTA pair the two CTAs' shared::cluster windows differ in one address bit; clearing it turns the
 // address of a barrier in this CTA into the address of the same barrier in the pair's even (leader) CTA.

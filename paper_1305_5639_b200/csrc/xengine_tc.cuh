@@ -161,25 +161,31 @@ __device__ __forceinline__ void drain_accumulator(const Params& prm, int c, int 
             if (lane < 8) ptx::bulk_wait_read<kBufs - 1>();   // staging[buf] (kBufs passes ago) has been read
             __syncwarp();
             const uint32_t sbuf = stage_smem + buf * kEpiBufBytes;
+            // both 32-column TMEM loads of the pass are issued before the first wait (latency overlap)
+            uint32_t v0[32], v1[32];
+            const bool two = h0 + 32 < h_end;
+            ptx::tmem_ld_32x32(taddr + h0, v0);
+            if (two) ptx::tmem_ld_32x32(taddr + h0 + 32, v1);
+            ptx::tmem_ld_wait();
+            if (h0 + kEpiCols >= h_end) {                // all of this warp's columns are in registers
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) release(release_bar);
+            }
+            {
+                uint32_t re[8], im[8];
+                combine_chunk<kFloat>(v0, ri, re, im);
+                // (i, p) x (j = j0 + 8 half + y, q = ri): byte offset j*32 + p*16 + q*8 in the station row
+                const uint32_t dst = sbuf + il * kEpiRowBytes + p * 16 + ri * 8;
 #pragma unroll
-            for (int half = 0; half < kEpiCols / 32; ++half) {
-                const int hh = h0 + 32 * half;
-                if (hh < h_end) {
-                    uint32_t v[32];
-                    ptx::tmem_ld_32x32(taddr + hh, v);
-                    ptx::tmem_ld_wait();
-                    if (hh + 32 >= h_end) {              // all of this warp's columns are in registers
-                        ptx::tc_fence_before();
-                        __syncwarp();
-                        if (lane == 0) release(release_bar);
-                    }
-                    uint32_t re[8], im[8];
-                    combine_chunk<kFloat>(v, ri, re, im);
-                    // (i, p) x (j = j0 + 8 half + y, q = ri): byte offset j*32 + p*16 + q*8 in the station row
-                    const uint32_t dst = sbuf + il * kEpiRowBytes + half * 256 + p * 16 + ri * 8;
+                for (int y = 0; y < 8; ++y) ptx::st_shared_v2(dst + y * 32, re[y], im[y]);
+            }
+            if (two) {
+                uint32_t re[8], im[8];
+                combine_chunk<kFloat>(v1, ri, re, im);
+                const uint32_t dst = sbuf + il * kEpiRowBytes + 256 + p * 16 + ri * 8;
 #pragma unroll
-                    for (int y = 0; y < 8; ++y) ptx::st_shared_v2(dst + y * 32, re[y], im[y]);
-                }
+                for (int y = 0; y < 8; ++y) ptx::st_shared_v2(dst + y * 32, re[y], im[y]);
             }
             ptx::fence_proxy_async_smem();               // generic-proxy writes -> visible to the bulk copy
             __syncwarp();
