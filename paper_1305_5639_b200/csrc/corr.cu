@@ -202,8 +202,22 @@ int launch_direct(corr_plan* h, const void* in, void* out, int accumulate, cudaS
     prm.out = out;
     prm.accumulate = accumulate ? 1 : 0;
     // samples per TMEM accumulation pass: everything for int32 (exact); 1024 for fp32 (see xengine_tc.cuh)
-    const int kstage = h->dtype == CORR_CI8 ? xtc::Cfg<1>::kKStage : xtc::Cfg<2>::kKStage;
-    prm.k_chunk = h->dtype == CORR_CI8 ? (h->T + kstage - 1) / kstage * kstage : xtc::kFloatChunk;
+    prm.k_chunk = h->dtype == CORR_CI8 ? (1 << 30) : xtc::kFloatChunk;      // int32 sums are exact: one pass
+    {   // operand ring geometry: widest B of any tile, plus separate A chunks only if some tile is off the diagonal
+        const int chunk_elems = h->dtype == CORR_CI8 ? 128 : 64;
+        const int chunk_bytes = 128 * (h->dtype == CORR_CI8 ? xtc::Cfg<1>::kKStage : xtc::Cfg<2>::kKStage);
+        int nb_max = 1;
+        bool need_a = false;
+        for (const xtc::TileDesc& t : h->h_tiles) {
+            const int nb = (t.ncols + chunk_elems - 1) / chunk_elems;
+            if (nb > nb_max) nb_max = nb;
+            if (!(t.row0 >= t.col0 && t.row0 + xtc::kTileRows <= t.col0 + nb * chunk_elems)) need_a = true;
+        }
+        prm.b_chunks = nb_max;
+        prm.stage_bytes = (nb_max + (need_a ? xtc::kTileRows / chunk_elems : 0)) * chunk_bytes;
+        prm.n_stages = xtc::kRingBytes / prm.stage_bytes;
+        if (prm.n_stages > xtc::kMaxStages) prm.n_stages = xtc::kMaxStages;
+    }
     const long long grid = prm.n_tiles < h->sm_count ? prm.n_tiles : h->sm_count;
     if (h->dtype == CORR_CI8)
         xtc::xengine_direct_kernel<1><<<static_cast<unsigned>(grid), xtc::kNumThreads, xtc::kSmemBytes, st>>>(h->tmap_in, prm);

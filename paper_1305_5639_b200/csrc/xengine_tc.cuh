@@ -32,8 +32,8 @@
 
 namespace xtc {
 
-constexpr int kNumStages = 6;
-constexpr int kStageBytes = 24 * 1024;
+constexpr int kMaxStages = 12;                // barrier slots; the stage count is chosen per geometry (Params::n_stages)
+constexpr int kRingBytes = 144 * 1024;        // operand ring of the 1-CTA kernel, cut into n_stages stages of stage_bytes
 constexpr int kTileRows = 128;        // G rows per tile   (TMEM lanes)
 constexpr int kTileCols = 256;        // G columns per tile (TMEM columns per accumulator stage)
 constexpr int kNumEpiWarps = 8;
@@ -46,7 +46,7 @@ constexpr int kEpiRowBytes = 544;
 constexpr int kEpiBufBytes = 8 * kEpiRowBytes;
 constexpr int kEpiWarpBytes = 2 * kEpiBufBytes;                       // double buffered
 constexpr int kEpiBytes = kNumEpiWarps * kEpiWarpBytes;
-constexpr int kSmemBytes = kNumStages * kStageBytes + kEpiBytes + 1024 /*alignment slack*/ + 256 /*barriers*/;
+constexpr int kSmemBytes = kRingBytes + kEpiBytes + 1024 /*alignment slack*/ + 256 /*barriers*/;
 
 struct TileDesc {
     int row0;    // first G row   of the tile, in real components u within the channel (multiple of 128)
@@ -65,6 +65,8 @@ struct Params {
     void* out;               // DEVICE: packed output
     int accumulate;
     int k_chunk;             // samples per TMEM accumulation pass (multiple of the pipeline stage)
+    // 1-CTA kernel: a stage holds [b_chunks 128-byte-wide B chunks][A chunks, only if some tile is off the diagonal]
+    int n_stages, stage_bytes, b_chunks;
 #ifdef CORR_STATS
     unsigned long long* stats;   // DEVICE, 8 counters per CTA (developer build only: python -m ...build with CORR_STATS=1)
 #endif
@@ -80,7 +82,7 @@ struct Params {
 
 template <int kElt> struct Cfg;
 template <> struct Cfg<1> {                      // complex int8 -> int32
-    static constexpr int kKStage = 64;           // time samples per pipeline stage
+    static constexpr int kKStage = 128;          // time samples per pipeline stage of the 1-CTA kernel (one TMA box)
     static constexpr int kMmaK = 32;             // time samples per tcgen05.mma (kind::i8)
     static constexpr bool kFloat = false;
     // instruction descriptor: D = S32 (2<<4), A = B = signed 8 bit (1<<7, 1<<10), A and B MN-major
@@ -88,7 +90,7 @@ template <> struct Cfg<1> {                      // complex int8 -> int32
     static constexpr uint32_t kIdesc = (2u << 4) | (1u << 7) | (1u << 10) | (1u << 15) | (1u << 16) | (8u << 24);
 };
 template <> struct Cfg<2> {                      // complex fp16 -> fp32
-    static constexpr int kKStage = 32;
+    static constexpr int kKStage = 64;
     static constexpr int kMmaK = 16;
     static constexpr bool kFloat = true;
     // D = F32 (1<<4), A = B = F16 (0), MN-major both, M = 128.
@@ -261,19 +263,21 @@ xengine_direct_kernel(const __grid_constant__ CUtensorMap tmap_in, const Params 
     constexpr int kAChunks = kTileRows / kChunkElems;       // 1 (ci8) / 2 (cf16)
     constexpr int kBChunksMax = kTileCols / kChunkElems;    // 2 (ci8) / 4 (cf16)
     constexpr int kKStepBytes = C::kMmaK * 128;             // smem advance per MMA k-step
-    constexpr int kKSteps = C::kKStage / C::kMmaK;          // 2
-    static_assert((kAChunks + kBChunksMax) * kChunkBytes == kStageBytes, "stage size");
+    constexpr int kKSteps = C::kKStage / C::kMmaK;          // 4
+    static_assert((kAChunks + kBChunksMax) * kChunkBytes * 3 <= kRingBytes, "at least three stages");
+    const int kNumStages = prm.n_stages;
+    const int kStageBytes = prm.stage_bytes;
 
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;   // SWIZZLE_128B atoms: 1024-B aligned
-    const uint32_t epi_base = smem_base + kNumStages * kStageBytes;
+    const uint32_t epi_base = smem_base + kRingBytes;
     const uint32_t bar_base = epi_base + kEpiBytes;
     // barrier slots (8 bytes each): full[S], empty[S], tmem_full[2], tmem_empty[2], then the TMEM base word
     auto full_bar = [&](int s) { return bar_base + 8u * s; };
-    auto empty_bar = [&](int s) { return bar_base + 8u * (kNumStages + s); };
-    auto tfull_bar = [&](int a) { return bar_base + 8u * (2 * kNumStages + a); };
-    auto tempty_bar = [&](int a) { return bar_base + 8u * (2 * kNumStages + 2 + a); };
-    const uint32_t tmem_slot = bar_base + 8u * (2 * kNumStages + 4);
+    auto empty_bar = [&](int s) { return bar_base + 8u * (kMaxStages + s); };
+    auto tfull_bar = [&](int a) { return bar_base + 8u * (2 * kMaxStages + a); };
+    auto tempty_bar = [&](int a) { return bar_base + 8u * (2 * kMaxStages + 2 + a); };
+    const uint32_t tmem_slot = bar_base + 8u * (2 * kMaxStages + 4);
     uint32_t* tmem_slot_ptr =
         reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - ptx::smem_u32(smem_raw)));
 
@@ -302,7 +306,7 @@ xengine_direct_kernel(const __grid_constant__ CUtensorMap tmap_in, const Params 
     const uint32_t tmem_base = *tmem_slot_ptr;
 
     const int num_kb = (prm.n_time + C::kKStage - 1) / C::kKStage;     // pipeline stages over the whole integration
-    const int kb_per_chunk = prm.k_chunk / C::kKStage;
+    const int kb_per_chunk = prm.k_chunk / C::kKStage > 0 ? prm.k_chunk / C::kKStage : 1;
     const int n_kchunks = (num_kb + kb_per_chunk - 1) / kb_per_chunk;
     const int M2 = 2 * prm.M;
 
@@ -317,19 +321,23 @@ xengine_direct_kernel(const __grid_constant__ CUtensorMap tmap_in, const Params 
                 const int w_row = c * M2 + td.row0;        // element coordinate in the [T][C*2M] view
                 const int w_col = c * M2 + td.col0;
                 const int nb = (td.ncols + kChunkElems - 1) / kChunkElems;
-                const uint32_t tx = static_cast<uint32_t>((kAChunks + nb) * kChunkBytes);
+                // tile on the diagonal: the 128 A rows are among the loaded B columns -> A is not loaded at all
+                const bool a_in_b = td.row0 >= td.col0 && td.row0 + kTileRows <= td.col0 + nb * kChunkElems;
+                const uint32_t tx = static_cast<uint32_t>(((a_in_b ? 0 : kAChunks) + nb) * kChunkBytes);
                 for (int kb = 0; kb < num_kb; ++kb) {
                     ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
-                    const uint32_t sa = smem_base + stage * kStageBytes;
+                    const uint32_t sb = smem_base + stage * kStageBytes;
+                    const uint32_t sa = sb + prm.b_chunks * kChunkBytes;
                     ptx::mbar_arrive_expect_tx(full_bar(stage), tx);
 #pragma unroll
                     for (int a = 0; a < kAChunks; ++a)
-                        ptx::tma_load_2d(sa + a * kChunkBytes, &tmap_in, full_bar(stage),
+                        if (!a_in_b)
+                            ptx::tma_load_2d(sa + a * kChunkBytes, &tmap_in, full_bar(stage),
                                          w_row + a * kChunkElems, kb * C::kKStage);
 #pragma unroll
                     for (int b = 0; b < kBChunksMax; ++b)
                         if (b < nb)
-                            ptx::tma_load_2d(sa + (kAChunks + b) * kChunkBytes, &tmap_in, full_bar(stage),
+                            ptx::tma_load_2d(sb + b * kChunkBytes, &tmap_in, full_bar(stage),
                                              w_col + b * kChunkElems, kb * C::kKStage);
                     if (++stage == kNumStages) { stage = 0; phase ^= 1u; }
                 }
@@ -346,6 +354,10 @@ xengine_direct_kernel(const __grid_constant__ CUtensorMap tmap_in, const Params 
                 const int c = static_cast<int>(tile / prm.tiles_per_chan);
                 const TileDesc td = prm.tiles[tile - static_cast<long long>(c) * prm.tiles_per_chan];
                 const uint32_t idesc = C::kIdesc | (static_cast<uint32_t>(td.ncols >> 3) << 17);
+                const int nb = (td.ncols + kChunkElems - 1) / kChunkElems;
+                const bool a_in_b = td.row0 >= td.col0 && td.row0 + kTileRows <= td.col0 + nb * kChunkElems;
+                // A operand = the B chunks holding rows row0 .. row0 + 127 when the tile lies on the diagonal
+                const uint32_t a_off = (a_in_b ? (td.row0 - td.col0) / kChunkElems : prm.b_chunks) * kChunkBytes;
                 for (int kb0 = 0; kb0 < num_kb; kb0 += kb_per_chunk) {
                     const int kb1 = kb0 + kb_per_chunk < num_kb ? kb0 + kb_per_chunk : num_kb;
                     const uint32_t d_tmem = tmem_base + acc * kTileCols;
@@ -354,13 +366,12 @@ xengine_direct_kernel(const __grid_constant__ CUtensorMap tmap_in, const Params 
                     for (int kb = kb0; kb < kb1; ++kb) {
                         ptx::mbar_wait(full_bar(stage), phase);          // TMA bytes have landed
                         ptx::tc_fence_after();
-                        const uint32_t sa = smem_base + stage * kStageBytes;
-                        const uint32_t sb = sa + kAChunks * kChunkBytes;
+                        const uint32_t sb = smem_base + stage * kStageBytes;
 #pragma unroll
                         for (int k = 0; k < kKSteps; ++k) {
                             // MN-major SWIZZLE_128B: LBO = distance between 128-byte-wide chunks (one TMA box),
                             // SBO = distance between 8-row groups along K (8 * 128 B).
-                            const uint64_t adesc = ptx::smem_desc_sw128(sa + k * kKStepBytes, kChunkBytes, 1024);
+                            const uint64_t adesc = ptx::smem_desc_sw128(sb + a_off + k * kKStepBytes, kChunkBytes, 1024);
                             const uint64_t bdesc = ptx::smem_desc_sw128(sb + k * kKStepBytes, kChunkBytes, 1024);
                             const uint32_t accum = (kb != kb0 || k != 0) ? 1u : 0u;
                             if constexpr (C::kFloat) ptx::mma_f16(d_tmem, adesc, bdesc, idesc, accum);
