@@ -32,6 +32,10 @@ def _load():
             f = getattr(lib, name)
             f.restype = i32
             f.argtypes = [vp, vp, i32, i32, i32, i32, vp, i32, i32]
+        for name in ("xo_xengine_cross_ci8", "xo_xengine_cross_cf16"):
+            f = getattr(lib, name)
+            f.restype = i32
+            f.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp, i32, i32]
         for name in ("xo_pair_ci8", "xo_pair_cf16"):
             f = getattr(lib, name)
             f.restype = None
@@ -111,3 +115,32 @@ def visibility(x, c, i, p, j, q):
     v = (ctypes.c_double * 2)()
     _load().xo_pair_cf16(x.ctypes.data, N, P, C, T, c, i, p, j, q, v)
     return float(v[0]), float(v[1])
+
+
+def xengine_cross(xa, xb, chans=None, accumulate_into=None):
+    """Rectangular cross-only X-engine (Sec. 4): V[n_sel, Na, Nb, P, P, 2] with
+    V[c, i, j, p, q] = sum_t conj(xa[t, c, i, p]) * xb[t, c, j, q]; no triangle, no autocorrelations."""
+    xa, kind = _check_x(xa)
+    xb, kind_b = _check_x(xb)
+    T, C, Na, P, _ = xa.shape
+    Tb, Cb, Nb, Pb, _ = xb.shape
+    if kind != kind_b or (T, C, P) != (Tb, Cb, Pb):
+        raise ValueError("the two groups must share dtype, T, C and P")
+    if chans is None:
+        n_sel, sel_ptr = C, None
+    else:
+        sel = np.ascontiguousarray(chans, dtype=np.int32)
+        n_sel, sel_ptr = int(sel.size), sel.ctypes.data
+    odt = np.int64 if kind == "ci8" else np.float64
+    shape = (n_sel, Na, Nb, P, P, 2)
+    if accumulate_into is None:
+        out, acc = np.empty(shape, dtype=odt), 0
+    else:
+        out, acc = accumulate_into, 1
+        if out.shape != shape or out.dtype != odt or not out.flags.c_contiguous:
+            raise ValueError("accumulate_into has the wrong shape/dtype/layout")
+    fn = _load().xo_xengine_cross_ci8 if kind == "ci8" else _load().xo_xengine_cross_cf16
+    rc = fn(xa.ctypes.data, xb.ctypes.data, out.ctypes.data, Na, Nb, P, C, T, sel_ptr, n_sel, acc)
+    if rc != 0:
+        raise RuntimeError("oracle failed with code %d" % rc)
+    return out

@@ -30,6 +30,10 @@
  * Arithmetic: ci8 exact in int64; cf16 inputs converted exactly to double, products and
  * sums in double in the order t = 0..T-1.  No blocking, no reordering: the loops are Eq. 2.
  *
+ * The rectangular cross-only variant (xo_xengine_cross_*) is at the end of this file; its pins are
+ * tests/test_oracle_cross_pins.py (einsum brute force, ZGEMM, the triangle oracle's off-diagonal block,
+ * conjugate swap, constant closed form).
+ *
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): brute force against numpy complex128
  * einsum on tiny inputs, reduction to a library ZGEMM, Hermitian symmetry, real non-negative
  * autocorrelations, constant-input closed form with asymmetric constants (pins the sign of
@@ -202,6 +206,78 @@ int xo_xengine_cf16(const uint16_t* in, double* out, int N, int P, int C, int T,
                     }
         free(xr);
         free(xi);
+    }
+    return fail ? -2 : 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Rectangular, cross-only X-engine (Sec. 4: nodes of the space-division models
+ * "process two parts of the input streams in a rectangle pattern for cross-correlations only"):
+ *
+ *     V[c][i][j][p][q] = sum_t conj(a[t][c][i][p]) * b[t][c][j][q]      i in group A, j in group B
+ *
+ * Eq. 2 with the conjugated stream taken from group A and the other from group B; every (i, j)
+ * is stored (no triangle, no autocorrelations).  Layouts: in_a [T][C][Na][P], in_b [T][C][Nb][P]
+ * complex interleaved; out [n_sel][Na][Nb][P][P] complex interleaved (int64 / double).
+ * Plain loops, time innermost, no gather, no blocking.
+ * ------------------------------------------------------------------------------------------ */
+int xo_xengine_cross_ci8(const int8_t* in_a, const int8_t* in_b, int64_t* out, int Na, int Nb, int P,
+                         int C, int T, const int* chans, int n_sel, int accumulate)
+{
+    if (!in_a || !in_b || !out || Na <= 0 || Nb <= 0 || P <= 0 || C <= 0 || T < 0) return -1;
+    if (!chans) n_sel = C;
+    int fail = 0;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int k = 0; k < n_sel; ++k) {
+        const int c = chans ? chans[k] : k;
+        if (c < 0 || c >= C) { fail = 1; continue; }
+        for (int i = 0; i < Na; ++i)
+            for (int j = 0; j < Nb; ++j)
+                for (int p = 0; p < P; ++p)
+                    for (int q = 0; q < P; ++q) {
+                        int64_t re = 0, im = 0;
+                        for (int t = 0; t < T; ++t) {
+                            const int8_t* a = in_a + 2 * ((((size_t)t * C + c) * Na + i) * P + p);
+                            const int8_t* b = in_b + 2 * ((((size_t)t * C + c) * Nb + j) * P + q);
+                            int64_t ar = a[0], ai = a[1], br = b[0], bi = b[1];
+                            re += ar * br + ai * bi;      /* Re conj(a) b */
+                            im += ar * bi - ai * br;      /* Im conj(a) b */
+                        }
+                        int64_t* o = out + 2 * (((((size_t)k * Na + i) * Nb + j) * P + p) * P + q);
+                        if (accumulate) { o[0] += re; o[1] += im; }
+                        else            { o[0]  = re; o[1]  = im; }
+                    }
+    }
+    return fail ? -2 : 0;
+}
+
+int xo_xengine_cross_cf16(const uint16_t* in_a, const uint16_t* in_b, double* out, int Na, int Nb, int P,
+                          int C, int T, const int* chans, int n_sel, int accumulate)
+{
+    if (!in_a || !in_b || !out || Na <= 0 || Nb <= 0 || P <= 0 || C <= 0 || T < 0) return -1;
+    if (!chans) n_sel = C;
+    int fail = 0;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int k = 0; k < n_sel; ++k) {
+        const int c = chans ? chans[k] : k;
+        if (c < 0 || c >= C) { fail = 1; continue; }
+        for (int i = 0; i < Na; ++i)
+            for (int j = 0; j < Nb; ++j)
+                for (int p = 0; p < P; ++p)
+                    for (int q = 0; q < P; ++q) {
+                        double re = 0.0, im = 0.0;
+                        for (int t = 0; t < T; ++t) {
+                            const uint16_t* a = in_a + 2 * ((((size_t)t * C + c) * Na + i) * P + p);
+                            const uint16_t* b = in_b + 2 * ((((size_t)t * C + c) * Nb + j) * P + q);
+                            double ar = half_bits_to_double(a[0]), ai = half_bits_to_double(a[1]);
+                            double br = half_bits_to_double(b[0]), bi = half_bits_to_double(b[1]);
+                            re += ar * br + ai * bi;
+                            im += ar * bi - ai * br;
+                        }
+                        double* o = out + 2 * (((((size_t)k * Na + i) * Nb + j) * P + p) * P + q);
+                        if (accumulate) { o[0] += re; o[1] += im; }
+                        else            { o[0]  = re; o[1]  = im; }
+                    }
     }
     return fail ? -2 : 0;
 }
