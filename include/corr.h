@@ -94,6 +94,27 @@ int corr_xengine(corr_handle h, const void* in, void* out, int accumulate, void*
  */
 int corr_xengine_host(corr_handle h, const void* in_host, void* out_host, int accumulate);
 
+/*
+ * Rectangular, cross-only X-engine.  PAPER.md:79, Sec. 4: in the space-division models "some
+ * of the nodes ... need to process two parts of the input streams in a rectangle pattern for cross-correlations
+ * only".  For two station groups A (n_station_a) and B (n_station_b) sharing n_pol, n_chan, n_time and dtype:
+ *
+ *     out[c][i][j][p][q] = sum_t conj(in_a[t][c][i][p]) * in_b[t][c][j][q]        (Eq. 2, i in A, j in B)
+ *
+ * every (i, j) is stored: no triangle, no autocorrelations.  Layouts as for corr_xengine with
+ *   in_a [n_time][n_chan][n_station_a][n_pol], in_b [n_time][n_chan][n_station_b][n_pol]   (DEVICE, 16-byte aligned)
+ *   out  [n_chan][n_station_a][n_station_b][n_pol][n_pol] complex int32 / fp32               (DEVICE, 16-byte aligned)
+ * corr_input_bytes(h) is the size of in_a, corr_input_bytes_b(h) of in_b, corr_output_bytes(h) of out.
+ * corr_create_cross returns NULL on failure (corr_last_error(NULL)); the handle is used with corr_xengine_cross
+ * only (corr_xengine, corr_xengine_host and corr_corner_turn return CORR_EINVAL on it, and corr_xengine_cross
+ * returns CORR_EINVAL on a corr_create handle).  accumulate / stream / CORR_EOVERFLOW exactly as corr_xengine.
+ * Runs on the CTA-pair tcgen05 kernel (full rectangle of 256 x 256 tiles, group A and group B read in place through
+ * two tensor maps) or, when a group's per-channel row is not a multiple of 16 bytes, on the SIMT kernel.
+ */
+corr_handle corr_create_cross(int n_station_a, int n_station_b, int n_pol, int n_chan, int n_time, int dtype);
+int corr_xengine_cross(corr_handle h, const void* in_a, const void* in_b, void* out, int accumulate, void* stream);
+size_t corr_input_bytes_b(corr_handle h);    /* cross plans: T*C*Nb*P * (2 or 4); else 0 */
+
 /* corr_destroy -- frees the handle and everything it owns.  NULL is a no-op. */
 void corr_destroy(corr_handle h);
 

@@ -23,6 +23,9 @@ SYMBOLS = {
     "corr_create": (_vp, [_i, _i, _i, _i, _i]),
     "corr_xengine": (_i, [_vp, _vp, _vp, _i, _vp]),
     "corr_xengine_host": (_i, [_vp, _vp, _vp, _i]),
+    "corr_create_cross": (_vp, [_i, _i, _i, _i, _i, _i]),
+    "corr_xengine_cross": (_i, [_vp, _vp, _vp, _vp, _i, _vp]),
+    "corr_input_bytes_b": (_sz, [_vp]),
     "corr_destroy": (None, [_vp]),
     "corr_input_bytes": (_sz, [_vp]),
     "corr_output_bytes": (_sz, [_vp]),
@@ -209,3 +212,41 @@ class Correlator:
 
     def __exit__(self, *a):
         self.close()
+
+
+class CrossCorrelator(Correlator):
+    """corr_create_cross / corr_xengine_cross: rectangular cross-only X-engine of two station groups."""
+
+    def __init__(self, n_station_a, n_station_b, n_pol, n_chan, n_time, dtype="ci8"):
+        self._L = lib()
+        self.N, self.Nb, self.P, self.C, self.T, self.dtype = n_station_a, n_station_b, n_pol, n_chan, n_time, dtype
+        self._h = self._L.corr_create_cross(n_station_a, n_station_b, n_pol, n_chan, n_time, DTYPES[dtype])
+        if not self._h:
+            msg = self._L.corr_last_error(None).decode()
+            raise CorrError(CORR_EINVAL if "invalid" in msg or "too large" in msg else CORR_EUNSUPPORTED, msg)
+        self.n_baseline = n_station_a * n_station_b
+
+    @property
+    def input_bytes_b(self):
+        return int(self._L.corr_input_bytes_b(self._h))
+
+    def input_shape_b(self):
+        return (self.T, self.C, self.Nb, self.P, 2)
+
+    def output_shape(self):
+        return (self.C, self.N, self.Nb, self.P, self.P, 2)
+
+    def xengine_cross(self, xa, xb, out=None, accumulate=False, stream=None):
+        import torch
+        self._check_in(xa, "cuda")
+        want = torch.int8 if self.dtype == "ci8" else torch.float16
+        if xb.dtype != want or tuple(xb.shape) != self.input_shape_b() or not xb.is_contiguous() or xb.device.type != "cuda":
+            raise ValueError("group B must be a contiguous CUDA %s tensor of shape %s" % (want, self.input_shape_b()))
+        if out is None:
+            if accumulate:
+                raise ValueError("accumulate=True needs the running `out`")
+            out = self.empty_output(xa.device)
+        self._check_out(out, "cuda")
+        self._check(self._L.corr_xengine_cross(self._h, xa.data_ptr(), xb.data_ptr(), out.data_ptr(),
+                                               int(bool(accumulate)), _stream_ptr(stream)))
+        return out

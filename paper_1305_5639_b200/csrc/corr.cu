@@ -34,6 +34,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 struct corr_plan {
     int N, P, C, T, dtype;
     int M;                 // N * P
+    int Nb, Mb;            // rectangular cross-only plan (corr_create_cross): stations / streams of group B; 0 = HERK
     long long B;           // N (N + 1) / 2
     int sample_bytes;      // 2 (ci8) or 4 (cf16)
     int device;
@@ -54,6 +55,8 @@ struct corr_plan {
     CUtensorMap tmap_in;     // 1-CTA kernel: box [128 B][Cfg::kKStage samples]
     CUtensorMap tmap_pair;   // pair kernels: box [128 B][kPairStageK / kPairBoxes samples]
     const void* tmap_in_ptr;
+    CUtensorMap tmap_b;      // cross plans: group B, pair-kernel box
+    const void* tmap_b_ptr;
 
     // corner-turn feed
     int Tp;                // padded time extent of the workspace
@@ -140,9 +143,22 @@ void build_groups(int N, int P, int pairs_per_cluster, std::vector<xtc::PairGrou
     if (k < odd.size()) g.push_back(xtc::PairGroup{{odd[k], odd[k]}, 3, 0});
 }
 
+// Rectangular cross-only plan: every 256 x 256 block of the [2 M_a] x [2 M_b] rectangle, column-block major.
+void build_groups_rect(int Na, int Nb, int P, std::vector<xtc::PairGroup>& g) {
+    g.clear();
+    const int Ra = (2 * Na * P + xtc::kPairRows - 1) / xtc::kPairRows;
+    const int Rb = (2 * Nb * P + xtc::kPairRows - 1) / xtc::kPairRows;
+    for (int cb = 0; cb < Rb; ++cb)
+        for (int rb = 0; rb < Ra; ++rb) {
+            const xtc::PairTile t{rb * xtc::kPairRows, cb * xtc::kPairRows};
+            g.push_back(xtc::PairGroup{{t, t}, 0, 0});
+        }
+}
+
 int resolve_kernel(const corr_plan* h) {
     if (!h->tma_ok) return CORR_KERNEL_SIMT;
     if (h->kernel != CORR_KERNEL_AUTO) return h->kernel;
+    if (h->Nb) return h->max_clusters[0] > 0 ? CORR_KERNEL_PAIR : CORR_KERNEL_SIMT;
     const int M2 = 2 * h->M;
     // CORR_KERNEL_QUAD (multicast between two pairs) is never chosen: measured 12 % slower than PAIR at config 4
     // (profiles/): the multicast saves L2 reads but not delivered bytes, and couples the two pairs' pipelines
@@ -160,30 +176,40 @@ size_t workspace_bytes(const corr_plan* h) {
     return 2 * static_cast<size_t>(h->C) * h->M * h->Tp * h->sample_bytes;
 }
 
-int encode_input_map(corr_plan* h, const void* in) {
-    if (h->tmap_in_ptr == in) return CORR_OK;
+int encode_map(corr_plan* h, CUtensorMap* map, const void* ptr, int M, int box_rows) {
     const int elt = h->sample_bytes / 2;                       // bytes per real component
-    const cuuint64_t W = static_cast<cuuint64_t>(h->C) * 2 * h->M;
+    const cuuint64_t W = static_cast<cuuint64_t>(h->C) * 2 * M;
     cuuint64_t dims[2] = {W, static_cast<cuuint64_t>(h->T)};
     cuuint64_t strides[1] = {W * elt};
-    cuuint32_t box[2] = {static_cast<cuuint32_t>(128 / elt),
-                         static_cast<cuuint32_t>(elt == 1 ? xtc::Cfg<1>::kKStage : xtc::Cfg<2>::kKStage)};
+    cuuint32_t box[2] = {static_cast<cuuint32_t>(128 / elt), static_cast<cuuint32_t>(box_rows)};
     cuuint32_t estr[2] = {1, 1};
-    const CUresult r = h->encode(&h->tmap_in, elt == 1 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16,
-                                 2, const_cast<void*>(in), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+    const CUresult r = h->encode(map, elt == 1 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2,
+                                 const_cast<void*>(ptr), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                                  CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    cuuint32_t box2[2] = {box[0], static_cast<cuuint32_t>((elt == 1 ? xtc::kPairStageK<1> : xtc::kPairStageK<2>) / xtc::kPairBoxes)};
-    const CUresult r2 = r != CUDA_SUCCESS ? r :
-        h->encode(&h->tmap_pair, elt == 1 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16,
-                  2, const_cast<void*>(in), dims, strides, box2, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                  CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r2 != CUDA_SUCCESS) {
-        h->tmap_in_ptr = nullptr;
-        return fail(h, CORR_ECUDA, "cuTensorMapEncodeTiled(in) failed with CUresult %d", static_cast<int>(r2));
-    }
-    h->tmap_in_ptr = in;
+    if (r != CUDA_SUCCESS) return fail(h, CORR_ECUDA, "cuTensorMapEncodeTiled failed with CUresult %d", static_cast<int>(r));
     return CORR_OK;
+}
+
+// Tensor maps of `in` viewed as [T][C*2M]: box [128 B][stage samples] for the 1-CTA kernel and for the pair kernels.
+int encode_input_map(corr_plan* h, const void* in) {
+    if (h->tmap_in_ptr == in) return CORR_OK;
+    h->tmap_in_ptr = nullptr;
+    const int elt = h->sample_bytes / 2;
+    int rc = encode_map(h, &h->tmap_in, in, h->M, elt == 1 ? xtc::Cfg<1>::kKStage : xtc::Cfg<2>::kKStage);
+    if (rc == CORR_OK)
+        rc = encode_map(h, &h->tmap_pair, in, h->M, (elt == 1 ? xtc::kPairStageK<1> : xtc::kPairStageK<2>) / xtc::kPairBoxes);
+    if (rc == CORR_OK) h->tmap_in_ptr = in;
+    return rc;
+}
+
+int encode_input_map_b(corr_plan* h, const void* in_b) {
+    if (h->tmap_b_ptr == in_b) return CORR_OK;
+    h->tmap_b_ptr = nullptr;
+    const int elt = h->sample_bytes / 2;
+    const int rc = encode_map(h, &h->tmap_b, in_b, h->Mb, (elt == 1 ? xtc::kPairStageK<1> : xtc::kPairStageK<2>) / xtc::kPairBoxes);
+    if (rc == CORR_OK) h->tmap_b_ptr = in_b;
+    return rc;
 }
 
 int launch_direct(corr_plan* h, const void* in, void* out, int accumulate, cudaStream_t st) {
@@ -199,6 +225,8 @@ int launch_direct(corr_plan* h, const void* in, void* out, int accumulate, cudaS
     prm.n_time = h->T;
     prm.M = h->M;
     prm.n_baseline = h->B;
+    prm.n_station_b = 0;
+    prm.M_b = 0;
     prm.out = out;
     prm.accumulate = accumulate ? 1 : 0;
     // samples per TMEM accumulation pass: everything for int32 (exact); 1024 for fp32 (see xengine_tc.cuh)
@@ -230,7 +258,8 @@ int launch_direct(corr_plan* h, const void* in, void* out, int accumulate, cudaS
 }
 
 template <int kElt, int kPairs>
-cudaError_t launch_pair_kernel(const CUtensorMap& tmap, const xtc::PairParams& pp, unsigned clusters, cudaStream_t st) {
+cudaError_t launch_pair_kernel(const CUtensorMap& tmap, const CUtensorMap& tmap_b, const xtc::PairParams& pp, unsigned clusters,
+                               cudaStream_t st) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(clusters * 2 * kPairs);
     cfg.blockDim = dim3(xtc::kNumThreads);
@@ -243,12 +272,15 @@ cudaError_t launch_pair_kernel(const CUtensorMap& tmap, const xtc::PairParams& p
     at[0].val.clusterDim.z = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, xtc::xengine_pair_kernel<kElt, kPairs>, tmap, pp);
+    return cudaLaunchKernelEx(&cfg, xtc::xengine_pair_kernel<kElt, kPairs>, tmap, tmap_b, pp);
 }
 
-int launch_pair(corr_plan* h, const void* in, void* out, int accumulate, cudaStream_t st, int pairs_per_cluster) {
+int launch_pair(corr_plan* h, const void* in, const void* in_b, void* out, int accumulate, cudaStream_t st,
+                int pairs_per_cluster) {
     int rc = encode_input_map(h, in);
+    if (rc == CORR_OK && h->Nb) rc = encode_input_map_b(h, in_b);
     if (rc != CORR_OK) return rc;
+    const CUtensorMap& map_b = h->Nb ? h->tmap_b : h->tmap_pair;
     const int v = pairs_per_cluster - 1;
     xtc::PairParams pp;
     pp.base.tiles = nullptr;
@@ -260,6 +292,8 @@ int launch_pair(corr_plan* h, const void* in, void* out, int accumulate, cudaStr
     pp.base.n_time = h->T;
     pp.base.M = h->M;
     pp.base.n_baseline = h->B;
+    pp.base.n_station_b = h->Nb;
+    pp.base.M_b = h->Mb;
     pp.base.out = out;
     pp.base.accumulate = accumulate ? 1 : 0;
     pp.base.k_chunk = h->dtype == CORR_CI8 ? (1 << 30) : xtc::kFloatChunk;      // int32 sums are exact: one pass
@@ -275,9 +309,9 @@ int launch_pair(corr_plan* h, const void* in, void* out, int accumulate, cudaStr
     const unsigned clusters = static_cast<unsigned>(pp.n_groups < h->max_clusters[v] ? pp.n_groups : h->max_clusters[v]);
     cudaError_t e;
     if (h->dtype == CORR_CI8)
-        e = v ? launch_pair_kernel<1, 2>(h->tmap_pair, pp, clusters, st) : launch_pair_kernel<1, 1>(h->tmap_pair, pp, clusters, st);
+        e = v ? launch_pair_kernel<1, 2>(h->tmap_pair, map_b, pp, clusters, st) : launch_pair_kernel<1, 1>(h->tmap_pair, map_b, pp, clusters, st);
     else
-        e = v ? launch_pair_kernel<2, 2>(h->tmap_pair, pp, clusters, st) : launch_pair_kernel<2, 1>(h->tmap_pair, pp, clusters, st);
+        e = v ? launch_pair_kernel<2, 2>(h->tmap_pair, map_b, pp, clusters, st) : launch_pair_kernel<2, 1>(h->tmap_pair, map_b, pp, clusters, st);
     if (e != cudaSuccess) return fail_cuda(h, e, "xengine_pair_kernel launch");
 #ifdef CORR_STATS
     if (getenv("CORR_STATS_PRINT")) {
@@ -297,9 +331,11 @@ int launch_pair(corr_plan* h, const void* in, void* out, int accumulate, cudaStr
     return CORR_OK;
 }
 
-int launch_simt(corr_plan* h, const void* in, void* out, int accumulate, cudaStream_t st) {
+int launch_simt(corr_plan* h, const void* in, const void* in_b, void* out, int accumulate, cudaStream_t st) {
     xsimt::Params prm;
     prm.in = in;
+    prm.in_b = in_b;
+    prm.n_station_b = h->Nb;
     prm.out = out;
     prm.n_station = h->N;
     prm.n_pol = h->P;
@@ -377,16 +413,17 @@ int corr_tile_schedule(int n_station, int n_pol, int dtype, int kernel, int* til
     return n;
 }
 
-corr_handle corr_create(int n_station, int n_pol, int n_chan, int n_time, int dtype) {
+static corr_handle create_plan(int n_station, int n_station_b, int n_pol, int n_chan, int n_time, int dtype) {
     g_create_error[0] = 0;
-    if (!valid_geometry(n_station, n_pol, dtype) || n_chan < 1 || n_time < 1) {
-        fail(nullptr, CORR_EINVAL, "corr_create: invalid geometry N=%d P=%d C=%d T=%d dtype=%d", n_station, n_pol,
-             n_chan, n_time, dtype);
+    if (!valid_geometry(n_station, n_pol, dtype) || n_station_b < 0 || n_chan < 1 || n_time < 1) {
+        fail(nullptr, CORR_EINVAL, "corr_create: invalid geometry N=%d Nb=%d P=%d C=%d T=%d dtype=%d", n_station, n_station_b,
+             n_pol, n_chan, n_time, dtype);
         return nullptr;
     }
     const long long M = static_cast<long long>(n_station) * n_pol;
-    const long long W = static_cast<long long>(n_chan) * 2 * M;
-    if (M > (1 << 20) || W > (1ll << 31) - 1024 || n_time > (1 << 24)) {
+    const long long Mb = static_cast<long long>(n_station_b) * n_pol;
+    const long long W = static_cast<long long>(n_chan) * 2 * (M > Mb ? M : Mb);
+    if (M > (1 << 20) || Mb > (1 << 20) || W > (1ll << 31) - 1024 || n_time > (1 << 24)) {
         fail(nullptr, CORR_EINVAL, "corr_create: geometry too large (N*P=%lld, C*2*N*P=%lld, T=%d)", M, W, n_time);
         return nullptr;
     }
@@ -418,11 +455,15 @@ corr_handle corr_create(int n_station, int n_pol, int n_chan, int n_time, int dt
     h->T = n_time;
     h->dtype = dtype;
     h->M = static_cast<int>(M);
-    h->B = static_cast<long long>(n_station) * (n_station + 1) / 2;
+    h->Nb = n_station_b;
+    h->Mb = static_cast<int>(Mb);
+    h->B = n_station_b ? static_cast<long long>(n_station) * n_station_b       // rectangle: every (i, j)
+                       : static_cast<long long>(n_station) * (n_station + 1) / 2;
     h->sample_bytes = dtype == CORR_CI8 ? 2 : 4;
     h->device = dev;
     h->sm_count = prop.multiProcessorCount;
-    h->tma_ok = (M * h->sample_bytes) % 16 == 0;
+    h->tma_ok = (M * h->sample_bytes) % 16 == 0 && (Mb * h->sample_bytes) % 16 == 0;
+    h->tmap_b_ptr = nullptr;
     h->t_total = 0;
     h->last_launches = 0;
     h->d_tiles = nullptr;
@@ -468,8 +509,9 @@ corr_handle corr_create(int n_station, int n_pol, int n_chan, int n_time, int dt
             return nullptr;
         }
         // CTA-pair kernels: group tables and the number of co-resident clusters (the persistent grid)
-        for (int v = 0; v < 2 && e == cudaSuccess; ++v) {
-            build_groups(h->N, h->P, v + 1, h->h_groups[v]);
+        for (int v = 0; v < (h->Nb ? 1 : 2) && e == cudaSuccess; ++v) {
+            if (h->Nb) build_groups_rect(h->N, h->Nb, h->P, h->h_groups[v]);
+            else build_groups(h->N, h->P, v + 1, h->h_groups[v]);
             const size_t bytes = h->h_groups[v].size() * sizeof(xtc::PairGroup);
             e = cudaMalloc(&h->d_groups[v], bytes);
             if (e == cudaSuccess) e = cudaMemcpy(h->d_groups[v], h->h_groups[v].data(), bytes, cudaMemcpyHostToDevice);
@@ -504,6 +546,19 @@ corr_handle corr_create(int n_station, int n_pol, int n_chan, int n_time, int dt
     return h;
 }
 
+corr_handle corr_create(int n_station, int n_pol, int n_chan, int n_time, int dtype) {
+    return create_plan(n_station, 0, n_pol, n_chan, n_time, dtype);
+}
+
+corr_handle corr_create_cross(int n_station_a, int n_station_b, int n_pol, int n_chan, int n_time, int dtype) {
+    if (n_station_b < 1) {
+        g_create_error[0] = 0;
+        fail(nullptr, CORR_EINVAL, "corr_create_cross: invalid geometry Na=%d Nb=%d", n_station_a, n_station_b);
+        return nullptr;
+    }
+    return create_plan(n_station_a, n_station_b, n_pol, n_chan, n_time, dtype);
+}
+
 void corr_destroy(corr_handle h) {
     if (!h) return;
     if (h->d_tiles) cudaFree(h->d_tiles);
@@ -517,6 +572,7 @@ void corr_destroy(corr_handle h) {
 }
 
 size_t corr_input_bytes(corr_handle h) { return h ? input_bytes(h) : 0; }
+size_t corr_input_bytes_b(corr_handle h) { return h ? static_cast<size_t>(h->T) * h->C * h->Mb * h->sample_bytes : 0; }
 size_t corr_output_bytes(corr_handle h) { return h ? output_bytes(h) : 0; }
 size_t corr_workspace_bytes(corr_handle h) { return h ? workspace_bytes(h) : 0; }
 int corr_workspace_time(corr_handle h) { return h ? h->Tp : 0; }
@@ -530,6 +586,8 @@ int corr_set_kernel(corr_handle h, int kernel) {
     if (kernel != CORR_KERNEL_AUTO && kernel != CORR_KERNEL_SIMT && !h->tma_ok)
         return fail(h, CORR_EUNSUPPORTED, "corr_set_kernel: per-channel row of %lld B is not a multiple of 16, only the SIMT kernel applies",
                     static_cast<long long>(h->M) * h->sample_bytes);
+    if (h->Nb && (kernel == CORR_KERNEL_SINGLE || kernel == CORR_KERNEL_QUAD))
+        return fail(h, CORR_EUNSUPPORTED, "corr_set_kernel: cross plans run on the PAIR or the SIMT kernel");
     if ((kernel == CORR_KERNEL_PAIR && h->max_clusters[0] <= 0) || (kernel == CORR_KERNEL_QUAD && h->max_clusters[1] <= 0))
         return fail(h, CORR_EUNSUPPORTED, "corr_set_kernel: no co-resident clusters for kernel %d on this device", kernel);
     h->kernel = kernel;
@@ -539,6 +597,7 @@ int corr_last_launch_count(corr_handle h) { return h ? h->last_launches : CORR_E
 
 int corr_corner_turn(corr_handle h, const void* in, void* ws, void* stream) {
     if (!h) return CORR_EINVAL;
+    if (h->Nb) return fail(h, CORR_EINVAL, "corr_corner_turn: not available on cross plans");
     if (!in || !ws) return fail(h, CORR_EINVAL, "corr_corner_turn: NULL pointer");
     if ((reinterpret_cast<uintptr_t>(in) & 15) || (reinterpret_cast<uintptr_t>(ws) & 127))
         return fail(h, CORR_EINVAL, "corr_corner_turn: `in` must be 16-byte and `ws` 128-byte aligned");
@@ -549,8 +608,23 @@ int corr_corner_turn(corr_handle h, const void* in, void* ws, void* stream) {
     return launch_corner_turn(h, in, ws, static_cast<cudaStream_t>(stream));
 }
 
+static int run_xengine(corr_handle h, const void* in, const void* in_b, void* out, int accumulate, void* stream);
+
 int corr_xengine(corr_handle h, const void* in, void* out, int accumulate, void* stream) {
     if (!h) return CORR_EINVAL;
+    if (h->Nb) return fail(h, CORR_EINVAL, "corr_xengine: this is a cross plan (corr_create_cross); call corr_xengine_cross");
+    return run_xengine(h, in, nullptr, out, accumulate, stream);
+}
+
+int corr_xengine_cross(corr_handle h, const void* in_a, const void* in_b, void* out, int accumulate, void* stream) {
+    if (!h) return CORR_EINVAL;
+    if (!h->Nb) return fail(h, CORR_EINVAL, "corr_xengine_cross: this is not a cross plan; call corr_xengine");
+    if (!in_b || (reinterpret_cast<uintptr_t>(in_b) & 15))
+        return fail(h, CORR_EINVAL, "corr_xengine_cross: `in_b` must be a non-NULL, 16-byte aligned device pointer");
+    return run_xengine(h, in_a, in_b, out, accumulate, stream);
+}
+
+static int run_xengine(corr_handle h, const void* in, const void* in_b, void* out, int accumulate, void* stream) {
     if (!in || !out) return fail(h, CORR_EINVAL, "corr_xengine: NULL pointer");
     if ((reinterpret_cast<uintptr_t>(in) & 15) || (reinterpret_cast<uintptr_t>(out) & 15))
         return fail(h, CORR_EINVAL, "corr_xengine: `in` and `out` must be 16-byte aligned");
@@ -562,10 +636,10 @@ int corr_xengine(corr_handle h, const void* in, void* out, int accumulate, void*
     h->last_launches = 0;
     int rc;
     switch (resolve_kernel(h)) {
-        case CORR_KERNEL_QUAD: rc = launch_pair(h, in, out, accumulate, st, 2); break;
-        case CORR_KERNEL_PAIR: rc = launch_pair(h, in, out, accumulate, st, 1); break;
+        case CORR_KERNEL_QUAD: rc = launch_pair(h, in, in_b, out, accumulate, st, 2); break;
+        case CORR_KERNEL_PAIR: rc = launch_pair(h, in, in_b, out, accumulate, st, 1); break;
         case CORR_KERNEL_SINGLE: rc = launch_direct(h, in, out, accumulate, st); break;
-        default: rc = launch_simt(h, in, out, accumulate, st); break;
+        default: rc = launch_simt(h, in, in_b, out, accumulate, st); break;
     }
     if (rc == CORR_OK) h->t_total = t_next;
     return rc;
@@ -573,6 +647,7 @@ int corr_xengine(corr_handle h, const void* in, void* out, int accumulate, void*
 
 int corr_xengine_host(corr_handle h, const void* in_host, void* out_host, int accumulate) {
     if (!h) return CORR_EINVAL;
+    if (h->Nb) return fail(h, CORR_EINVAL, "corr_xengine_host: not available on cross plans");
     if (!in_host) return fail(h, CORR_EINVAL, "corr_xengine_host: NULL input pointer");
     cudaError_t e;
     if (!h->own_stream) {

@@ -57,7 +57,8 @@ struct PairParams {
 
 template <int kElt, int kPairs>
 __global__ void __launch_bounds__(kNumThreads, 1)
-xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const PairParams pp) {
+xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const __grid_constant__ CUtensorMap tmap_b,
+                    const PairParams pp) {
     using C = Cfg<kElt>;
     const Params& prm = pp.base;
     constexpr int kChunkElems = 128 / kElt;                 // u per 128-byte chunk
@@ -98,6 +99,7 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const PairParam
 
     if (threadIdx.x == 0) {
         ptx::prefetch_tensormap(&tmap_in);
+        ptx::prefetch_tensormap(&tmap_b);
         for (int s = 0; s < kPairStages; ++s) {
             ptx::mbar_init(full_bar(s), 1);                  // leader: its own arrive.expect_tx
             ptx::mbar_init(empty_bar(s), kPairs);            // one tcgen05.commit arrival per pair of the cluster
@@ -120,7 +122,9 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const PairParam
     const int num_kb = (prm.n_time + kStageK - 1) / kStageK;
     const int kb_per_chunk = prm.k_chunk / kStageK > 0 ? prm.k_chunk / kStageK : 1;
     const int n_kchunks = (num_kb + kb_per_chunk - 1) / kb_per_chunk;
-    const int M2 = 2 * prm.M;
+    const int M2 = 2 * prm.M;                                  // G rows per channel (group A in cross mode)
+    const bool rect = prm.n_station_b > 0;                     // rectangular cross-only mode: B columns from tmap_b
+    const int M2b = rect ? 2 * prm.M_b : M2;                   // G columns per channel
 
     if (warp == 0) {
         // ===================== TMA producer =====================
@@ -134,12 +138,12 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const PairParam
                 const PairGroup gd = pp.groups[g - static_cast<long long>(c) * pp.groups_per_chan];
                 const PairTile td = (kPairs == 2 && pair == 1) ? gd.t[1] : gd.t[0];
                 const int w_a = c * M2 + td.row0 + 128 * half;      // this CTA's A rows in the [T][C*2M] view
-                const int w_b = c * M2 + td.col0 + 128 * half;      // this CTA's half of the B columns
+                const int w_b = c * M2b + td.col0 + 128 * half;     // this CTA's half of the B columns
                 // a shared operand is fetched once, by pair 0's CTA, and multicast to the same-half CTA of pair 1
                 const bool mc_a = kPairs == 2 && (gd.share & 1);
                 const bool mc_b = kPairs == 2 && (gd.share & 2);
                 // diagonal tile: this CTA's half of the B columns IS its 128 A rows -> one load serves both operands
-                const bool diag = kPairs == 1 && td.row0 == td.col0;
+                const bool diag = kPairs == 1 && !rect && td.row0 == td.col0;
                 const uint16_t mc_mask = static_cast<uint16_t>((1u << half) | (4u << half));
                 for (int kb = 0; kb < num_kb; ++kb) {
                     {
@@ -170,10 +174,10 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const PairParam
 #pragma unroll
                         for (int b = 0; b < kPairBoxes; ++b) {
                             if (!mc_b)
-                                ptx::tma_load_2d_pair(sb + ch * kChunkBytes + b * kBoxBytes, &tmap_in, full_bar(stage),
+                                ptx::tma_load_2d_pair(sb + ch * kChunkBytes + b * kBoxBytes, &tmap_b, full_bar(stage),
                                                       w_b + ch * kChunkElems, kb * kStageK + b * kBoxRows);
                             else if (pair == 0)
-                                ptx::tma_load_2d_pair_mc(sb + ch * kChunkBytes + b * kBoxBytes, &tmap_in, full_bar(stage),
+                                ptx::tma_load_2d_pair_mc(sb + ch * kChunkBytes + b * kBoxBytes, &tmap_b, full_bar(stage),
                                                          w_b + ch * kChunkElems, kb * kStageK + b * kBoxRows, mc_mask);
                         }
                     if (++stage == kPairStages) { stage = 0; phase ^= 1u; }
@@ -194,7 +198,7 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const PairParam
             [[maybe_unused]] long long st_tempty = 0, st_full = 0;
             for (long long g = cluster_id; g < pp.n_groups; g += n_clusters) {
                 const PairGroup gd = pp.groups[g % pp.groups_per_chan];
-                const bool diag = kPairs == 1 && gd.t[0].row0 == gd.t[0].col0;      // B operand = the A buffer
+                const bool diag = kPairs == 1 && !rect && gd.t[0].row0 == gd.t[0].col0;      // B operand = the A buffer
                 for (int kb0 = 0; kb0 < num_kb; kb0 += kb_per_chunk) {
                     const int kb1 = kb0 + kb_per_chunk < num_kb ? kb0 + kb_per_chunk : num_kb;
                     const uint32_t d_tmem = tmem_base + acc * kTileCols;
@@ -256,7 +260,7 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const PairParam
             if (r0 < M2 && !(kPairs == 2 && pair == 1 && gd.share == 3)) {
                 int i_max = (r0 + 127) / (2 * prm.n_pol);
                 if (i_max > prm.n_station - 1) i_max = prm.n_station - 1;
-                need = (i_max + 1) * 2 * prm.n_pol - td.col0;
+                need = (rect ? M2b : (i_max + 1) * 2 * prm.n_pol) - td.col0;
                 if (need > kTileCols) need = kTileCols;
                 if (need < 0) need = 0;
             }

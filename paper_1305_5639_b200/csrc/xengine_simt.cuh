@@ -14,6 +14,10 @@ struct Params {
     long long n_baseline;
     long long n_vis;     // n_chan * n_baseline * n_pol * n_pol
     int accumulate;
+    // rectangular cross-only mode: second stream from in_b ([T][C][n_station_b][P]); n_baseline is then
+    // n_station * n_station_b and visibilities are ordered [c][i][j][p][q].  n_station_b == 0: packed triangle of `in`.
+    const void* in_b;
+    int n_station_b;
 };
 
 __device__ __forceinline__ void decode_baseline(long long b, int& i, int& j) {
@@ -36,16 +40,25 @@ __global__ void xengine_simt_kernel(const Params prm) {
         const long long b = cb % prm.n_baseline;
         const int c = static_cast<int>(cb / prm.n_baseline);
         int i, j;
-        decode_baseline(b, i, j);
-        const long long pitch = static_cast<long long>(C) * N * P;          // samples per time step
+        const bool rect = prm.n_station_b > 0;
+        if (rect) {
+            i = static_cast<int>(b / prm.n_station_b);
+            j = static_cast<int>(b % prm.n_station_b);
+        } else {
+            decode_baseline(b, i, j);
+        }
+        const int Nb = rect ? prm.n_station_b : N;
+        const long long pitch = static_cast<long long>(C) * N * P;          // samples per time step of the first stream
+        const long long pitch_b = static_cast<long long>(C) * Nb * P;
         const long long ia = (static_cast<long long>(c) * N + i) * P + p;
-        const long long ib = (static_cast<long long>(c) * N + j) * P + q;
+        const long long ib = (static_cast<long long>(c) * Nb + j) * P + q;
         if constexpr (kFloat) {
             const __half2* x = static_cast<const __half2*>(prm.in);
+            const __half2* xb = rect ? static_cast<const __half2*>(prm.in_b) : x;
             double re = 0.0, im = 0.0;
             for (int t = 0; t < prm.n_time; ++t) {
                 const float2 a = __half22float2(x[t * pitch + ia]);
-                const float2 bb = __half22float2(x[t * pitch + ib]);
+                const float2 bb = __half22float2(xb[t * pitch_b + ib]);
                 re += static_cast<double>(a.x) * bb.x + static_cast<double>(a.y) * bb.y;
                 im += static_cast<double>(a.x) * bb.y - static_cast<double>(a.y) * bb.x;
             }
@@ -55,10 +68,11 @@ __global__ void xengine_simt_kernel(const Params prm) {
             *o = r;
         } else {
             const char2* x = static_cast<const char2*>(prm.in);
+            const char2* xb = rect ? static_cast<const char2*>(prm.in_b) : x;
             int re = 0, im = 0;
             for (int t = 0; t < prm.n_time; ++t) {
                 const char2 a = x[t * pitch + ia];
-                const char2 bb = x[t * pitch + ib];
+                const char2 bb = xb[t * pitch_b + ib];
                 re += a.x * bb.x + a.y * bb.y;
                 im += a.x * bb.y - a.y * bb.x;
             }

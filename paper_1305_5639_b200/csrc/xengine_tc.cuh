@@ -65,6 +65,9 @@ struct Params {
     void* out;               // DEVICE: packed output
     int accumulate;
     int k_chunk;             // samples per TMEM accumulation pass (multiple of the pipeline stage)
+    // rectangular cross-only mode: rows are the n_station streams of group A (conjugated), columns the
+    // n_station_b stations (M_b = n_station_b * n_pol streams) of group B; 0 = triangular HERK of one group
+    int n_station_b, M_b;
     // 1-CTA kernel: a stage holds [b_chunks 128-byte-wide B chunks][A chunks, only if some tile is off the diagonal]
     int n_stages, stage_bytes, b_chunks;
 #ifdef CORR_STATS
@@ -146,6 +149,7 @@ __device__ __forceinline__ void drain_accumulator(const Params& prm, int c, int 
     uint8_t* out8 = static_cast<uint8_t*>(prm.out);
     struct { int col0; } td{col0};
     const int kc = first_pass ? 0 : 1;
+    const bool rect = prm.n_station_b > 0;
     const uint64_t policy = ptx::policy_evict_first();
     if (P == 2) {
         // ---- fast path: station rows are 32-byte aligned runs; bulk async store / reduce-add ----
@@ -195,10 +199,12 @@ __device__ __forceinline__ void drain_accumulator(const Params& prm, int c, int 
                 const int j0 = (td.col0 + h0) >> 2;                       // first station of this pass
                 int cnt = (h_end - h0) >> 2;                              // stations staged in this pass
                 if (cnt > kEpiCols / 4) cnt = kEpiCols / 4;
-                if (cnt > i_row - j0 + 1) cnt = i_row - j0 + 1;           // triangle: j <= i
+                const int j_end = rect ? prm.n_station_b : i_row + 1;     // triangle: j <= i; rectangle: every j of group B
+                if (cnt > j_end - j0) cnt = j_end - j0;
                 if (i_row < prm.n_station && cnt > 0) {
-                    uint8_t* dst = out8 + ((static_cast<long long>(c) * prm.n_baseline +
-                                            static_cast<long long>(i_row) * (i_row + 1) / 2 + j0) << 5);
+                    const long long row = rect ? (static_cast<long long>(c) * prm.n_station + i_row) * prm.n_station_b
+                                               : static_cast<long long>(c) * prm.n_baseline + static_cast<long long>(i_row) * (i_row + 1) / 2;
+                    uint8_t* dst = out8 + ((row + j0) << 5);
                     const uint32_t src = sbuf + lane * kEpiRowBytes;
                     const uint32_t bytes = static_cast<uint32_t>(cnt) << 5;
                     if (!reduce) ptx::bulk_store(dst, src, bytes, policy);
@@ -215,8 +221,10 @@ __device__ __forceinline__ void drain_accumulator(const Params& prm, int c, int 
         const int i = m / P, p = m - i * P;
         const bool row_ok = m < prm.M;
         // word offset of (c, b(i,0), p, q=0); b(i,j) = i(i+1)/2 + j
-        const long long row_base =
-            ((static_cast<long long>(c) * prm.n_baseline + static_cast<long long>(i) * (i + 1) / 2) * P + p) * P * 2;
+        const long long row = rect ? (static_cast<long long>(c) * prm.n_station + i) * prm.n_station_b
+                                   : static_cast<long long>(c) * prm.n_baseline + static_cast<long long>(i) * (i + 1) / 2;
+        const long long row_base = (row * P + p) * P * 2;
+        const int n_cols = rect ? prm.M_b : prm.M;
         uint32_t* out = static_cast<uint32_t*>(prm.out);
         if (h_begin >= h_end) {
             ptx::tc_fence_before();
@@ -239,7 +247,7 @@ __device__ __forceinline__ void drain_accumulator(const Params& prm, int c, int 
             for (int y = 0; y < 8; ++y) {
                 const int n = n0 + 2 * y + ri;
                 const int j = n / P, q = n - j * P;
-                if (row_ok && n < prm.M && j <= i) {
+                if (row_ok && n < n_cols && (rect || j <= i)) {
                     uint2* dst = reinterpret_cast<uint2*>(out + row_base + (static_cast<long long>(j) * P * P + q) * 2);
                     uint2 val = make_uint2(re[y], im[y]);
                     if (reduce) {

@@ -323,3 +323,82 @@ def test_config4_full_size_four_calls(corr, oracle):
 @pytest.mark.parametrize("N", [32, 128, 512, 1024])
 def test_config5_sweep_points(corr, oracle, N):
     check_full_config(corr, oracle, "cfg5_n%d" % N, 4 if N <= 128 else 2)
+
+
+# ---------------------------------------------------------------------------------------------
+# rectangular cross-only X-engine (corr_xengine_cross) against oracle.xengine_cross
+# ---------------------------------------------------------------------------------------------
+def run_cross(corr, xa, xb, dtype, calls=1, kernel=None):
+    T, C, Na, P, _ = xa.shape
+    Nb = xb.shape[2]
+    with corr.CrossCorrelator(Na, Nb, P, C, T, dtype) as h:
+        if kernel is not None:
+            h.set_kernel(kernel)
+            assert h.kernel == kernel
+        out = None
+        for k in range(calls):
+            out = h.xengine_cross(xa.cuda(), xb.cuda(), out, accumulate=k > 0)
+        torch.cuda.synchronize()
+        return out.cpu().numpy(), h.kernel
+
+
+CROSS_CASES = [(1, 1, 1, 1, 1), (4, 4, 2, 3, 70), (16, 48, 2, 5, 130), (64, 64, 2, 4, 200), (72, 136, 2, 2, 129),
+               (200, 60, 2, 2, 64), (130, 70, 1, 3, 96), (33, 8, 2, 2, 50), (128, 256, 2, 2, 257)]
+
+
+@pytest.mark.parametrize("kernel", [None, "simt"])
+@pytest.mark.parametrize("Na,Nb,P,C,T", CROSS_CASES)
+def test_cross_ci8_bit_exact(corr, oracle, kernel, Na, Nb, P, C, T):
+    xa = inputs.gauss_ci8(T, C, Na, P, 40.0, seed=7300 + Na)
+    xb = inputs.gauss_ci8(T, C, Nb, P, 40.0, seed=7400 + Nb)
+    got, used = run_cross(corr, xa, xb, "ci8", calls=2, kernel=kernel)
+    tma = (Na * P * 2) % 16 == 0 and (Nb * P * 2) % 16 == 0
+    assert used == ("pair" if tma and kernel is None else "simt")
+    want = oracle.xengine_cross(xa.numpy(), xb.numpy())
+    want = oracle.xengine_cross(xa.numpy(), xb.numpy(), accumulate_into=want)
+    assert got.dtype == np.int32 and got.shape == want.shape
+    bad = np.argwhere(got.astype(np.int64) != want)
+    assert bad.size == 0, "first mismatches (c,i,j,p,q,reim): %s" % bad[:8].tolist()
+
+
+@pytest.mark.parametrize("Na,Nb,P,C,T", [(24, 40, 2, 3, 100), (64, 160, 2, 2, 2100), (96, 32, 1, 2, 1030)])
+def test_cross_cf16_within_tolerance(corr, oracle, Na, Nb, P, C, T):
+    x = inputs.corr_phase_cf16(T, C, Na + Nb, P, seed=7500 + Na)      # one sky, two station groups
+    xa, xb = x[:, :, :Na].contiguous(), x[:, :, Na:].contiguous()
+    got, used = run_cross(corr, xa, xb, "cf16")
+    assert used == "pair"
+    want = oracle.xengine_cross(xa.numpy(), xb.numpy())
+    # |dV_ij| <= 2e-5 sqrt(V_ii V_jj): autocorrelations of each group from the (pinned) triangle oracle
+    auto_a = oracle.xengine(xa.numpy())[:, [i * (i + 1) // 2 + i for i in range(Na)]]
+    auto_b = oracle.xengine(xb.numpy())[:, [j * (j + 1) // 2 + j for j in range(Nb)]]
+    pa = np.stack([auto_a[:, :, p, p, 0] for p in range(P)], axis=-1)           # [C, Na, P]
+    pb = np.stack([auto_b[:, :, q, q, 0] for q in range(P)], axis=-1)           # [C, Nb, P]
+    d = got.astype(np.float64) - want
+    err = np.sqrt(d[..., 0] ** 2 + d[..., 1] ** 2) / np.sqrt(pa[:, :, None, :, None] * pb[:, None, :, None, :])
+    assert err.max() <= FP16_TOL, "normalised error %.3g" % err.max()
+
+
+def test_cross_matches_the_triangle_kernel_block(corr):
+    """GPU against GPU: the rectangle of stations [k, N) x [0, k) equals the triangle kernel's off-diagonal block."""
+    T, C, N, P, k = 256, 3, 96, 2, 40
+    x = inputs.gauss_ci8(T, C, N, P, 30.0, seed=7600)
+    tri, _ = run_gpu(corr, [x], "ci8")
+    got, _ = run_cross(corr, x[:, :, k:].contiguous(), x[:, :, :k].contiguous(), "ci8")
+    for i in range(k, N):
+        assert (got[:, i - k] == tri[:, i * (i + 1) // 2: i * (i + 1) // 2 + k]).all()
+
+
+def test_cross_argument_errors(corr):
+    with corr.CrossCorrelator(8, 16, 2, 2, 64, "ci8") as h, corr.Correlator(8, 2, 2, 64, "ci8") as g:
+        L = corr.lib()
+        xa = torch.zeros(h.input_shape(), dtype=torch.int8, device="cuda")
+        xb = torch.zeros(h.input_shape_b(), dtype=torch.int8, device="cuda")
+        out = h.empty_output()
+        assert h.input_bytes == xa.numel() and h.input_bytes_b == xb.numel() and h.output_bytes == out.numel() * 4
+        assert L.corr_xengine(h._h, xa.data_ptr(), out.data_ptr(), 0, None) == corr.CORR_EINVAL        # wrong entry point
+        assert L.corr_xengine_cross(g._h, xa.data_ptr(), xb.data_ptr(), out.data_ptr(), 0, None) == corr.CORR_EINVAL
+        assert L.corr_xengine_cross(h._h, xa.data_ptr(), None, out.data_ptr(), 0, None) == corr.CORR_EINVAL
+        assert L.corr_xengine_cross(h._h, xa.data_ptr(), xb.data_ptr() + 2, out.data_ptr(), 0, None) == corr.CORR_EINVAL
+        with pytest.raises(corr.CorrError):
+            h.set_kernel("single")
+    assert not corr.lib().corr_create_cross(4, 0, 2, 1, 1, 0)
