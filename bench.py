@@ -69,13 +69,13 @@ def workload(name):
     from paper_1305_5639_b200 import inputs
     cfg = dict(inputs.CONFIGS[name])
     N, P, C, T = cfg["N"], cfg["P"], cfg["C"], cfg["T"]
-    B = N * (N + 1) // 2
+    B = N * cfg["Nb"] if cfg.get("Nb") else N * (N + 1) // 2       # rectangle (cross workload) or packed triangle
     cfg["name"] = name
     cfg["n_baseline"] = B
     cfg["cmacs_per_call"] = C * T * B * P * P
     cfg["ops_per_call"] = 8 * cfg["cmacs_per_call"]
     elt = 2 if cfg["dtype"] == "ci8" else 4
-    cfg["in_bytes"] = T * C * N * P * elt
+    cfg["in_bytes"] = T * C * (N + cfg.get("Nb", 0)) * P * elt
     cfg["out_bytes"] = C * B * P * P * 8
     return cfg
 
@@ -144,7 +144,7 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------
 # CPU oracle legs (the ONLY places bench.py touches oracle/)
 # ------------------------------------------------------------------------------------------------
-def oracle_sample_rate(cfg, x_host, min_seconds):
+def oracle_sample_rate(cfg, x_host, min_seconds, xb_host=None):
     """Times oracle.xengine on whole channels of `x_host` ([T, n, N, P, 2] numpy) -> (CMAC/s, seconds, channels)."""
     import oracle
     n = x_host.shape[1]
@@ -152,7 +152,10 @@ def oracle_sample_rate(cfg, x_host, min_seconds):
     done, secs = 0, 0.0
     while True:
         t0 = time.perf_counter()
-        oracle.xengine(x_host)
+        if xb_host is None:
+            oracle.xengine(x_host)
+        else:
+            oracle.xengine_cross(x_host, xb_host)
         secs += time.perf_counter() - t0
         done += n
         if secs >= min_seconds or done >= 64 * n:
@@ -176,12 +179,17 @@ def run_reference(args):
     cores = oracle.max_threads()
     n_chan = max(1, min(cfg["C"], cores))
     x = cpu_sample_input(cfg, n_chan)
+    xb = None
+    if cfg.get("Nb"):
+        from paper_1305_5639_b200 import inputs
+        xb = inputs.make_input_b(cfg, call=0, device="cpu", C=n_chan).numpy()
+    run = (lambda: oracle.xengine(x)) if xb is None else (lambda: oracle.xengine_cross(x, xb))
     cm_per_chan = cfg["cmacs_per_call"] // cfg["C"]
     for _ in range(max(0, min(args.warmup, 1))):          # one warm-up pass is plenty for a CPU loop
-        oracle.xengine(x)
+        run()
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        oracle.xengine(x)
+        run()
     secs = time.perf_counter() - t0
     tops = 8.0 * args.steps * n_chan * cm_per_chan / secs / 1e12
     sample = "%d of %d channels of %s call 0 per step (all %d baselines x %d pol products, full T=%d)" % (
@@ -236,6 +244,11 @@ def library_gemm_peak(torch, dtype, n=8192, secs=2.0):
 
 
 def describe(cfg):
+    if cfg.get("Nb"):
+        return ("%s: rectangle of %d x %d stations (cross-correlations only, PAPER.md:79), %d pol, %d channels, T=%d samples/call, "
+                "complex %s -> %s [c][i][j][p][q]" % (cfg["name"], cfg["N"], cfg["Nb"], cfg["P"], cfg["C"], cfg["T"],
+                                                      "int8" if cfg["dtype"] == "ci8" else "fp16",
+                                                      "int32" if cfg["dtype"] == "ci8" else "fp32"))
     return ("%s: N=%d stations, %d pol, %d channels, T=%d samples/call, %d call(s) integrated (accumulate 0,1,..), "
             "complex %s -> %s packed triangle" % (cfg["name"], cfg["N"], cfg["P"], cfg["C"], cfg["T"], cfg["calls"],
                                                     "int8" if cfg["dtype"] == "ci8" else "fp16",
@@ -320,7 +333,9 @@ def run_native(args):
 
     # every rank is an independent replica on its own seeded inputs (replicas only; no sharding)
     xs = [inputs.make_input(cfg, call=k, device="cuda") for k in range(calls)]
-    h = binding.Correlator(N, P, C, T, dtype)
+    cross = bool(cfg.get("Nb"))
+    xbs = [inputs.make_input_b(cfg, call=k, device="cuda") for k in range(calls)] if cross else None
+    h = binding.CrossCorrelator(N, cfg["Nb"], P, C, T, dtype) if cross else binding.Correlator(N, P, C, T, dtype)
     if args.kernel != "auto":
         h.set_kernel(args.kernel)
     kernel = h.kernel
@@ -337,7 +352,10 @@ def run_native(args):
         for k in range(calls):
             if ev is not None:
                 ev[2 * k].record()
-            h.xengine(xs[k], out, accumulate=k > 0)
+            if cross:
+                h.xengine_cross(xs[k], xbs[k], out, accumulate=k > 0)
+            else:
+                h.xengine(xs[k], out, accumulate=k > 0)
             if ev is not None:
                 ev[2 * k + 1].record()
 
@@ -373,7 +391,7 @@ def run_native(args):
 
     # ---- e2e: HOST pinned buffers through corr_xengine_host --------------------------------------
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not cross:          # the host-buffer entry point exists for corr_xengine only
         Ke = args.e2e_steps or min(K, 5)
         xh = [x.cpu().pin_memory() for x in xs]
         oh = torch.empty(h.output_shape(), dtype=out.dtype).pin_memory()
@@ -438,7 +456,8 @@ def run_native(args):
         cores = oracle.max_threads()
         n_chan = max(1, min(C, cores))
         x_host = xs[0][:, :n_chan].contiguous().cpu().numpy()      # the same bytes the GPU consumed
-        rate, secs, done = oracle_sample_rate(cfg, x_host, min_seconds=10.0)
+        xb_host = xbs[0][:, :n_chan].contiguous().cpu().numpy() if cross else None
+        rate, secs, done = oracle_sample_rate(cfg, x_host, min_seconds=10.0, xb_host=xb_host)
         cpu = {"value": 8.0 * rate / 1e12, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": "channels 0..%d of call 0 (all %d baselines x %d pol products, full T=%d), %d channel passes in %.1f s"
                          % (n_chan - 1, cfg["n_baseline"], P * P, T, done, secs),

@@ -117,6 +117,17 @@ for _n in (32, 64, 128, 256, 512, 1024):
                                     sigma=20.0, seed=1500 + int(math.log2(_n)), calls=1)
 
 
+# the rectangle a space-division node processes: two groups of 256 dual-pol stations
+# (N here is group A, Nb group B; group B is drawn with seed + 500), values as config 5.
+CONFIGS["cross_n256"] = dict(N=256, Nb=256, P=2, C=512, T=2048, dtype="ci8", recipe="gauss", sigma=20.0, seed=1600, calls=1)
+
+
+def make_input_b(cfg, call=0, device="cpu", T=None, C=None):
+    """Group B of a cross workload (same recipe, Nb stations, its own seed)."""
+    cfg_b = dict(cfg, N=cfg["Nb"], seed=cfg["seed"] + 500)
+    return make_input(cfg_b, call, device, T, C)
+
+
 def make_input(cfg, call=0, device="cpu", T=None, C=None):
     """Input tensor of one call of a config (dict from CONFIGS); T / C may be overridden to
     cut a smaller case of the same recipe (used by CPU-sized parity tests)."""
