@@ -49,6 +49,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     cmd = [_nvcc()] + NVCC_FLAGS + ["-I", INCLUDE]
     if verbose:
         cmd += ["-Xptxas", "-v"]
+    if os.environ.get("CORR_DEFINES"):        # developer build: extra -D switches for A/B experiments
+        cmd += os.environ["CORR_DEFINES"].split()
     if os.environ.get("CORR_STATS"):          # developer build: per-role stall counters (clock64) in the pair kernel
         cmd += ["-DCORR_STATS"]
     cmd += _sources() + ["-o", LIB + ".tmp"]

@@ -21,7 +21,8 @@
 
 namespace {
 
-constexpr long long kMaxIntegrationCi8 = 65535;   // 2 * 128^2 * T_total <= 2^31 - 1
+constexpr long long kMaxIntegrationCi8 = 65535;
+constexpr unsigned kSchedRing = 256;            // launches in flight on different streams never share a feed counter   // 2 * 128^2 * T_total <= 2^31 - 1
 
 thread_local char g_create_error[512] = "";
 
@@ -49,6 +50,8 @@ struct corr_plan {
     xtc::TileDesc* d_tiles;
     std::vector<xtc::PairGroup> h_groups[2];   // [0]: one pair per cluster, [1]: two pairs per cluster (multicast)
     xtc::PairGroup* d_groups[2];
+    unsigned int* d_sched;                     // ring of tile-feed counters, one per launch (kSchedRing)
+    unsigned int sched_seq;
     int max_clusters[2];                       // co-resident clusters of 2 / 4 CTAs (cudaOccupancyMaxActiveClusters)
     EncodeTiledFn encode;
 
@@ -307,7 +310,10 @@ int launch_pair(corr_plan* h, const void* in, const void* in_b, void* out, int a
     pp.groups_per_chan = static_cast<int>(h->h_groups[v].size());
     pp.n_groups = static_cast<long long>(pp.groups_per_chan) * h->C;
     const unsigned clusters = static_cast<unsigned>(pp.n_groups < h->max_clusters[v] ? pp.n_groups : h->max_clusters[v]);
-    cudaError_t e;
+    if (pp.n_groups > (1ll << 31) - 4096) return fail(h, CORR_EINVAL, "xengine_pair_kernel: %lld tiles exceed the tile feed's range", pp.n_groups);
+    pp.sched_counter = h->d_sched + (h->sched_seq++ % kSchedRing);
+    cudaError_t e = cudaMemsetAsync(pp.sched_counter, 0, sizeof(unsigned int), st);
+    if (e != cudaSuccess) return fail_cuda(h, e, "tile-feed counter reset");
     if (h->dtype == CORR_CI8)
         e = v ? launch_pair_kernel<1, 2>(h->tmap_pair, map_b, pp, clusters, st) : launch_pair_kernel<1, 1>(h->tmap_pair, map_b, pp, clusters, st);
     else
@@ -323,6 +329,9 @@ int launch_pair(corr_plan* h, const void* in, const void* in_b, void* out, int a
         for (int b = 0; b < nb; ++b) for (int k = 0; k < 8; ++k) a[k] += static_cast<double>(hs[b * 8 + k]) / nb;
         double lead_tempty = 0, lead_full = 0;
         for (int b = 0; b < nb; b += 2) { lead_tempty += hs[b * 8 + 2] / (nb / 2.0); lead_full += hs[b * 8 + 3] / (nb / 2.0); }
+        double tmin = 1e30, tmax = 0;
+        for (int b = 0; b < nb; ++b) { if (hs[b * 8] < tmin) tmin = hs[b * 8]; if (hs[b * 8] > tmax) tmax = hs[b * 8]; }
+        fprintf(stderr, "[corr stats] producer loop clk: min %.0f max %.0f (spread %.1f %%)\n", tmin, tmax, 100.0 * (tmax - tmin) / tmax);
         fprintf(stderr, "[corr stats] clk/CTA: total %.0f | producer wait empty %.0f | mma wait tmem-empty %.0f, wait full %.0f | epi(warp2) wait tmem-full %.0f, drain %.0f\n",
                 a[0], a[1], lead_tempty, lead_full, a[4], a[5]);
     }
@@ -469,6 +478,8 @@ static corr_handle create_plan(int n_station, int n_station_b, int n_pol, int n_
     h->d_tiles = nullptr;
     h->kernel = CORR_KERNEL_AUTO;
     h->d_groups[0] = h->d_groups[1] = nullptr;
+    h->d_sched = nullptr;
+    h->sched_seq = 0;
     h->max_clusters[0] = h->max_clusters[1] = 0;
     h->encode = nullptr;
     h->tmap_in_ptr = nullptr;
@@ -505,6 +516,12 @@ static corr_handle create_plan(int n_station, int n_station_b, int n_pol, int n_
             e = cudaFuncSetAttribute(xtc::xengine_direct_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, xtc::kSmemBytes);
         if (e != cudaSuccess) {
             fail(nullptr, CORR_ECUDA, "corr_create: cudaFuncSetAttribute(smem): %s", cudaGetErrorString(e));
+            corr_destroy(h);
+            return nullptr;
+        }
+        e = cudaMalloc(&h->d_sched, kSchedRing * sizeof(unsigned int));
+        if (e != cudaSuccess) {
+            fail(nullptr, CORR_ENOMEM, "corr_create: tile-feed counters: %s", cudaGetErrorString(e));
             corr_destroy(h);
             return nullptr;
         }
@@ -562,6 +579,7 @@ corr_handle corr_create_cross(int n_station_a, int n_station_b, int n_pol, int n
 void corr_destroy(corr_handle h) {
     if (!h) return;
     if (h->d_tiles) cudaFree(h->d_tiles);
+    if (h->d_sched) cudaFree(h->d_sched);
     if (h->d_groups[0]) cudaFree(h->d_groups[0]);
     if (h->d_groups[1]) cudaFree(h->d_groups[1]);
     if (h->d_ws) cudaFree(h->d_ws);

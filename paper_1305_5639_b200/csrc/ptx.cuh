@@ -76,7 +76,11 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst_smem, const CUtensorMap
 // input tiles other CTAs are about to re-read out of L2
 __device__ __forceinline__ uint64_t policy_evict_first() {
     uint64_t p;
+#ifdef CORR_AB_EVICT_NORMAL
+    asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
+#else
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+#endif
     return p;
 }
 __device__ __forceinline__ void bulk_store(void* dst_gmem, uint32_t src_smem, uint32_t bytes, uint64_t policy) {
@@ -206,6 +210,41 @@ __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
 }
 // In a CTA pair the two CTAs' shared::cluster windows differ in one address bit; clearing it turns the
 // address of a barrier in this CTA into the address of the same barrier in the pair's even (leader) CTA.
+// ---- cluster-scope pieces of the dynamic tile feed (xengine_pair.cuh) ----------------------------------------
+__device__ __forceinline__ void st_shared_cluster_u32(uint32_t cluster_addr, uint32_t v) {
+    asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(cluster_addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t ld_shared_u32(uint32_t addr) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ void fence_acq_rel_cluster() { asm volatile("fence.acq_rel.cluster;" ::: "memory"); }
+// relaxed arrive that cannot issue before `dep` (a value just loaded from the slot the arrival frees) is available
+__device__ __forceinline__ void mbar_arrive_cluster_after(uint32_t cluster_addr, uint32_t dep) {
+    asm volatile("{\n\t.reg .b32 t;\n\tand.b32 t, %1, 0;\n\tadd.u32 t, t, %0;\n\t"
+                 "mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [t];\n\t}" ::"r"(cluster_addr), "r"(dep) : "memory");
+}
+// wait with cluster-scope acquire: the waiter then sees shared-memory data a remote CTA stored before its arrive
+__device__ __forceinline__ bool mbar_try_wait_cluster(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity) {
+    if (mbar_try_wait_cluster(bar, parity)) return;
+    const long long t0 = clock64();
+    uint32_t spins = 0;
+    while (!mbar_try_wait_cluster(bar, parity)) {
+        if ((++spins & 0x3ffu) == 0 && clock64() - t0 > (1ll << 32)) __trap();
+    }
+}
 constexpr uint32_t kPeerBitMask = 0xFEFFFFFFu;
 // 2-D tiled load into THIS CTA's shared memory whose completion bytes are counted on the PAIR LEADER's mbarrier.
 __device__ __forceinline__ void tma_load_2d_pair(uint32_t dst_smem, const CUtensorMap* map, uint32_t bar,
