@@ -41,8 +41,11 @@ FALLBACK_HBM_GBS = 6650.0
 # DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum) of ONE xengine_direct_kernel launch from
 # the committed `ncu --set full` capture of this workload (profiles/), or None where not captured.
 NCU_TRAFFIC_BYTES = {
-    # profiles/r1b_cfg4_ncu_pair_kernel.md: 4.09 GB (accumulate = 0) and 5.08 GB (accumulate = 1) -> mean of the step's 4 calls
-    "cfg4": (4.086e9 + 3 * 5.078e9) / 4,
+    # profiles/r1c_final_ncu_pair_feed.md (dram__bytes_read.sum + dram__bytes_write.sum of one launch)
+    "cfg4": (3.198e9 + 3 * 4.275e9) / 4,          # accumulate = 0 once, accumulate = 1 three times per step
+    "cfg3": 4.651e9,
+    "cfg5_n64": 1.200e9,
+    "cfg5_n32": 1.139e9,
 }
 
 
