@@ -11,11 +11,12 @@
 // channel sharing a column block (or a row block) form a 4-CTA cluster and fetch the shared operand ONCE
 // with a multicast TMA load: 128 + 64 bytes per CTA and sample.
 //
-// Roles per CTA (320 threads, one CTA per SM, persistent; both CTAs of a pair walk the same tile list):
+// Roles per CTA (320 threads, one CTA per SM, persistent; the tiles come from the dynamic TileFeed below):
 //   warp 0      TMA producer (one lane): its 128 A rows and its 128 B columns of every pipeline stage; completion
 //               bytes of both CTAs are counted on the pair LEADER's `full` barrier
 //   warp 1      TMEM allocator (both CTAs) + tcgen05.mma.cta_group::2 issuer (one lane of the leader CTA);
-//               tcgen05.commit multicasts the `empty` (all CTAs of the cluster) and `tmem full` (the pair) arrivals
+//               tcgen05.commit multicasts the `empty` (all CTAs of the cluster) and `tmem full` (the pair) arrivals;
+//               in cluster rank 1 (no MMAs to issue) the same lane is the tile-feed writer
 //   warps 2..9  epilogue of this CTA's 128 TMEM lanes (drain_accumulator in xengine_tc.cuh); they release the
 //               accumulator by arriving on the leader's `tmem empty` barrier through shared::cluster
 #pragma once
