@@ -115,6 +115,20 @@ corr_handle corr_create_cross(int n_station_a, int n_station_b, int n_pol, int n
 int corr_xengine_cross(corr_handle h, const void* in_a, const void* in_b, void* out, int accumulate, void* stream);
 size_t corr_input_bytes_b(corr_handle h);    /* cross plans: T*C*Nb*P * (2 or 4); else 0 */
 
+/*
+ * corr_fengine -- the F-engine in front of the X-engine.  PAPER.md:49-52 (Sec. 2, Eq. 1):
+ *     S[k] = sum_{n=0}^{N-1} s[n] exp(-j (2 pi / N) k n),   N = 256 ("An FFT length of 256 is used across all tests",
+ * PAPER.md:176), applied to consecutive non-overlapping blocks of each stream's 8-bit REAL samples.
+ *   in    DEVICE, 16-byte aligned: int8 [n_stream][n_spectra * 256], each stream contiguous in time.
+ *   out   DEVICE, 4-byte aligned: complex fp16 (re, im) [n_spectra][128][n_stream]: the 128 non-redundant channels
+ *         k = 0..127 of every block (real input: S[256 - k] = conj(S[k]); the Nyquist bin is dropped), raw sums
+ *         (|S| <= 128 * 256 fits fp16), computed in fp32 and rounded to nearest.  With n_stream = n_station * n_pol
+ *         (stream m = s * n_pol + p) this IS corr_xengine's CORR_CF16 input [n_time = n_spectra][n_chan = 128]
+ *         [n_station][n_pol]: no corner turn between the engines.
+ * Stateless (no handle), asynchronous on `stream`; CORR_OK or a negative code, message via corr_last_error(NULL).
+ */
+int corr_fengine(const void* in, void* out, int n_stream, long long n_spectra, void* stream);
+
 /* corr_destroy -- frees the handle and everything it owns.  NULL is a no-op. */
 void corr_destroy(corr_handle h);
 

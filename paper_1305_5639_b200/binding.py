@@ -26,6 +26,7 @@ SYMBOLS = {
     "corr_create_cross": (_vp, [_i, _i, _i, _i, _i, _i]),
     "corr_xengine_cross": (_i, [_vp, _vp, _vp, _vp, _i, _vp]),
     "corr_input_bytes_b": (_sz, [_vp]),
+    "corr_fengine": (_i, [_vp, _vp, _i, _ll, _vp]),
     "corr_destroy": (None, [_vp]),
     "corr_input_bytes": (_sz, [_vp]),
     "corr_output_bytes": (_sz, [_vp]),
@@ -85,6 +86,24 @@ def _stream_ptr(stream):
         import torch
         stream = torch.cuda.current_stream()
     return ctypes.c_void_p(getattr(stream, "cuda_stream", stream))
+
+
+def fengine(samples, out=None, stream=None):
+    """corr_fengine: int8 real samples [n_stream, n_spectra * 256] (CUDA) -> complex fp16 [n_spectra, 128, n_stream, 2]."""
+    import torch
+    if samples.dtype != torch.int8 or samples.dim() != 2 or samples.shape[1] % 256 or not samples.is_contiguous() \
+            or samples.device.type != "cuda":
+        raise ValueError("samples must be a contiguous CUDA int8 tensor [n_stream, n_spectra * 256]")
+    n_stream, n_spec = samples.shape[0], samples.shape[1] // 256
+    if out is None:
+        out = torch.empty((n_spec, 128, n_stream, 2), dtype=torch.float16, device=samples.device)
+    if out.dtype != torch.float16 or tuple(out.shape) != (n_spec, 128, n_stream, 2) or not out.is_contiguous():
+        raise ValueError("out must be a contiguous float16 tensor [n_spectra, 128, n_stream, 2]")
+    L = lib()
+    rc = L.corr_fengine(samples.data_ptr(), out.data_ptr(), n_stream, n_spec, _stream_ptr(stream))
+    if rc != CORR_OK:
+        raise CorrError(rc, L.corr_last_error(None).decode())
+    return out
 
 
 class Correlator:

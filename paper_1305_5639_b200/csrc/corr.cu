@@ -15,6 +15,7 @@
 #include <vector>
 
 #include "corner_turn.cuh"
+#include "fengine.cuh"
 #include "xengine_simt.cuh"
 #include "xengine_tc.cuh"
 #include "xengine_pair.cuh"
@@ -612,6 +613,25 @@ int corr_set_kernel(corr_handle h, int kernel) {
     return CORR_OK;
 }
 int corr_last_launch_count(corr_handle h) { return h ? h->last_launches : CORR_EINVAL; }
+
+int corr_fengine(const void* in, void* out, int n_stream, long long n_spectra, void* stream) {
+    g_create_error[0] = 0;
+    if (!in || !out || n_stream < 1 || n_spectra < 1 || n_spectra > 0x7fffffffLL ||
+        (n_stream + feng::kStreamsPerBlock - 1) / feng::kStreamsPerBlock > 65535)
+        return fail(nullptr, CORR_EINVAL, "corr_fengine: invalid arguments (n_stream=%d, n_spectra=%lld)", n_stream, n_spectra);
+    if ((reinterpret_cast<uintptr_t>(in) & 15) || (reinterpret_cast<uintptr_t>(out) & 3))
+        return fail(nullptr, CORR_EINVAL, "corr_fengine: `in` must be 16-byte and `out` 4-byte aligned");
+    feng::Params prm;
+    prm.in = static_cast<const int8_t*>(in);
+    prm.out = static_cast<__half2*>(out);
+    prm.n_stream = n_stream;
+    prm.n_spectra = n_spectra;
+    const dim3 grid(static_cast<unsigned>(n_spectra), static_cast<unsigned>((n_stream + feng::kStreamsPerBlock - 1) / feng::kStreamsPerBlock));
+    feng::fengine_kernel<<<grid, feng::kThreads, 0, static_cast<cudaStream_t>(stream)>>>(prm);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(nullptr, e, "fengine_kernel launch");
+    return CORR_OK;
+}
 
 int corr_corner_turn(corr_handle h, const void* in, void* ws, void* stream) {
     if (!h) return CORR_EINVAL;

@@ -1,0 +1,90 @@
+"""GPU parity of corr_fengine (Eq. 1, N = 256) against the fp64 DFT-definition oracle, and the F -> X chain.
+
+Tolerance: the kernel computes in fp32 and rounds once to fp16, the oracle is exact to fp64:
+    |d component| <= 0.5 ulp_fp16(|exact component|) + 2e-6 * sum_n |s[n]|
+(the first term is the one rounding to the fp16 output format, the second bounds the fp32 round-off of an 8-stage
+256-point transform: log2(256) * 2^-23 * sum|s| = 9.5e-7 sum|s|, doubled).
+"""
+import numpy as np
+import pytest
+import torch
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def corr():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (there is no CPU fallback)")
+    from paper_1305_5639_b200 import binding
+    binding.lib()
+    return binding
+
+
+def check(corr, s):
+    from oracle import fengine as fo
+    got = corr.fengine(torch.from_numpy(s).cuda()).cpu().numpy().astype(np.float64)       # [A, 128, M, 2]
+    want = fo.fengine(s)
+    A, K, M = want.shape
+    assert got.shape == (A, K, M, 2)
+    l1 = np.abs(s.reshape(M, A, 256).astype(np.float64)).sum(axis=2).T[:, None, :]         # [A, 1, M]
+    for part, w in ((0, want.real), (1, want.imag)):
+        ulp = np.spacing(np.abs(w).astype(np.float16)).astype(np.float64)
+        tol = 0.5 * ulp + 2e-6 * l1
+        bad = np.argwhere(np.abs(got[..., part] - w) > tol)
+        assert bad.size == 0, "part %d first mismatches (a,k,m): %s" % (part, bad[:6].tolist())
+
+
+@pytest.mark.parametrize("M,A", [(1, 1), (2, 3), (7, 2), (32, 4), (33, 5), (64, 16), (100, 9), (512, 8)])
+def test_fengine_random_full_range(corr, M, A):
+    rng = np.random.default_rng(9000 + M)
+    check(corr, rng.integers(-128, 128, size=(M, A * 256), dtype=np.int8))
+
+
+def test_fengine_exact_cases(corr):
+    n = np.arange(512)
+    s = np.zeros((6, 512), np.int8)
+    s[0, 0] = 7; s[0, 256 + 5] = 9                       # impulses
+    s[1, :] = -3                                         # DC
+    s[2, :] = np.array([100, 50, -100, -50])[n % 4]      # quarter-rate tone: channel 64 = 128 (100 - 50 j)
+    s[3, :] = 127; s[4, :] = -128                        # extreme DC: 32512 and -32768 are exact in fp16
+    s[5, :] = np.where(n % 2 == 0, 127, -128)            # lives in the dropped Nyquist bin (+ DC -128)
+    got = corr.fengine(torch.from_numpy(s).cuda()).cpu().numpy().astype(np.float64)
+    assert (got[0, :, 0, 0] == 7).all() and (got[0, :, 0, 1] == 0).all()
+    assert got[0, 0, 1, 0] == -768 and np.abs(got[:, 1:, 1]).max() <= 1e-3
+    assert got[1, 64, 2, 0] == 12800 and got[1, 64, 2, 1] == -6400
+    assert got[0, 0, 3, 0] == 127 * 256 and got[0, 0, 4, 0] == -128 * 256
+    assert got[0, 0, 5, 0] == -128 and np.abs(got[:, 1:, 5]).max() <= 0.05
+    check(corr, s)
+
+
+def test_fengine_then_xengine_chain(corr):
+    """F-engine output is consumed in place by the fp16 X-engine (no corner turn): the visibilities equal the X-engine
+    oracle applied to the F-engine's own fp16 output, within the X-engine tolerance."""
+    import oracle
+    N, P, A = 24, 2, 192
+    rng = np.random.default_rng(77)
+    s = np.clip(np.rint(rng.normal(0, 20, size=(N * P, A * 256))), -127, 127).astype(np.int8)
+    x = corr.fengine(torch.from_numpy(s).cuda())                             # [A, 128, N*P, 2] fp16
+    x5 = x.view(A, 128, N, P, 2)
+    with corr.Correlator(N, P, 128, A, "cf16") as h:
+        got = h.xengine(x5).cpu().numpy().astype(np.float64)
+    want = oracle.xengine(x5.cpu().numpy())
+    auto_b = np.array([i * (i + 1) // 2 + i for i in range(N)])
+    i_of_b = np.concatenate([np.full(i + 1, i) for i in range(N)]); j_of_b = np.concatenate([np.arange(i + 1) for i in range(N)])
+    auto = np.stack([want[:, auto_b, p, p, 0] for p in range(P)], axis=-1)
+    d = got - want
+    err = np.sqrt(d[..., 0] ** 2 + d[..., 1] ** 2) / np.sqrt(auto[:, i_of_b, :, None] * auto[:, j_of_b, None, :])
+    assert err[1:].max() <= 2e-5            # channel 0 (DC) of zero-mean noise has tiny autocorrelations; skip its ratio
+
+
+def test_fengine_argument_errors(corr):
+    L = corr.lib()
+    s = torch.zeros((4, 512), dtype=torch.int8, device="cuda")
+    out = torch.empty((2, 128, 4, 2), dtype=torch.float16, device="cuda")
+    assert L.corr_fengine(None, out.data_ptr(), 4, 2, None) == corr.CORR_EINVAL
+    assert L.corr_fengine(s.data_ptr(), out.data_ptr(), 0, 2, None) == corr.CORR_EINVAL
+    assert L.corr_fengine(s.data_ptr() + 1, out.data_ptr(), 4, 2, None) == corr.CORR_EINVAL
+    assert b"corr_fengine" in L.corr_last_error(None)
+    with pytest.raises(ValueError):
+        corr.fengine(torch.zeros((4, 500), dtype=torch.int8, device="cuda"))
