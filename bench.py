@@ -58,8 +58,9 @@ def parse_args():
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
     ap.add_argument("--kernel", default="auto", choices=["auto", "single", "pair", "quad", "simt"],
                     help="force a kernel variant (default: the library's own choice)")
-    ap.add_argument("--piece", default="xengine", choices=["xengine", "corner_turn"],
-                    help="corner_turn: time the standalone corner-turn kernel (SURVEY 8(a) a1) on the workload's input")
+    ap.add_argument("--piece", default="xengine", choices=["xengine", "corner_turn", "fengine"],
+                    help="corner_turn: time the standalone corner-turn kernel (SURVEY 8(a) a1) on the workload's input; "
+                         "fengine: time corr_fengine (SURVEY 8(f) rank 2) on 512 streams x 8192 spectra of 256 real int8 samples")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-gemm-peak", action="store_true",
@@ -306,6 +307,41 @@ def run_corner_turn(args):
                                    "algorithmic_bytes_per_launch": nbytes}}), flush=True)
 
 
+def run_fengine(args):
+    """corr_fengine alone: HBM-bound (1 byte read + 2 bytes written per real sample)."""
+    import torch
+    from paper_1305_5639_b200 import binding
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device")
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    pk = peaks()
+    M, A = 512, 8192
+    g = torch.Generator(device="cuda"); g.manual_seed(1700)
+    s = torch.clamp(torch.round(torch.randn((M, A * 256), generator=g, device="cuda") * 20.0), -127, 127).to(torch.int8)
+    out = binding.fengine(s)
+    K, W = args.steps, max(args.warmup, 3)
+    for _ in range(W):
+        binding.fengine(s, out)
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    for a, b in ev:
+        a.record(); binding.fengine(s, out); b.record()
+    torch.cuda.synchronize()
+    ms = sum(a.elapsed_time(b) for a, b in ev) / K
+    nbytes = s.numel() + out.numel() * 2
+    gbs = nbytes / (ms * 1e-3) / 1e9
+    print(json.dumps({"metric": "fengine_gbs", "value": gbs, "unit": "GB/s", "n_gpus": 1, "steps": K, "warmup": W,
+                      "ms_per_step": ms, "higher_is_better": True, "dtype": "f32", "data": "synthetic",
+                      "config": {"workload": "F-engine: %d streams x %d spectra of 256 real int8 samples (sigma 20) -> 128 complex fp16 "
+                                             "channels in the X-engine layout" % (M, A),
+                                 "l2": "input + output (%.0f MiB) larger than L2" % (nbytes / 2 ** 20),
+                                 "gsamples_per_s": s.numel() / (ms * 1e-3) / 1e9},
+                      "gpu_launches": K,
+                      "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s", "frac": gbs / pk["hbm"],
+                                   "traffic": None, "kernel": "feng::fengine_kernel", "kernel_ms": ms,
+                                   "algorithmic_bytes_per_launch": nbytes}}), flush=True)
+
+
 # ------------------------------------------------------------------------------------------------
 # native arm
 # ------------------------------------------------------------------------------------------------
@@ -488,6 +524,8 @@ def main():
         run_reference(args)
     elif args.piece == "corner_turn":
         run_corner_turn(args)
+    elif args.piece == "fengine":
+        run_fengine(args)
     else:
         run_native(args)
 

@@ -616,8 +616,7 @@ int corr_last_launch_count(corr_handle h) { return h ? h->last_launches : CORR_E
 
 int corr_fengine(const void* in, void* out, int n_stream, long long n_spectra, void* stream) {
     g_create_error[0] = 0;
-    if (!in || !out || n_stream < 1 || n_spectra < 1 || n_spectra > 0x7fffffffLL ||
-        (n_stream + feng::kStreamsPerBlock - 1) / feng::kStreamsPerBlock > 65535)
+    if (!in || !out || n_stream < 1 || n_spectra < 1 || n_spectra > 0x7fffffffLL)
         return fail(nullptr, CORR_EINVAL, "corr_fengine: invalid arguments (n_stream=%d, n_spectra=%lld)", n_stream, n_spectra);
     if ((reinterpret_cast<uintptr_t>(in) & 15) || (reinterpret_cast<uintptr_t>(out) & 3))
         return fail(nullptr, CORR_EINVAL, "corr_fengine: `in` must be 16-byte and `out` 4-byte aligned");
@@ -626,7 +625,10 @@ int corr_fengine(const void* in, void* out, int n_stream, long long n_spectra, v
     prm.out = static_cast<__half2*>(out);
     prm.n_stream = n_stream;
     prm.n_spectra = n_spectra;
-    const dim3 grid(static_cast<unsigned>(n_spectra), static_cast<unsigned>((n_stream + feng::kStreamsPerBlock - 1) / feng::kStreamsPerBlock));
+    const long long n_sb = (n_stream + feng::kStreamsPerBlock - 1) / feng::kStreamsPerBlock;
+    const long long n_ab = (n_spectra + feng::kSpectraPerBlock - 1) / feng::kSpectraPerBlock;
+    if (n_sb * n_ab > 0x7fffffffLL) return fail(nullptr, CORR_EINVAL, "corr_fengine: problem too large for one launch");
+    const dim3 grid(static_cast<unsigned>(n_sb * n_ab));
     feng::fengine_kernel<<<grid, feng::kThreads, 0, static_cast<cudaStream_t>(stream)>>>(prm);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail_cuda(nullptr, e, "fengine_kernel launch");

@@ -23,6 +23,7 @@ constexpr int kChan = kFft / 2;          // channels kept
 constexpr int kThreads = 256;
 constexpr int kStreamsPerBlock = 32;
 constexpr int kPitch = kFft + 16;        // float2 per transform buffer: index n + n / 16 (bank spread)
+constexpr int kSpectraPerBlock = 8;      // consecutive spectra per block (amortises the twiddle table and the launch)
 
 struct Params {
     const int8_t* in;        // [n_stream][n_spectra * 256]
@@ -91,8 +92,10 @@ __global__ void __launch_bounds__(kThreads) fengine_kernel(const Params prm) {
     const int tid = threadIdx.x;
     const int g = tid >> 4;              // transform within the block (stream pair)
     const int c = tid & 15;              // thread within the transform
-    const long long a = blockIdx.x;      // spectrum index
-    const int m0 = blockIdx.y * kStreamsPerBlock;
+    // blocks that run together cover ALL streams of the same spectra, so the 128-byte output rows of one (a, k) meet in L2
+    const unsigned n_sb = (prm.n_stream + kStreamsPerBlock - 1) / kStreamsPerBlock;
+    const unsigned ab = blockIdx.x / n_sb;
+    const int m0 = static_cast<int>(blockIdx.x % n_sb) * kStreamsPerBlock;
     const int m = m0 + 2 * g;            // streams m (real part) and m + 1 (imaginary part)
 
     {
@@ -100,27 +103,24 @@ __global__ void __launch_bounds__(kThreads) fengine_kernel(const Params prm) {
         sincospif(-static_cast<float>(tid) / 128.0f, &sn, &cs);
         tw[tid] = make_float2(cs, sn);
     }
+    __syncthreads();
 
-    // ---- load 16 consecutive samples of both streams (16-byte loads), z[n] = s_m[n] + j s_{m+1}[n] ----
     const long long row = prm.n_spectra * kFft;
-    int4 ra = make_int4(0, 0, 0, 0), rb = make_int4(0, 0, 0, 0);
-    if (m < prm.n_stream) ra = *reinterpret_cast<const int4*>(prm.in + m * row + a * kFft + 16 * c);
-    if (m + 1 < prm.n_stream) rb = *reinterpret_cast<const int4*>(prm.in + (m + 1) * row + a * kFft + 16 * c);
-    const int wa[4] = {ra.x, ra.y, ra.z, ra.w}, wb[4] = {rb.x, rb.y, rb.z, rb.w};
     float2* z = buf[g];
-#pragma unroll
-    for (int i = 0; i < 16; ++i) {
-        const int n = 16 * c + i;
-        const float re = static_cast<float>(static_cast<int8_t>(wa[i >> 2] >> (8 * (i & 3))));
-        const float im = static_cast<float>(static_cast<int8_t>(wb[i >> 2] >> (8 * (i & 3))));
-        z[n + (n >> 4)] = make_float2(re, im);
-    }
-    __syncthreads();                                              // also publishes tw[]
-
-    // ---- pass A: n = 16 n1 + n2, this thread is n2 = c: DFT16 over n1, then twiddle W256^{n2 k1} ----
+    const long long a_end = (ab + 1ll) * kSpectraPerBlock < prm.n_spectra ? (ab + 1ll) * kSpectraPerBlock : prm.n_spectra;
+    for (long long a = static_cast<long long>(ab) * kSpectraPerBlock; a < a_end; ++a) {
+    // ---- pass A operands straight from global memory: n = 16 n1 + n2, this thread is n2 = c and takes the 16 samples
+    //      n1 = 0..15 (stride 16 bytes) of both streams; the 16 threads of a transform cover each 16-byte run together,
+    //      z[n] = s_m[n] + j s_{m+1}[n] ----
     float2 v[16];
+    {
+        const int8_t* pa = prm.in + m * row + a * kFft + c;
+        const int8_t* pb = pa + row;
+        const bool oka = m < prm.n_stream, okb = m + 1 < prm.n_stream;
 #pragma unroll
-    for (int n1 = 0; n1 < 16; ++n1) v[n1] = z[16 * n1 + c + n1];
+        for (int n1 = 0; n1 < 16; ++n1)
+            v[n1] = make_float2(oka ? static_cast<float>(pa[16 * n1]) : 0.0f, okb ? static_cast<float>(pb[16 * n1]) : 0.0f);
+    }
     dft16(v);
     __syncwarp();                                                 // the 16 threads of a transform share a warp
 #pragma unroll
@@ -168,6 +168,8 @@ __global__ void __launch_bounds__(kThreads) fengine_kernel(const Params prm) {
         for (int k = tid >> 5; k < kChan; k += kThreads / 32)
             prm.out[(a * kChan + k) * prm.n_stream + m0 + col] = ost[k][col];
     }
+    __syncthreads();                                              // staging (aliased onto buf) is free again
+    }   // spectra of this block
 }
 
 }  // namespace feng
