@@ -10,8 +10,9 @@
 // DFT256 = 16 x 16 (Cooley-Tukey): 16 threads per transform, each computes a 16-point DFT in registers
 // (radix 4 x 4) per pass, with one shared-memory exchange between the passes.  fp32 arithmetic, fp16 (RN) output.
 //
-// One block = 32 streams (16 transforms x 16 threads) of ONE spectrum index a: loads are 16 bytes per thread along
-// time, stores are 128-byte rows along the stream axis (32 streams x 4 bytes) for each channel.
+// One block = 32 streams (16 transforms x 16 threads) x 8 consecutive spectra: the 16 threads of a transform read each
+// 16-byte run of samples together (one byte each, already in pass-A order), stores are 128-byte rows along the stream
+// axis (32 streams x 4 bytes) for each channel.
 #pragma once
 #include <cuda_fp16.h>
 #include <cstdint>

@@ -76,11 +76,7 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst_smem, const CUtensorMap
 // input tiles other CTAs are about to re-read out of L2
 __device__ __forceinline__ uint64_t policy_evict_first() {
     uint64_t p;
-#ifdef CORR_AB_EVICT_NORMAL
-    asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
-#else
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
-#endif
     return p;
 }
 __device__ __forceinline__ void bulk_store(void* dst_gmem, uint32_t src_smem, uint32_t bytes, uint64_t policy) {
