@@ -116,6 +116,20 @@ int corr_xengine_cross(corr_handle h, const void* in_a, const void* in_b, void* 
 size_t corr_input_bytes_b(corr_handle h);    /* cross plans: T*C*Nb*P * (2 or 4); else 0 */
 
 /*
+ * corr_xengine_dumps -- short-integration mode (the paper's "transient detector ... between
+ * conjugate multiplications and accumulations" wants visibilities every few samples): the n_time samples
+ * of `in` are cut into n_dump consecutive integrations of n_time / n_dump samples, each integrated SEPARATELY (Eq. 2
+ * per integration, no sum across them) in ONE kernel launch.
+ *   in     DEVICE, as for corr_xengine ([n_time][n_chan][n_station][n_pol]; integration d = samples
+ *          [d * n_time/n_dump, (d+1) * n_time/n_dump)).
+ *   out    DEVICE, n_dump * corr_output_bytes(h) bytes: [n_dump][n_chan][B][n_pol][n_pol] complex int32 / fp32;
+ *          every word is overwritten (there is no accumulate).
+ *   n_dump must divide n_time.  HERK plans only (CORR_EINVAL on a cross plan).  Runs on the CTA-pair kernel for every
+ *   TMA-addressable geometry (rank-3 tensor map: a TMA box never crosses into the next integration), else SIMT.
+ */
+int corr_xengine_dumps(corr_handle h, const void* in, void* out, int n_dump, void* stream);
+
+/*
  * corr_fengine -- the F-engine in front of the X-engine.  PAPER.md:49-52 (Sec. 2, Eq. 1):
  *     S[k] = sum_{n=0}^{N-1} s[n] exp(-j (2 pi / N) k n),   N = 256 ("An FFT length of 256 is used across all tests",
  * PAPER.md:176), applied to consecutive non-overlapping blocks of each stream's 8-bit REAL samples.

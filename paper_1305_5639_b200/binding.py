@@ -27,6 +27,7 @@ SYMBOLS = {
     "corr_xengine_cross": (_i, [_vp, _vp, _vp, _vp, _i, _vp]),
     "corr_input_bytes_b": (_sz, [_vp]),
     "corr_fengine": (_i, [_vp, _vp, _i, _ll, _vp]),
+    "corr_xengine_dumps": (_i, [_vp, _vp, _vp, _i, _vp]),
     "corr_destroy": (None, [_vp]),
     "corr_input_bytes": (_sz, [_vp]),
     "corr_output_bytes": (_sz, [_vp]),
@@ -194,6 +195,19 @@ class Correlator:
         self._check_out(out, "cuda")
         self._check(self._L.corr_xengine(self._h, x.data_ptr(), out.data_ptr(), int(bool(accumulate)),
                                          _stream_ptr(stream)))
+        return out
+
+    def xengine_dumps(self, x, n_dump, out=None, stream=None):
+        """corr_xengine_dumps: n_dump separate integrations of n_time / n_dump samples in one launch ->
+        [n_dump, C, B, P, P, 2]."""
+        import torch
+        self._check_in(x, "cuda")
+        shape = (int(n_dump),) + tuple(self.output_shape())
+        if out is None:
+            out = torch.empty(shape, device=x.device, dtype=torch.int32 if self.dtype == "ci8" else torch.float32)
+        if tuple(out.shape) != shape or not out.is_contiguous() or out.device.type != "cuda":
+            raise ValueError("out must be a contiguous CUDA tensor of shape %s" % (shape,))
+        self._check(self._L.corr_xengine_dumps(self._h, x.data_ptr(), out.data_ptr(), int(n_dump), _stream_ptr(stream)))
         return out
 
     def xengine_host(self, x_host, out_host, accumulate=False):

@@ -59,6 +59,7 @@ struct corr_plan {
     CUtensorMap tmap_in;     // 1-CTA kernel: box [128 B][Cfg::kKStage samples]
     CUtensorMap tmap_pair;   // pair kernels: box [128 B][kPairStageK / kPairBoxes samples]
     const void* tmap_in_ptr;
+    int tmap_dumps;          // n_dump the pair tensor map was encoded for
     CUtensorMap tmap_b;      // cross plans: group B, pair-kernel box
     const void* tmap_b_ptr;
 
@@ -195,23 +196,42 @@ int encode_map(corr_plan* h, CUtensorMap* map, const void* ptr, int M, int box_r
     return CORR_OK;
 }
 
+// Pair kernels: `ptr` viewed as [n_dump][T / n_dump][C*2M] (rank 3), box [128 B][stage samples][1]: a box never crosses
+// from one integration into the next, rows past an integration's end are zero-filled.
+int encode_map3(corr_plan* h, CUtensorMap* map, const void* ptr, int M, int box_rows, int n_dump) {
+    const int elt = h->sample_bytes / 2;
+    const cuuint64_t W = static_cast<cuuint64_t>(h->C) * 2 * M;
+    const cuuint64_t Ts = static_cast<cuuint64_t>(h->T / n_dump);
+    cuuint64_t dims[3] = {W, Ts, static_cast<cuuint64_t>(n_dump)};
+    cuuint64_t strides[2] = {W * elt, Ts * W * elt};
+    cuuint32_t box[3] = {static_cast<cuuint32_t>(128 / elt), static_cast<cuuint32_t>(box_rows), 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    const CUresult r = h->encode(map, elt == 1 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3,
+                                 const_cast<void*>(ptr), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                 CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(h, CORR_ECUDA, "cuTensorMapEncodeTiled (rank 3) failed with CUresult %d", static_cast<int>(r));
+    return CORR_OK;
+}
+
 // Tensor maps of `in` viewed as [T][C*2M]: box [128 B][stage samples] for the 1-CTA kernel and for the pair kernels.
-int encode_input_map(corr_plan* h, const void* in) {
-    if (h->tmap_in_ptr == in) return CORR_OK;
+int encode_input_map(corr_plan* h, const void* in, int n_dump = 1) {
+    if (h->tmap_in_ptr == in && h->tmap_dumps == n_dump) return CORR_OK;
     h->tmap_in_ptr = nullptr;
     const int elt = h->sample_bytes / 2;
     int rc = encode_map(h, &h->tmap_in, in, h->M, elt == 1 ? xtc::Cfg<1>::kKStage : xtc::Cfg<2>::kKStage);
     if (rc == CORR_OK)
-        rc = encode_map(h, &h->tmap_pair, in, h->M, (elt == 1 ? xtc::kPairStageK<1> : xtc::kPairStageK<2>) / xtc::kPairBoxes);
-    if (rc == CORR_OK) h->tmap_in_ptr = in;
+        rc = encode_map3(h, &h->tmap_pair, in, h->M, (elt == 1 ? xtc::kPairStageK<1> : xtc::kPairStageK<2>) / xtc::kPairBoxes, n_dump);
+    if (rc == CORR_OK) { h->tmap_in_ptr = in; h->tmap_dumps = n_dump; }
     return rc;
 }
 
 int encode_input_map_b(corr_plan* h, const void* in_b) {
     if (h->tmap_b_ptr == in_b) return CORR_OK;
     h->tmap_b_ptr = nullptr;
+    h->tmap_dumps = 1;
     const int elt = h->sample_bytes / 2;
-    const int rc = encode_map(h, &h->tmap_b, in_b, h->Mb, (elt == 1 ? xtc::kPairStageK<1> : xtc::kPairStageK<2>) / xtc::kPairBoxes);
+    const int rc = encode_map3(h, &h->tmap_b, in_b, h->Mb, (elt == 1 ? xtc::kPairStageK<1> : xtc::kPairStageK<2>) / xtc::kPairBoxes, 1);
     if (rc == CORR_OK) h->tmap_b_ptr = in_b;
     return rc;
 }
@@ -231,6 +251,7 @@ int launch_direct(corr_plan* h, const void* in, void* out, int accumulate, cudaS
     prm.n_baseline = h->B;
     prm.n_station_b = 0;
     prm.M_b = 0;
+    prm.n_dump = 1;
     prm.out = out;
     prm.accumulate = accumulate ? 1 : 0;
     // samples per TMEM accumulation pass: everything for int32 (exact); 1024 for fp32 (see xengine_tc.cuh)
@@ -280,8 +301,8 @@ cudaError_t launch_pair_kernel(const CUtensorMap& tmap, const CUtensorMap& tmap_
 }
 
 int launch_pair(corr_plan* h, const void* in, const void* in_b, void* out, int accumulate, cudaStream_t st,
-                int pairs_per_cluster) {
-    int rc = encode_input_map(h, in);
+                int pairs_per_cluster, int n_dump = 1) {
+    int rc = encode_input_map(h, in, n_dump);
     if (rc == CORR_OK && h->Nb) rc = encode_input_map_b(h, in_b);
     if (rc != CORR_OK) return rc;
     const CUtensorMap& map_b = h->Nb ? h->tmap_b : h->tmap_pair;
@@ -293,7 +314,8 @@ int launch_pair(corr_plan* h, const void* in, const void* in_b, void* out, int a
     pp.base.n_station = h->N;
     pp.base.n_pol = h->P;
     pp.base.n_chan = h->C;
-    pp.base.n_time = h->T;
+    pp.base.n_time = h->T / n_dump;
+    pp.base.n_dump = n_dump;
     pp.base.M = h->M;
     pp.base.n_baseline = h->B;
     pp.base.n_station_b = h->Nb;
@@ -309,7 +331,7 @@ int launch_pair(corr_plan* h, const void* in, const void* in_b, void* out, int a
 #endif
     pp.groups = h->d_groups[v];
     pp.groups_per_chan = static_cast<int>(h->h_groups[v].size());
-    pp.n_groups = static_cast<long long>(pp.groups_per_chan) * h->C;
+    pp.n_groups = static_cast<long long>(pp.groups_per_chan) * h->C * n_dump;
     const unsigned clusters = static_cast<unsigned>(pp.n_groups < h->max_clusters[v] ? pp.n_groups : h->max_clusters[v]);
     if (pp.n_groups > (1ll << 31) - 4096) return fail(h, CORR_EINVAL, "xengine_pair_kernel: %lld tiles exceed the tile feed's range", pp.n_groups);
     pp.sched_counter = h->d_sched + (h->sched_seq++ % kSchedRing);
@@ -654,6 +676,34 @@ int corr_xengine(corr_handle h, const void* in, void* out, int accumulate, void*
     if (!h) return CORR_EINVAL;
     if (h->Nb) return fail(h, CORR_EINVAL, "corr_xengine: this is a cross plan (corr_create_cross); call corr_xengine_cross");
     return run_xengine(h, in, nullptr, out, accumulate, stream);
+}
+
+int corr_xengine_dumps(corr_handle h, const void* in, void* out, int n_dump, void* stream) {
+    if (!h) return CORR_EINVAL;
+    if (h->Nb) return fail(h, CORR_EINVAL, "corr_xengine_dumps: not available on cross plans");
+    if (!in || !out) return fail(h, CORR_EINVAL, "corr_xengine_dumps: NULL pointer");
+    if ((reinterpret_cast<uintptr_t>(in) & 15) || (reinterpret_cast<uintptr_t>(out) & 15))
+        return fail(h, CORR_EINVAL, "corr_xengine_dumps: `in` and `out` must be 16-byte aligned");
+    if (n_dump < 1 || h->T % n_dump)
+        return fail(h, CORR_EINVAL, "corr_xengine_dumps: n_dump = %d must divide n_time = %d", n_dump, h->T);
+    const int Ts = h->T / n_dump;
+    if (h->dtype == CORR_CI8 && Ts > kMaxIntegrationCi8)
+        return fail(h, CORR_EOVERFLOW, "corr_xengine_dumps: integrating %d samples would overflow int32", Ts);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    h->last_launches = 0;
+    h->t_total = Ts;
+    const int kernel = resolve_kernel(h);
+    if (kernel != CORR_KERNEL_SIMT && h->max_clusters[0] > 0)
+        return launch_pair(h, in, nullptr, out, 0, st, 1, n_dump);       // any TMA-addressable geometry runs on the pair kernel
+    // SIMT: one launch per integration on slices of `in` and `out`
+    const int T_full = h->T;
+    int rc = CORR_OK;
+    h->T = Ts;
+    for (int d = 0; d < n_dump && rc == CORR_OK; ++d)
+        rc = launch_simt(h, static_cast<const uint8_t*>(in) + d * input_bytes(h), nullptr,
+                         static_cast<uint8_t*>(out) + d * output_bytes(h), 0, st);
+    h->T = T_full;
+    return rc;
 }
 
 int corr_xengine_cross(corr_handle h, const void* in_a, const void* in_b, void* out, int accumulate, void* stream) {

@@ -199,10 +199,11 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const __grid_co
             [[maybe_unused]] const long long st_begin = clock64();
             TileFeed feed(feed_full0, feed_free0, feed_slot0);
             for (long long g = cluster_id; g < pp.n_groups; g = feed.next()) {
-                const int c = static_cast<int>(g / pp.groups_per_chan);
-                const PairGroup gd = pp.groups[g - static_cast<long long>(c) * pp.groups_per_chan];
+                const int cd = static_cast<int>(g / pp.groups_per_chan);            // integration * C + channel
+                const PairGroup gd = pp.groups[g - static_cast<long long>(cd) * pp.groups_per_chan];
                 const PairTile td = (kPairs == 2 && pair == 1) ? gd.t[1] : gd.t[0];
-                const int w_a = c * M2 + td.row0 + 128 * half;      // this CTA's A rows in the [T][C*2M] view
+                const int dump = cd / prm.n_chan, c = cd - dump * prm.n_chan;
+                const int w_a = c * M2 + td.row0 + 128 * half;      // this CTA's A rows in the [n_dump][T][C*2M] view
                 const int w_b = c * M2b + td.col0 + 128 * half;     // this CTA's half of the B columns
                 // a shared operand is fetched once, by pair 0's CTA, and multicast to the same-half CTA of pair 1
                 const bool mc_a = kPairs == 2 && (gd.share & 1);
@@ -224,11 +225,11 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const __grid_co
 #pragma unroll
                         for (int b = 0; b < kPairBoxes; ++b) {
                             if (!mc_a)
-                                ptx::tma_load_2d_pair(sa + ch * kChunkBytes + b * kBoxBytes, &tmap_in, full_bar(stage),
-                                                      w_a + ch * kChunkElems, kb * kStageK + b * kBoxRows);
+                                ptx::tma_load_3d_pair(sa + ch * kChunkBytes + b * kBoxBytes, &tmap_in, full_bar(stage),
+                                                      w_a + ch * kChunkElems, kb * kStageK + b * kBoxRows, dump);
                             else if (pair == 0)
-                                ptx::tma_load_2d_pair_mc(sa + ch * kChunkBytes + b * kBoxBytes, &tmap_in, full_bar(stage),
-                                                         w_a + ch * kChunkElems, kb * kStageK + b * kBoxRows, mc_mask);
+                                ptx::tma_load_3d_pair_mc(sa + ch * kChunkBytes + b * kBoxBytes, &tmap_in, full_bar(stage),
+                                                         w_a + ch * kChunkElems, kb * kStageK + b * kBoxRows, dump, mc_mask);
                         }
                     if (diag) {
                         if (++stage == kPairStages) { stage = 0; phase ^= 1u; }
@@ -239,11 +240,11 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const __grid_co
 #pragma unroll
                         for (int b = 0; b < kPairBoxes; ++b) {
                             if (!mc_b)
-                                ptx::tma_load_2d_pair(sb + ch * kChunkBytes + b * kBoxBytes, &tmap_b, full_bar(stage),
-                                                      w_b + ch * kChunkElems, kb * kStageK + b * kBoxRows);
+                                ptx::tma_load_3d_pair(sb + ch * kChunkBytes + b * kBoxBytes, &tmap_b, full_bar(stage),
+                                                      w_b + ch * kChunkElems, kb * kStageK + b * kBoxRows, dump);
                             else if (pair == 0)
-                                ptx::tma_load_2d_pair_mc(sb + ch * kChunkBytes + b * kBoxBytes, &tmap_b, full_bar(stage),
-                                                         w_b + ch * kChunkElems, kb * kStageK + b * kBoxRows, mc_mask);
+                                ptx::tma_load_3d_pair_mc(sb + ch * kChunkBytes + b * kBoxBytes, &tmap_b, full_bar(stage),
+                                                         w_b + ch * kChunkElems, kb * kStageK + b * kBoxRows, dump, mc_mask);
                         }
                     if (++stage == kPairStages) { stage = 0; phase ^= 1u; }
                 }

@@ -68,6 +68,9 @@ struct Params {
     // rectangular cross-only mode: rows are the n_station streams of group A (conjugated), columns the
     // n_station_b stations (M_b = n_station_b * n_pol streams) of group B; 0 = triangular HERK of one group
     int n_station_b, M_b;
+    // pair kernels: number of separate integrations of n_time samples in one call (corr_xengine_dumps); the input is
+    // [n_dump][n_time][C][...], the output [n_dump][C][...]: integration d, channel c is handled as "channel" d*C + c
+    int n_dump;
     // 1-CTA kernel: a stage holds [b_chunks 128-byte-wide B chunks][A chunks, only if some tile is off the diagonal]
     int n_stages, stage_bytes, b_chunks;
 #ifdef CORR_STATS

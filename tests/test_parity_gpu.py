@@ -402,3 +402,43 @@ def test_cross_argument_errors(corr):
         with pytest.raises(corr.CorrError):
             h.set_kernel("single")
     assert not corr.lib().corr_create_cross(4, 0, 2, 1, 1, 0)
+
+
+# ---------------------------------------------------------------------------------------------
+# short-integration mode (corr_xengine_dumps): every dump is Eq. 2 on its own slice of samples
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("N,P,C,T,n_dump", [(16, 2, 5, 300, 3), (64, 2, 4, 512, 4), (72, 2, 3, 260, 2), (136, 1, 2, 384, 3),
+                                            (256, 2, 2, 256, 8), (33, 2, 2, 90, 3), (80, 2, 3, 64, 64)])
+def test_dumps_ci8_bit_exact(corr, oracle, N, P, C, T, n_dump):
+    x = inputs.gauss_ci8(T, C, N, P, 40.0, seed=7700 + N + n_dump)
+    with corr.Correlator(N, P, C, T, "ci8") as h:
+        got = h.xengine_dumps(x.cuda(), n_dump).cpu().numpy()
+        whole = h.xengine(x.cuda()).cpu().numpy()                 # the same handle still integrates the whole block
+    Ts = T // n_dump
+    assert got.shape[0] == n_dump
+    for d in range(n_dump):
+        assert_bit_exact(got[d], oracle.xengine(x[d * Ts:(d + 1) * Ts].numpy()))
+    assert (got.astype(np.int64).sum(axis=0) == whole).all()      # additivity in time (pin 8) through the GPU path
+    assert_bit_exact(whole, oracle.xengine(x.numpy()))
+
+
+def test_dumps_cf16_within_tolerance(corr, oracle):
+    N, P, C, T, n_dump = 48, 2, 3, 2400, 2                       # 1200 samples per dump: two TMEM passes each
+    x = inputs.corr_phase_cf16(T, C, N, P, seed=7800)
+    with corr.Correlator(N, P, C, T, "cf16") as h:
+        got = h.xengine_dumps(x.cuda(), n_dump).cpu().numpy()
+    for d in range(n_dump):
+        want = oracle.xengine(x[d * 1200:(d + 1) * 1200].numpy())
+        assert fp16_normalised_error(got[d], want, N, P) <= FP16_TOL
+
+
+def test_dumps_argument_errors(corr):
+    with corr.Correlator(16, 2, 2, 96, "ci8") as h, corr.CrossCorrelator(8, 8, 2, 2, 64, "ci8") as g:
+        L = corr.lib()
+        x = torch.zeros(h.input_shape(), dtype=torch.int8, device="cuda")
+        out = torch.empty((4,) + tuple(h.output_shape()), dtype=torch.int32, device="cuda")
+        assert L.corr_xengine_dumps(h._h, x.data_ptr(), out.data_ptr(), 5, None) == corr.CORR_EINVAL     # 5 does not divide 96
+        assert L.corr_xengine_dumps(h._h, x.data_ptr(), out.data_ptr(), 0, None) == corr.CORR_EINVAL
+        assert L.corr_xengine_dumps(h._h, None, out.data_ptr(), 4, None) == corr.CORR_EINVAL
+        assert L.corr_xengine_dumps(g._h, x.data_ptr(), out.data_ptr(), 4, None) == corr.CORR_EINVAL     # cross plan
+        assert L.corr_xengine_dumps(None, x.data_ptr(), out.data_ptr(), 4, None) == corr.CORR_EINVAL
