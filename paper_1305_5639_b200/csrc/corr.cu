@@ -65,7 +65,6 @@ struct corr_plan {
 
     // corner-turn feed
     int Tp;                // padded time extent of the workspace
-    void* d_ws;            // owned workspace (lazy)
 
     // corr_xengine_host staging
     void* d_in_stage;
@@ -507,7 +506,6 @@ static corr_handle create_plan(int n_station, int n_station_b, int n_pol, int n_
     h->encode = nullptr;
     h->tmap_in_ptr = nullptr;
     h->Tp = (n_time + 63) / 64 * 64;
-    h->d_ws = nullptr;
     h->d_in_stage = nullptr;
     h->d_out_stage = nullptr;
     h->own_stream = nullptr;
@@ -605,7 +603,6 @@ void corr_destroy(corr_handle h) {
     if (h->d_sched) cudaFree(h->d_sched);
     if (h->d_groups[0]) cudaFree(h->d_groups[0]);
     if (h->d_groups[1]) cudaFree(h->d_groups[1]);
-    if (h->d_ws) cudaFree(h->d_ws);
     if (h->d_in_stage) cudaFree(h->d_in_stage);
     if (h->d_out_stage) cudaFree(h->d_out_stage);
     if (h->own_stream) cudaStreamDestroy(h->own_stream);
