@@ -8,7 +8,8 @@
 // Two real streams per complex transform: z[n] = s_m[n] + j s_{m+1}[n] (the two polarisations of one station when
 // n_pol = 2), Z = DFT256(z), then S_m[k] = (Z[k] + conj(Z[N-k])) / 2 and S_{m+1}[k] = (Z[k] - conj(Z[N-k])) / (2j).
 // DFT256 = 16 x 16 (Cooley-Tukey): 16 threads per transform, each computes a 16-point DFT in registers
-// (radix 4 x 4) per pass, with one shared-memory exchange between the passes.  fp32 arithmetic, fp16 (RN) output.
+// (radix 4 x 4) per pass, with one shared-memory exchange between the passes; the pass-A twiddles live in registers and
+// the two-stream split pairs Z[k] with Z[N-k] by shuffles.  fp32 arithmetic, fp16 (RN) output.
 //
 // One block = 32 streams (16 transforms x 16 threads) x 8 consecutive spectra: the 16 threads of a transform read each
 // 16-byte run of samples together (one byte each, already in pass-A order), stores are 128-byte rows along the stream
@@ -85,7 +86,6 @@ __device__ __forceinline__ void dft16(float2 (&v)[16]) {
 
 __global__ void __launch_bounds__(kThreads) fengine_kernel(const Params prm) {
     __shared__ float2 buf[kThreads / 16][kPitch];                 // one 256-point complex buffer per transform
-    __shared__ float2 tw[kFft];                                    // W256^m = exp(-j 2 pi m / 256)
     // output staging [k][stream in block], aliased onto buf once every transform has been read back into registers
     __half2 (*ost)[kStreamsPerBlock + 1] = reinterpret_cast<__half2 (*)[kStreamsPerBlock + 1]>(&buf[0][0]);
     static_assert(sizeof(__half2) * kChan * (kStreamsPerBlock + 1) <= sizeof(float2) * (kThreads / 16) * kPitch, "staging fits");
@@ -99,12 +99,14 @@ __global__ void __launch_bounds__(kThreads) fengine_kernel(const Params prm) {
     const int m0 = static_cast<int>(blockIdx.x % n_sb) * kStreamsPerBlock;
     const int m = m0 + 2 * g;            // streams m (real part) and m + 1 (imaginary part)
 
-    {
+    // pass-A twiddles W256^{n2 k1} = exp(-j 2 pi c k1 / 256) of this thread (n2 = c), kept in registers for all spectra
+    float2 twr[16];
+#pragma unroll
+    for (int k1 = 0; k1 < 16; ++k1) {
         float sn, cs;
-        sincospif(-static_cast<float>(tid) / 128.0f, &sn, &cs);
-        tw[tid] = make_float2(cs, sn);
+        sincospif(-static_cast<float>(c * k1) / 128.0f, &sn, &cs);
+        twr[k1] = make_float2(cs, sn);
     }
-    __syncthreads();
 
     const long long row = prm.n_spectra * kFft;
     float2* z = buf[g];
@@ -126,7 +128,7 @@ __global__ void __launch_bounds__(kThreads) fengine_kernel(const Params prm) {
     __syncwarp();                                                 // the 16 threads of a transform share a warp
 #pragma unroll
     for (int k1 = 0; k1 < 16; ++k1) {
-        const float2 y = cmul(v[k1], tw[c * k1]);
+        const float2 y = cmul(v[k1], twr[k1]);
         z[16 * k1 + c + k1] = y;                                  // [k1][n2]
     }
     __syncwarp();
@@ -134,22 +136,17 @@ __global__ void __launch_bounds__(kThreads) fengine_kernel(const Params prm) {
     // ---- pass B: this thread is k1 = c: DFT16 over n2  ->  Z[k1 + 16 k2] ----
 #pragma unroll
     for (int n2 = 0; n2 < 16; ++n2) v[n2] = z[16 * c + n2 + c];
-    dft16(v);
-    __syncwarp();
-#pragma unroll
-    for (int k2 = 0; k2 < 16; ++k2) {
-        const int k = c + 16 * k2;
-        z[k + (k >> 4)] = v[k2];
-    }
-    __syncwarp();
+    dft16(v);                                                     // v[k2] = Z[c + 16 k2]
 
-    // ---- split the two real streams, round to fp16, stage as [k][stream] ----
+    // ---- split the two real streams: Z[N - k] for k = c + 16 i sits in thread (16 - c) mod 16 as v[15 - i]
+    //      (thread 0: its own v[(16 - i) mod 16]); one shuffle pair inside the 16-lane group, no shared memory ----
     __half2 h0[kChan / 16], h1[kChan / 16];
+    const int partner = (16 - c) & 15;
 #pragma unroll
     for (int i = 0; i < kChan / 16; ++i) {
-        const int k = c + 16 * i;                                 // 0 .. 127
-        const int kr = (kFft - k) & (kFft - 1);
-        const float2 p = z[k + (k >> 4)], q = z[kr + (kr >> 4)];  // Z[k], Z[N - k]
+        const float2 p = v[i];                                    // Z[k], k = c + 16 i in 0 .. 127
+        float2 q = make_float2(__shfl_sync(0xffffffffu, v[15 - i].x, partner, 16), __shfl_sync(0xffffffffu, v[15 - i].y, partner, 16));
+        if (c == 0) q = v[(16 - i) & 15];
         // S_m = (Z[k] + conj(Z[N-k])) / 2 ;  S_{m+1} = (Z[k] - conj(Z[N-k])) / (2j)
         h0[i] = __floats2half2_rn(0.5f * (p.x + q.x), 0.5f * (p.y - q.y));
         h1[i] = __floats2half2_rn(0.5f * (p.y + q.y), 0.5f * (q.x - p.x));
