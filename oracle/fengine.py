@@ -50,3 +50,13 @@ def to_xengine_input(S):
     out[..., 0] = S.real.astype(np.float16)
     out[..., 1] = S.imag.astype(np.float16)
     return out
+
+
+def quantise_ci8(S, scale):
+    """Requantised int8 codes of the spectra: clip(rint(S * scale), -127, 127) per component, rint = round half to even,
+    in the X-engine's [T, C, M, 2] layout.  Also returns the distance of every scaled component from the nearest
+    rounding tie (k + 0.5), so that a comparison can tell a genuine mismatch from a tie decided in lower precision."""
+    y = np.stack([S.real, S.imag], axis=-1) * float(scale)
+    codes = np.clip(np.rint(y), -127, 127).astype(np.int8)
+    tie_dist = np.abs(np.abs(y - np.floor(y)) - 0.5)
+    return codes, tie_dist

@@ -87,3 +87,15 @@ def test_rejects_bad_input():
         fo.fengine(np.zeros((2, 100), np.int8))
     with pytest.raises(ValueError):
         fo.fengine(np.zeros((2, L), np.int16))
+
+
+def test_quantise_ci8_rounding_clipping_and_tie_distance():
+    """clip(rint(S * scale), +-127): ties go to even (numpy rint and the kernel's cvt.rni agree on that), -128 is never
+    produced, and the reported tie distance is 0 exactly at k + 0.5."""
+    S = np.array([[[0.5 + 1.5j, 2.5 - 0.5j, 2.49 + 2.51j, 1000 - 1000j, -127.4 + 127.6j, 3.0 - 3.0j]]])   # [1, 1, 6]
+    codes, tie = fo.quantise_ci8(S, 1.0)
+    assert codes.dtype == np.int8 and codes.shape == (1, 1, 6, 2)
+    assert codes[0, 0].tolist() == [[0, 2], [2, 0], [2, 3], [127, -127], [-127, 127], [3, -3]]
+    assert tie[0, 0, 0, 0] == 0 and tie[0, 0, 1, 0] == 0 and abs(tie[0, 0, 5, 0] - 0.5) < 1e-12
+    codes2, _ = fo.quantise_ci8(S, 0.5)
+    assert codes2[0, 0, 3].tolist() == [127, -127] and codes2[0, 0, 5].tolist() == [2, -2]        # 1.5 -> 2, -1.5 -> -2
