@@ -143,6 +143,15 @@ int corr_xengine_dumps(corr_handle h, const void* in, void* out, int n_dump, voi
  */
 int corr_fengine(const void* in, void* out, int n_stream, long long n_spectra, void* stream);
 
+/*
+ * corr_fengine_ci8 -- the same transform with REQUANTISED complex int8 output, the input format of the int8 X-engine
+ * (CORR_CI8): out[n_spectra][128][n_stream] (re, im) int8 pairs, code = clip(rint(S * scale), -127, 127) per component
+ * (rint = round to nearest, ties to even, applied to the fp32 product; -128 is never produced).  `scale` > 0 is the
+ * caller's requantisation gain (e.g. 1 / (sigma_in * 16) * target sigma); `out` needs 2-byte alignment.  Everything
+ * else as corr_fengine.
+ */
+int corr_fengine_ci8(const void* in, void* out, int n_stream, long long n_spectra, float scale, void* stream);
+
 /* corr_destroy -- frees the handle and everything it owns.  NULL is a no-op. */
 void corr_destroy(corr_handle h);
 

@@ -27,6 +27,7 @@ SYMBOLS = {
     "corr_xengine_cross": (_i, [_vp, _vp, _vp, _vp, _i, _vp]),
     "corr_input_bytes_b": (_sz, [_vp]),
     "corr_fengine": (_i, [_vp, _vp, _i, _ll, _vp]),
+    "corr_fengine_ci8": (_i, [_vp, _vp, _i, _ll, ctypes.c_float, _vp]),
     "corr_xengine_dumps": (_i, [_vp, _vp, _vp, _i, _vp]),
     "corr_destroy": (None, [_vp]),
     "corr_input_bytes": (_sz, [_vp]),
@@ -89,9 +90,12 @@ def _stream_ptr(stream):
     return ctypes.c_void_p(getattr(stream, "cuda_stream", stream))
 
 
-def fengine(samples, out=None, stream=None):
-    """corr_fengine: int8 real samples [n_stream, n_spectra * 256] (CUDA) -> complex fp16 [n_spectra, 128, n_stream, 2]."""
+def fengine(samples, out=None, stream=None, scale=None):
+    """corr_fengine: int8 real samples [n_stream, n_spectra * 256] (CUDA) -> complex fp16 [n_spectra, 128, n_stream, 2];
+    with ``scale`` (corr_fengine_ci8): requantised complex int8 codes clip(rint(S * scale), +-127) of the same shape."""
     import torch
+    if scale is not None:
+        return _fengine_ci8(samples, float(scale), out, stream)
     if samples.dtype != torch.int8 or samples.dim() != 2 or samples.shape[1] % 256 or not samples.is_contiguous() \
             or samples.device.type != "cuda":
         raise ValueError("samples must be a contiguous CUDA int8 tensor [n_stream, n_spectra * 256]")
@@ -102,6 +106,23 @@ def fengine(samples, out=None, stream=None):
         raise ValueError("out must be a contiguous float16 tensor [n_spectra, 128, n_stream, 2]")
     L = lib()
     rc = L.corr_fengine(samples.data_ptr(), out.data_ptr(), n_stream, n_spec, _stream_ptr(stream))
+    if rc != CORR_OK:
+        raise CorrError(rc, L.corr_last_error(None).decode())
+    return out
+
+
+def _fengine_ci8(samples, scale, out, stream):
+    import torch
+    if samples.dtype != torch.int8 or samples.dim() != 2 or samples.shape[1] % 256 or not samples.is_contiguous() \
+            or samples.device.type != "cuda":
+        raise ValueError("samples must be a contiguous CUDA int8 tensor [n_stream, n_spectra * 256]")
+    n_stream, n_spec = samples.shape[0], samples.shape[1] // 256
+    if out is None:
+        out = torch.empty((n_spec, 128, n_stream, 2), dtype=torch.int8, device=samples.device)
+    if out.dtype != torch.int8 or tuple(out.shape) != (n_spec, 128, n_stream, 2) or not out.is_contiguous():
+        raise ValueError("out must be a contiguous int8 tensor [n_spectra, 128, n_stream, 2]")
+    L = lib()
+    rc = L.corr_fengine_ci8(samples.data_ptr(), out.data_ptr(), n_stream, n_spec, scale, _stream_ptr(stream))
     if rc != CORR_OK:
         raise CorrError(rc, L.corr_last_error(None).decode())
     return out

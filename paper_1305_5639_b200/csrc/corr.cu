@@ -633,25 +633,35 @@ int corr_set_kernel(corr_handle h, int kernel) {
 }
 int corr_last_launch_count(corr_handle h) { return h ? h->last_launches : CORR_EINVAL; }
 
-int corr_fengine(const void* in, void* out, int n_stream, long long n_spectra, void* stream) {
+static int run_fengine(const void* in, void* out, int n_stream, long long n_spectra, bool int8_out, float scale, void* stream) {
     g_create_error[0] = 0;
-    if (!in || !out || n_stream < 1 || n_spectra < 1 || n_spectra > 0x7fffffffLL)
+    if (!in || !out || n_stream < 1 || n_spectra < 1 || n_spectra > 0x7fffffffLL || (int8_out && !(scale > 0.0f)))
         return fail(nullptr, CORR_EINVAL, "corr_fengine: invalid arguments (n_stream=%d, n_spectra=%lld)", n_stream, n_spectra);
-    if ((reinterpret_cast<uintptr_t>(in) & 15) || (reinterpret_cast<uintptr_t>(out) & 3))
-        return fail(nullptr, CORR_EINVAL, "corr_fengine: `in` must be 16-byte and `out` 4-byte aligned");
+    if ((reinterpret_cast<uintptr_t>(in) & 15) || (reinterpret_cast<uintptr_t>(out) & (int8_out ? 1 : 3)))
+        return fail(nullptr, CORR_EINVAL, "corr_fengine: `in` must be 16-byte and `out` element aligned");
     feng::Params prm;
     prm.in = static_cast<const int8_t*>(in);
-    prm.out = static_cast<__half2*>(out);
+    prm.out = out;
     prm.n_stream = n_stream;
     prm.n_spectra = n_spectra;
+    prm.scale = scale;
     const long long n_sb = (n_stream + feng::kStreamsPerBlock - 1) / feng::kStreamsPerBlock;
     const long long n_ab = (n_spectra + feng::kSpectraPerBlock - 1) / feng::kSpectraPerBlock;
     if (n_sb * n_ab > 0x7fffffffLL) return fail(nullptr, CORR_EINVAL, "corr_fengine: problem too large for one launch");
     const dim3 grid(static_cast<unsigned>(n_sb * n_ab));
-    feng::fengine_kernel<<<grid, feng::kThreads, 0, static_cast<cudaStream_t>(stream)>>>(prm);
+    if (int8_out) feng::fengine_kernel<true><<<grid, feng::kThreads, 0, static_cast<cudaStream_t>(stream)>>>(prm);
+    else feng::fengine_kernel<false><<<grid, feng::kThreads, 0, static_cast<cudaStream_t>(stream)>>>(prm);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail_cuda(nullptr, e, "fengine_kernel launch");
     return CORR_OK;
+}
+
+int corr_fengine(const void* in, void* out, int n_stream, long long n_spectra, void* stream) {
+    return run_fengine(in, out, n_stream, n_spectra, false, 1.0f, stream);
+}
+
+int corr_fengine_ci8(const void* in, void* out, int n_stream, long long n_spectra, float scale, void* stream) {
+    return run_fengine(in, out, n_stream, n_spectra, true, scale, stream);
 }
 
 int corr_corner_turn(corr_handle h, const void* in, void* ws, void* stream) {

@@ -29,9 +29,25 @@ constexpr int kSpectraPerBlock = 8;      // consecutive spectra per block (amort
 
 struct Params {
     const int8_t* in;        // [n_stream][n_spectra * 256]
-    __half2* out;            // [n_spectra][128][n_stream] (re, im)
+    void* out;               // [n_spectra][128][n_stream] (re, im): __half2 (cf16) or char2 (ci8)
     int n_stream;
     long long n_spectra;
+    float scale;             // ci8 output only: code = clip(rint(S * scale), -127, 127)
+};
+
+// output element: complex fp16 (one rounding to nearest) or requantised complex int8
+template <bool kInt8> struct Out;
+template <> struct Out<false> {
+    using T = __half2;
+    static __device__ __forceinline__ T cvt(float re, float im, float) { return __floats2half2_rn(re, im); }
+};
+template <> struct Out<true> {
+    using T = char2;
+    static __device__ __forceinline__ T cvt(float re, float im, float scale) {
+        const int a = max(-127, min(127, __float2int_rn(re * scale)));      // rint, ties to even; -128 is never produced
+        const int b = max(-127, min(127, __float2int_rn(im * scale)));
+        return make_char2(static_cast<signed char>(a), static_cast<signed char>(b));
+    }
 };
 
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
@@ -84,11 +100,13 @@ __device__ __forceinline__ void dft16(float2 (&v)[16]) {
         }
 }
 
+template <bool kInt8>
 __global__ void __launch_bounds__(kThreads) fengine_kernel(const Params prm) {
+    using OutT = typename Out<kInt8>::T;
     __shared__ float2 buf[kThreads / 16][kPitch];                 // one 256-point complex buffer per transform
     // output staging [k][stream in block], aliased onto buf once every transform has been read back into registers
-    __half2 (*ost)[kStreamsPerBlock + 1] = reinterpret_cast<__half2 (*)[kStreamsPerBlock + 1]>(&buf[0][0]);
-    static_assert(sizeof(__half2) * kChan * (kStreamsPerBlock + 1) <= sizeof(float2) * (kThreads / 16) * kPitch, "staging fits");
+    OutT (*ost)[kStreamsPerBlock + 1] = reinterpret_cast<OutT (*)[kStreamsPerBlock + 1]>(&buf[0][0]);
+    static_assert(sizeof(OutT) * kChan * (kStreamsPerBlock + 1) <= sizeof(float2) * (kThreads / 16) * kPitch, "staging fits");
 
     const int tid = threadIdx.x;
     const int g = tid >> 4;              // transform within the block (stream pair)
@@ -140,7 +158,7 @@ __global__ void __launch_bounds__(kThreads) fengine_kernel(const Params prm) {
 
     // ---- split the two real streams: Z[N - k] for k = c + 16 i sits in thread (16 - c) mod 16 as v[15 - i]
     //      (thread 0: its own v[(16 - i) mod 16]); one shuffle pair inside the 16-lane group, no shared memory ----
-    __half2 h0[kChan / 16], h1[kChan / 16];
+    OutT h0[kChan / 16], h1[kChan / 16];
     const int partner = (16 - c) & 15;
 #pragma unroll
     for (int i = 0; i < kChan / 16; ++i) {
@@ -148,8 +166,8 @@ __global__ void __launch_bounds__(kThreads) fengine_kernel(const Params prm) {
         float2 q = make_float2(__shfl_sync(0xffffffffu, v[15 - i].x, partner, 16), __shfl_sync(0xffffffffu, v[15 - i].y, partner, 16));
         if (c == 0) q = v[(16 - i) & 15];
         // S_m = (Z[k] + conj(Z[N-k])) / 2 ;  S_{m+1} = (Z[k] - conj(Z[N-k])) / (2j)
-        h0[i] = __floats2half2_rn(0.5f * (p.x + q.x), 0.5f * (p.y - q.y));
-        h1[i] = __floats2half2_rn(0.5f * (p.y + q.y), 0.5f * (q.x - p.x));
+        h0[i] = Out<kInt8>::cvt(0.5f * (p.x + q.x), 0.5f * (p.y - q.y), prm.scale);
+        h1[i] = Out<kInt8>::cvt(0.5f * (p.y + q.y), 0.5f * (q.x - p.x), prm.scale);
     }
     __syncthreads();                                              // every z[] has been consumed: reuse the memory
 #pragma unroll
@@ -164,7 +182,7 @@ __global__ void __launch_bounds__(kThreads) fengine_kernel(const Params prm) {
     if (m0 + col < prm.n_stream) {
 #pragma unroll 4
         for (int k = tid >> 5; k < kChan; k += kThreads / 32)
-            prm.out[(a * kChan + k) * prm.n_stream + m0 + col] = ost[k][col];
+            static_cast<OutT*>(prm.out)[(a * kChan + k) * prm.n_stream + m0 + col] = ost[k][col];
     }
     __syncthreads();                                              // staging (aliased onto buf) is free again
     }   // spectra of this block

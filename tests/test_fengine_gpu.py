@@ -88,3 +88,48 @@ def test_fengine_argument_errors(corr):
     assert b"corr_fengine" in L.corr_last_error(None)
     with pytest.raises(ValueError):
         corr.fengine(torch.zeros((4, 500), dtype=torch.int8, device="cuda"))
+
+
+# ---- requantised int8 output (corr_fengine_ci8): the code is decided by rint of an fp32 product on the GPU and of an
+# fp64 product in the oracle, so the two must agree EXACTLY except where the scaled value lies within the fp32 round-off
+# bound of a rounding tie, and there they may differ by one code (quantised decisions) ----
+@pytest.mark.parametrize("M,A,scale", [(2, 3, 1.0 / 64), (33, 4, 1.0 / 40), (64, 8, 0.05), (100, 5, 1.0 / 300)])
+def test_fengine_ci8_codes(corr, M, A, scale):
+    from oracle import fengine as fo
+    rng = np.random.default_rng(9100 + M)
+    s = np.clip(np.rint(rng.normal(0, 25, size=(M, A * 256))), -127, 127).astype(np.int8)
+    got = corr.fengine(torch.from_numpy(s).cuda(), scale=scale).cpu().numpy()
+    S = fo.fengine(s)
+    want, tie = fo.quantise_ci8(S, scale)
+    assert got.dtype == np.int8 and got.shape == want.shape
+    l1 = np.abs(s.reshape(M, A, 256).astype(np.float64)).sum(axis=2).T[:, None, :, None]      # [A, 1, M, 1]
+    near_tie = tie <= (2e-6 * l1 + 1e-6 * np.abs(np.stack([S.real, S.imag], -1))) * scale + 1e-7
+    diff = got.astype(np.int16) - want.astype(np.int16)
+    assert (diff[~near_tie] == 0).all()
+    assert (np.abs(diff[near_tie]) <= 1).all()
+    assert near_tie.mean() < 5e-3                      # the tie band is tiny: the test is essentially exact
+    assert got.min() >= -127
+
+
+def test_fengine_ci8_then_int8_xengine_chain(corr):
+    """The whole int8 FX pair on the GPU: samples -> corr_fengine_ci8 -> corr_xengine (CORR_CI8); the X-engine stage is
+    bit-exact against the oracle on the F-engine's own codes."""
+    import oracle
+    N, P, A = 40, 2, 128
+    rng = np.random.default_rng(78)
+    s = np.clip(np.rint(rng.normal(0, 20, size=(N * P, A * 256))), -127, 127).astype(np.int8)
+    x = corr.fengine(torch.from_numpy(s).cuda(), scale=1.0 / 20)                 # sigma ~ 16 codes per component
+    assert 8 < x.float().std().item() < 24
+    x5 = x.view(A, 128, N, P, 2)
+    with corr.Correlator(N, P, 128, A, "ci8") as h:
+        got = h.xengine(x5).cpu().numpy().astype(np.int64)
+    assert (got == oracle.xengine(x5.cpu().numpy())).all()
+
+
+def test_fengine_ci8_argument_errors(corr):
+    L = corr.lib()
+    s = torch.zeros((4, 512), dtype=torch.int8, device="cuda")
+    out = torch.empty((2, 128, 4, 2), dtype=torch.int8, device="cuda")
+    assert L.corr_fengine_ci8(s.data_ptr(), out.data_ptr(), 4, 2, 0.0, None) == corr.CORR_EINVAL
+    assert L.corr_fengine_ci8(s.data_ptr(), None, 4, 2, 1.0, None) == corr.CORR_EINVAL
+    assert L.corr_fengine_ci8(s.data_ptr(), out.data_ptr() + 1, 4, 2, 1.0, None) == corr.CORR_EINVAL
