@@ -167,8 +167,9 @@ const char* corr_last_error(corr_handle h);
 
 /* Force one of the CORR_KERNEL_* variants for subsequent corr_xengine calls (CORR_KERNEL_AUTO restores the
  * default choice).  CORR_EUNSUPPORTED if the geometry / device cannot run it.  corr_get_kernel returns the
- * kernel that WILL run (never CORR_KERNEL_AUTO): SIMT when TMA cannot address the geometry, else PAIR for
- * 2*N*P >= 256 real components per channel, SINGLE below (QUAD only on request: it measured slower). */
+ * kernel that WILL run (never CORR_KERNEL_AUTO): SIMT when TMA cannot address the geometry, else PAIR or SINGLE,
+ * whichever executes the geometry cheaper (PAIR for 2*N*P >= 256 unless its 256 x 256 tiles pad a ragged 2*N*P by more
+ * than 1.39x the 128-row tiles of SINGLE; QUAD only on request: it measured slower). */
 int corr_set_kernel(corr_handle h, int kernel);
 int corr_get_kernel(corr_handle h);
 

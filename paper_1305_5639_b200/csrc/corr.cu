@@ -163,11 +163,16 @@ int resolve_kernel(const corr_plan* h) {
     if (!h->tma_ok) return CORR_KERNEL_SIMT;
     if (h->kernel != CORR_KERNEL_AUTO) return h->kernel;
     if (h->Nb) return h->max_clusters[0] > 0 ? CORR_KERNEL_PAIR : CORR_KERNEL_SIMT;
-    const int M2 = 2 * h->M;
     // CORR_KERNEL_QUAD (multicast between two pairs) is never chosen: measured 12 % slower than PAIR at config 4
-    // (profiles/): the multicast saves L2 reads but not delivered bytes, and couples the two pairs' pipelines
-    if (M2 >= 256 && h->max_clusters[0] > 0) return CORR_KERNEL_PAIR;
-    return CORR_KERNEL_SINGLE;
+    // (profiles/): the multicast saves L2 reads but not delivered bytes, and couples the two pairs' pipelines.
+    // PAIR vs SINGLE by executed MACs per sample and channel: a pair MAC costs ~0.72 of a 1-CTA MAC (half the operand
+    // bytes from L2), but 256 x 256 tiles pad ragged 2M far more than 128-row tiles do.  Measured crossover (T = 2048,
+    // N = 72 .. 384): PAIR wins iff pair MACs / single MACs < 1.39.
+    if (h->max_clusters[0] <= 0 || 2 * h->M < 256) return CORR_KERNEL_SINGLE;
+    double single_macs = 0.0;
+    for (const xtc::TileDesc& t : h->h_tiles) single_macs += static_cast<double>(xtc::kTileRows) * t.ncols;
+    const double pair_macs = static_cast<double>(h->h_groups[0].size()) * xtc::kPairRows * xtc::kTileCols;
+    return pair_macs < 1.39 * single_macs ? CORR_KERNEL_PAIR : CORR_KERNEL_SINGLE;
 }
 
 size_t input_bytes(const corr_plan* h) {
