@@ -135,12 +135,15 @@ __global__ void __launch_bounds__(kThreads) fengine_kernel(const Params prm) {
     //      z[n] = s_m[n] + j s_{m+1}[n] ----
     float2 v[16];
     {
-        const int8_t* pa = prm.in + m * row + a * kFft + c;
-        const int8_t* pb = pa + row;
+        const uint8_t* pa = reinterpret_cast<const uint8_t*>(prm.in) + m * row + a * kFft + c;
+        const uint8_t* pb = pa + row;
         const bool oka = m < prm.n_stream, okb = m + 1 < prm.n_stream;
+        // int8 -> fp32 on the ALU pipe: the byte b (two's complement of x) gives b ^ 0x80 = x + 128 in [0, 255]; placed in
+        // the mantissa of 2^23 it reads as the float 2^23 + x + 128 exactly (an I2F would run on the quarter-rate XU pipe)
+        auto cvt = [](uint32_t b) { return __uint_as_float(0x4B000000u | (b ^ 0x80u)) - 8388736.0f; };
 #pragma unroll
         for (int n1 = 0; n1 < 16; ++n1)
-            v[n1] = make_float2(oka ? static_cast<float>(pa[16 * n1]) : 0.0f, okb ? static_cast<float>(pb[16 * n1]) : 0.0f);
+            v[n1] = make_float2(oka ? cvt(pa[16 * n1]) : 0.0f, okb ? cvt(pb[16 * n1]) : 0.0f);
     }
     dft16(v);
     __syncwarp();                                                 // the 16 threads of a transform share a warp
