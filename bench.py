@@ -61,6 +61,9 @@ def parse_args():
     ap.add_argument("--piece", default="xengine", choices=["xengine", "corner_turn", "fengine"],
                     help="corner_turn: time the standalone corner-turn kernel (SURVEY 8(a) a1) on the workload's input; "
                          "fengine: time corr_fengine (SURVEY 8(f) rank 2) on 512 streams x 8192 spectra of 256 real int8 samples")
+    ap.add_argument("--shard", default="none", choices=["none", "channels"],
+                    help="channels: the N ranks split the workload's channels (strong scaling, SURVEY 8(f) rank 3); "
+                         "default: N independent replicas (north_star: the path does not shard)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-gemm-peak", action="store_true",
@@ -361,6 +364,16 @@ def run_native(args):
     binding.lib()                                   # raises if libcorr.so is missing / cannot be built
 
     cfg = workload(args.workload)
+    sharded = args.shard == "channels" and world > 1
+    if sharded:
+        # this rank owns a contiguous block of channels: a smaller, otherwise identical problem with its own output slab
+        from paper_1305_5639_b200.shard import channel_range
+        c0, c1 = channel_range(cfg["C"], world, rank)
+        frac = (c1 - c0) / cfg["C"]
+        for key in ("cmacs_per_call", "ops_per_call", "in_bytes", "out_bytes"):
+            cfg[key] = int(cfg[key] * frac)
+        cfg["C_total"], cfg["C"] = cfg["C"], c1 - c0
+        cfg["seed"] = cfg["seed"] + 7 * rank            # each slab gets its own noise
     N, P, C, T, dtype, calls = cfg["N"], cfg["P"], cfg["C"], cfg["T"], cfg["dtype"], cfg["calls"]
     K, W = args.steps, max(args.warmup, 3)
     pk = peaks()
@@ -425,7 +438,13 @@ def run_native(args):
     total_ms = sum(step_ms)          # device time of exactly K steps (flush kernels excluded)
     total_ms = max_over_ranks(total_ms, dist, world, "cuda")
     ops_step = cfg["ops_per_call"] * calls
-    value = whole_job_value(ops_step, K, world, total_ms) / 1e12
+    if sharded:
+        # strong scaling: the job is ONE workload; sum the ranks' (nearly equal) shares
+        t_ops = torch.tensor([float(ops_step)], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t_ops, op=dist.ReduceOp.SUM)
+        value = whole_job_value(float(t_ops.item()), K, 1, total_ms) / 1e12
+    else:
+        value = whole_job_value(ops_step, K, world, total_ms) / 1e12
     kernel_ms = sum(call_ms) / len(call_ms)          # average launch duration of the dominant (only) kernel
 
     # ---- e2e: HOST pinned buffers through corr_xengine_host --------------------------------------
@@ -504,11 +523,11 @@ def run_native(args):
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-        "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
         "dtype": "s8 x s8 -> s32" if dtype == "ci8" else "f16 x f16 -> f32", "data": "synthetic",
         "config": {"workload": describe(cfg), "l2": ("flushed between steps" if flush is not None else
                                                      "inputs (%.0f MiB per step) larger than L2" % (in_total / 2 ** 20)),
-                   "parallelism": "replicas only (x%d)" % world, "visibilities_per_s": world * K * C * cfg["n_baseline"] * P * P
+                   "parallelism": ("channels sharded over %d ranks, no collective" % world) if sharded else "replicas only (x%d)" % world, "visibilities_per_s": world * K * C * cfg["n_baseline"] * P * P
                    / (total_ms * 1e-3)},
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_call * calls * K,
         "roofline": roofline, "cpu_baseline": cpu,

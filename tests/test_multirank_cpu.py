@@ -64,3 +64,51 @@ def test_reference_arm_under_torchrun_prints_one_line():
     d = json.loads(lines[0])
     assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["value"] > 0
     assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
+
+
+# ---- channel sharding: host logic + equivalence to the unsharded result, world_size 2 on gloo ----
+def test_channel_ranges_partition_the_channels():
+    from paper_1305_5639_b200.shard import channel_range
+    for C in (0, 1, 5, 64, 1000, 1024):
+        for world in (1, 2, 3, 8):
+            parts = [channel_range(C, world, r) for r in range(world)]
+            assert parts[0][0] == 0 and parts[-1][1] == C
+            assert all(parts[r][1] == parts[r + 1][0] for r in range(world - 1))
+            sizes = [b - a for a, b in parts]
+            assert max(sizes) - min(sizes) <= 1
+
+
+def _shard_worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, ROOT)
+    import numpy as np
+    import torch
+    import oracle
+    from paper_1305_5639_b200 import inputs
+    from paper_1305_5639_b200.shard import channel_range
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    T, C, N, P = 40, 7, 5, 2
+    x = inputs.gauss_ci8(T, C, N, P, 30.0, seed=123)                 # every rank derives the same stream from the seed
+    c0, c1 = channel_range(C, world, rank)
+    mine = torch.from_numpy(oracle.xengine(x[:, c0:c1].contiguous().numpy()))     # this rank's output slab
+    slabs = [None] * world
+    dist.all_gather_object(slabs, (c0, c1, mine))                    # test-only gather; the data path has no collective
+    full = torch.cat([s[2] for s in sorted(slabs, key=lambda s: s[0])])
+    want = torch.from_numpy(oracle.xengine(x.numpy()))
+    out.put((rank, bool((full == want).all()), (c0, c1)))
+    dist.destroy_process_group()
+
+
+def test_channel_sharded_slabs_equal_the_unsharded_result_world2():
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 33500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_shard_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = sorted(q.get(timeout=180) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert [g[1] for g in got] == [True, True]
+    assert got[0][2] == (0, 4) and got[1][2] == (4, 7)
