@@ -11,9 +11,14 @@
  * no normalisation), optionally integrated across successive calls ("results are usually then
  * accumulated", Sec. 2).
  *
- * Every function is extern "C", never throws and never aborts.  Pointers are plain; each
+ * Every function is extern "C", never throws and never aborts the process.  Pointers are plain; each
  * argument says whether it is a HOST or a DEVICE pointer.  The library links only the CUDA
  * runtime; callers may use anything (e.g. PyTorch) for device memory and streams.
+ * Device-side watchdog: the tensor-core kernels wait on hardware barriers; should one not complete
+ * within 2^33 SM clocks (seconds; a legitimate wait is microseconds) the kernel traps instead of
+ * hanging the GPU, the stream reports a launch failure (CORR_ECUDA from the next call that checks)
+ * and the CUDA context is unusable afterwards, as after any device-side fault.
+ * Devices: compute capability 10.0 only (B200 / GB200); the library carries sm_100a code, no PTX.
  *
  * Layouts (C-contiguous, fastest axis last)
  *   in   [n_time][n_chan][n_station][n_pol] complex, (re, im) interleaved:
@@ -57,8 +62,7 @@ enum {
     CORR_KERNEL_AUTO = 0,    /* default: chosen from the geometry (see corr_get_kernel)                              */
     CORR_KERNEL_SINGLE = 1,  /* tcgen05, one CTA per 128 x 256 tile of the per-channel Gram matrix                   */
     CORR_KERNEL_PAIR = 2,    /* tcgen05 cta_group::2: a CTA pair per 256 x 256 tile (half the L2 bytes per MAC of B)  */
-    CORR_KERNEL_QUAD = 3,    /* two CTA pairs per 4-CTA cluster, the operand their tiles share fetched once (multicast) */
-    CORR_KERNEL_SIMT = 4     /* CUDA-core kernel for geometries TMA cannot address (and a cross-check)                */
+    CORR_KERNEL_SIMT = 3     /* CUDA-core kernel for geometries TMA cannot address (and a cross-check)                */
 };
 
 /*
@@ -69,6 +73,22 @@ enum {
  * The handle owns its device allocations until corr_destroy.
  */
 corr_handle corr_create(int n_station, int n_pol, int n_chan, int n_time, int dtype);
+
+/*
+ * corr_create_window -- plan for a CHANNEL WINDOW of a larger problem.  Eq. 2 is independent per
+ * frequency channel (the paper's "orthogonal correlation triangles separating frequency channels prior to the CMAC
+ * stage"), so several handles -- on one GPU or one per GPU / process -- can each integrate a block of
+ * channels of ONE input into their own slabs of ONE output with no communication.  The handle processes channels
+ * [chan0, chan0 + n_chan) of buffers laid out for n_chan_total channels, IN PLACE:
+ *   in   [n_time][n_chan_total][n_station][n_pol]  -- the whole-band buffer; only the window's columns are read
+ *   out  [n_chan_total][B][n_pol][n_pol]           -- the whole-band buffer; only slabs chan0 .. chan0 + n_chan - 1 are
+ *                                                     written (or accumulated into); every other byte is left untouched
+ * corr_input_bytes / corr_output_bytes report the WHOLE-BAND sizes.  0 <= chan0, 1 <= n_chan, chan0 + n_chan <=
+ * n_chan_total.  Everything else (corr_xengine, corr_xengine_dumps, corr_xengine_host, accumulate, errors) as for
+ * corr_create; corr_create(N, P, C, T, d) == corr_create_window(N, P, C, 0, C, T, d).  corr_corner_turn is not
+ * available on a window plan.  With corr_xengine_host only the window's input columns and output slabs cross the bus.
+ */
+corr_handle corr_create_window(int n_station, int n_pol, int n_chan_total, int chan0, int n_chan, int n_time, int dtype);
 
 /*
  * corr_xengine -- one integration of n_time samples (Eq. 2), asynchronous on `stream`.
@@ -85,12 +105,15 @@ corr_handle corr_create(int n_station, int n_pol, int n_chan, int n_time, int dt
 int corr_xengine(corr_handle h, const void* in, void* out, int accumulate, void* stream);
 
 /*
- * corr_xengine_host -- same operation with HOST buffers (blocking): copies `in_host` to a device
- * staging buffer owned by the handle, runs corr_xengine on the handle's own stream, copies the
- * result to `out_host` and synchronises.  With accumulate != 0 the running sum lives in the
- * handle's device staging buffer (state of the previous corr_xengine_host call on this handle) and
- * `out_host` receives the updated integration; `out_host` may be NULL to leave the running sum on
- * the device until a later call asks for it.  Pinned host memory makes the copies DMA directly.
+ * corr_xengine_host -- same operation with HOST buffers (blocking; layouts and sizes as corr_xengine).  The plan's
+ * channels are cut into up to 8 windows that flow through a three-stage pipeline on the handle's own streams: the
+ * host-to-device copy of window w+1 (a strided 2-D copy straight out of `in_host`), the X-engine kernel on window w,
+ * and the device-to-host copy of window w-1's output slab overlap, so the bus runs in both directions while the GPU
+ * computes.  The handle owns the device staging (two input windows + the running output).  With accumulate != 0 the
+ * running sum lives in that device buffer (state of the previous corr_xengine_host call on this handle) and
+ * `out_host` receives the updated integration; `out_host` may be NULL to leave the running sum on the device until a
+ * later call asks for it.  Returns after all copies have completed.  PINNED host memory is needed for the copies to
+ * overlap (pageable memory works but serialises).  CORR_EOVERFLOW as corr_xengine.
  */
 int corr_xengine_host(corr_handle h, const void* in_host, void* out_host, int accumulate);
 
@@ -157,7 +180,7 @@ void corr_destroy(corr_handle h);
 
 /* ---- helpers ------------------------------------------------------------------------------ */
 
-size_t corr_input_bytes(corr_handle h);      /* T*C*N*P * (2 or 4); 0 for NULL                  */
+size_t corr_input_bytes(corr_handle h);      /* T*C*N*P * (2 or 4); 0 for NULL  (C = n_chan_total of a window plan) */
 size_t corr_output_bytes(corr_handle h);     /* C*B*P*P * 8;        0 for NULL                  */
 long long corr_baseline_index(int i, int j); /* i(i+1)/2 + j for 0 <= j <= i, else -1           */
 
@@ -169,7 +192,7 @@ const char* corr_last_error(corr_handle h);
  * default choice).  CORR_EUNSUPPORTED if the geometry / device cannot run it.  corr_get_kernel returns the
  * kernel that WILL run (never CORR_KERNEL_AUTO): SIMT when TMA cannot address the geometry, else PAIR or SINGLE,
  * whichever executes the geometry cheaper (PAIR for 2*N*P >= 256 unless its 256 x 256 tiles pad a ragged 2*N*P by more
- * than 1.39x the 128-row tiles of SINGLE; QUAD only on request: it measured slower). */
+ * than 1.39x the 128-row tiles of SINGLE). */
 int corr_set_kernel(corr_handle h, int kernel);
 int corr_get_kernel(corr_handle h);
 
@@ -183,7 +206,8 @@ int corr_uses_tensor_cores(corr_handle h);
  * optimizing the GPU memory access"):
  *     ws    [c][m][t] = in[t][c][m]            (m = s*n_pol + p, complex kept interleaved)
  *     ws_rot[c][m][t] = (im, -re) of the same sample           (feeds the imaginary part)
- * with the time axis padded to corr_workspace_time(h) samples (zero filled).
+ * with the time axis padded to corr_workspace_time(h) samples (zero filled).  CORR_CI8: -re saturates, so a real part
+ * of -128 (outside the generators' [-127, 127]) becomes +127 in ws_rot; every other value is exact.
  *   in      DEVICE pointer as for corr_xengine.
  *   ws      DEVICE pointer, corr_workspace_bytes(h) bytes, 128-byte aligned: the two planes,
  *           ws then ws_rot, each n_chan * M * corr_workspace_time(h) samples.
@@ -197,14 +221,13 @@ int corr_workspace_time(corr_handle h);
  * Introspection of the triangular tile schedule (host logic, no GPU work): writes up to `max_tiles`
  * entries of {row0, col0, ncols} (units: real components u = 2*m + {re:0, im:1} within a channel,
  * rows = conjugated side) for ONE channel and returns the number of tiles per channel.
- * Usable without a handle or a GPU.  `kernel` is CORR_KERNEL_SINGLE (128-row tiles, ncols <= 256),
- * CORR_KERNEL_PAIR (256 x 256 tiles) or CORR_KERNEL_QUAD (256 x 256 tiles in cluster order: entries 2k and
- * 2k+1 run on the two pairs of one cluster and share their rows or their columns; ncols == 0 marks the
- * duplicate of an odd tile out, which is computed but not written).
+ * Usable without a handle or a GPU.  `kernel` is CORR_KERNEL_SINGLE (128-row tiles, ncols <= 256) or
+ * CORR_KERNEL_PAIR (256 x 256 tiles).
  */
 int corr_tile_schedule(int n_station, int n_pol, int dtype, int kernel, int* tiles3, int max_tiles);
 
-/* Number of kernels launched by the last corr_xengine / corr_xengine_host call on this handle. */
+/* Number of kernels launched by the last corr_xengine / corr_xengine_host call on this handle (corr_xengine_host: one
+ * per channel window). */
 int corr_last_launch_count(corr_handle h);
 
 #ifdef __cplusplus

@@ -13,7 +13,7 @@ LIB_PATH = os.path.join(HERE, "libcorr.so")
 
 CORR_CI8, CORR_CF16 = 0, 1
 CORR_OK, CORR_EINVAL, CORR_EUNSUPPORTED, CORR_ENOMEM, CORR_ECUDA, CORR_EOVERFLOW = 0, -1, -2, -3, -4, -5
-KERNELS = {"auto": 0, "single": 1, "pair": 2, "quad": 3, "simt": 4}      # CORR_KERNEL_*
+KERNELS = {"auto": 0, "single": 1, "pair": 2, "simt": 3}      # CORR_KERNEL_*
 KERNEL_NAMES = {v: k for k, v in KERNELS.items()}
 DTYPES = {"ci8": CORR_CI8, "cf16": CORR_CF16}
 
@@ -21,6 +21,7 @@ DTYPES = {"ci8": CORR_CI8, "cf16": CORR_CF16}
 _vp, _i, _sz, _ll, _cp = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t, ctypes.c_longlong, ctypes.c_char_p
 SYMBOLS = {
     "corr_create": (_vp, [_i, _i, _i, _i, _i]),
+    "corr_create_window": (_vp, [_i, _i, _i, _i, _i, _i, _i]),
     "corr_xengine": (_i, [_vp, _vp, _vp, _i, _vp]),
     "corr_xengine_host": (_i, [_vp, _vp, _vp, _i]),
     "corr_create_cross": (_vp, [_i, _i, _i, _i, _i, _i]),
@@ -131,10 +132,16 @@ def _fengine_ci8(samples, scale, out, stream):
 class Correlator:
     """corr_create / corr_xengine / corr_destroy with torch tensors as the device buffers."""
 
-    def __init__(self, n_station, n_pol, n_chan, n_time, dtype="ci8"):
+    def __init__(self, n_station, n_pol, n_chan, n_time, dtype="ci8", window=None):
+        """``window=(chan0, n_chan_window)``: corr_create_window -- the handle integrates only those channels of the
+        whole-band ``[T, n_chan, N, P, 2]`` input into their slabs of the whole-band output, in place."""
         self._L = lib()
         self.N, self.P, self.C, self.T, self.dtype = n_station, n_pol, n_chan, n_time, dtype
-        self._h = self._L.corr_create(n_station, n_pol, n_chan, n_time, DTYPES[dtype])
+        self.window = None if window is None else (int(window[0]), int(window[1]))
+        if window is None:
+            self._h = self._L.corr_create(n_station, n_pol, n_chan, n_time, DTYPES[dtype])
+        else:
+            self._h = self._L.corr_create_window(n_station, n_pol, n_chan, self.window[0], self.window[1], n_time, DTYPES[dtype])
         if not self._h:
             msg = self._L.corr_last_error(None).decode()
             raise CorrError(CORR_EINVAL if "invalid" in msg or "too large" in msg else CORR_EUNSUPPORTED, msg)
@@ -167,7 +174,7 @@ class Correlator:
 
     @property
     def kernel(self):
-        """Name of the kernel corr_xengine will launch: single / pair / quad / simt."""
+        """Name of the kernel corr_xengine will launch: single / pair / simt."""
         return KERNEL_NAMES[int(self._L.corr_get_kernel(self._h))]
 
     def set_kernel(self, kernel):
@@ -210,8 +217,8 @@ class Correlator:
         """corr_xengine on device tensors; asynchronous on ``stream`` (default: torch's current)."""
         self._check_in(x, "cuda")
         if out is None:
-            if accumulate:
-                raise ValueError("accumulate=True needs the running `out`")
+            if accumulate or self.window is not None:
+                raise ValueError("accumulate=True and window plans need the caller's `out`")
             out = self.empty_output(x.device)
         self._check_out(out, "cuda")
         self._check(self._L.corr_xengine(self._h, x.data_ptr(), out.data_ptr(), int(bool(accumulate)),

@@ -5,9 +5,11 @@
 nvcc cross-compiles without a GPU.  The CUDA runtime is linked statically, so the library has
 no dependency on torch (callers pass plain device pointers and a cudaStream_t).
 """
+import fcntl
 import os
 import subprocess
 import sys
+import tempfile
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
@@ -41,26 +43,41 @@ def _nvcc():
     return "nvcc"
 
 
+def _stale():
+    if not os.path.exists(LIB):
+        return True
+    newest = max(os.path.getmtime(d) for d in _deps() + [os.path.abspath(__file__)])
+    return os.path.getmtime(LIB) < newest
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and os.path.exists(LIB):
-        newest = max(os.path.getmtime(d) for d in _deps() + [os.path.abspath(__file__)])
-        if os.path.getmtime(LIB) >= newest:
-            return LIB
-    cmd = [_nvcc()] + NVCC_FLAGS + ["-I", INCLUDE]
-    if verbose:
-        cmd += ["-Xptxas", "-v"]
-    if os.environ.get("CORR_DEFINES"):        # developer build: extra -D switches for A/B experiments
-        cmd += os.environ["CORR_DEFINES"].split()
-    if os.environ.get("CORR_STATS"):          # developer build: per-role stall counters (clock64) in the pair kernel
-        cmd += ["-DCORR_STATS"]
-    cmd += _sources() + ["-o", LIB + ".tmp"]
-    res = subprocess.run(cmd, capture_output=True, text=True)
-    if res.returncode != 0:
-        sys.stderr.write(res.stdout + res.stderr)
-        raise RuntimeError("nvcc failed building libcorr.so")
-    if verbose:
-        sys.stderr.write(res.stdout + res.stderr)
-    os.replace(LIB + ".tmp", LIB)
+    """Compile libcorr.so if it is missing or older than its sources.  Safe when several processes (torchrun ranks)
+    call it at once: one compiles under a file lock into its own temporary file, the others wait and find it built."""
+    if not force and not _stale():
+        return LIB
+    with open(LIB + ".lock", "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        try:
+            if not force and not _stale():          # another process built it while this one waited for the lock
+                return LIB
+            fd, tmp = tempfile.mkstemp(prefix="libcorr.", suffix=".so.tmp", dir=HERE)
+            os.close(fd)
+            cmd = [_nvcc()] + NVCC_FLAGS + ["-I", INCLUDE]
+            if verbose:
+                cmd += ["-Xptxas", "-v"]
+            cmd += _sources() + ["-o", tmp]
+            res = subprocess.run(cmd, capture_output=True, text=True)
+            if res.returncode != 0:
+                sys.stderr.write(res.stdout + res.stderr)
+                if os.path.exists(tmp):
+                    os.unlink(tmp)
+                raise RuntimeError("nvcc failed building libcorr.so")
+            if verbose:
+                sys.stderr.write(res.stdout + res.stderr)
+            os.chmod(tmp, 0o755)
+            os.replace(tmp, LIB)
+        finally:
+            fcntl.flock(lock, fcntl.LOCK_UN)
     return LIB
 
 

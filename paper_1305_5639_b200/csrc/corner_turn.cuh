@@ -40,7 +40,7 @@ __device__ __forceinline__ uint4 ldg_stream(const uint4* p) {
 template <int kSampleBytes> __device__ __forceinline__ uint32_t rotate_word(uint32_t w) {
     if constexpr (kSampleBytes == 2) {
         const uint32_t sw = __byte_perm(w, 0, 0x2301);          // [im0, re0, im1, re1]
-        const uint32_t ng = __vneg4(sw);                         // bytewise two's-complement negate
+        const uint32_t ng = __vnegss4(sw);                       // bytewise negate, saturating: -(-128) -> 127
         return (sw & 0x00ff00ffu) | (ng & 0xff00ff00u);          // negate the (new) imaginary bytes
     } else {
         return __byte_perm(w, 0, 0x1032) ^ 0x80000000u;          // [im, re] halves, flip sign of the upper

@@ -22,8 +22,10 @@
 
 namespace {
 
-constexpr long long kMaxIntegrationCi8 = 65535;
-constexpr unsigned kSchedRing = 256;            // launches in flight on different streams never share a feed counter   // 2 * 128^2 * T_total <= 2^31 - 1
+constexpr long long kMaxIntegrationCi8 = 65535;   // 2 * 128^2 * T_total <= 2^31 - 1
+constexpr unsigned kSchedRing = 256;              // launches in flight on different streams never share a feed counter
+constexpr int kMapCache = 16;                     // encoded tensor maps kept per handle (config 4 cycles four inputs)
+constexpr int kHostWindows = 8;                   // corr_xengine_host: channel windows in flight through the copy pipeline
 
 thread_local char g_create_error[512] = "";
 
@@ -31,13 +33,33 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
+// What one launch addresses: `n_chan` channels starting at `chan0_in` of an input laid out for `c_total_in` channels
+// ([n_dump][n_time][c_total_in][M]), written to slabs `chan0_out`.. of an output laid out for `c_total_out` channels.
+struct View {
+    int n_time;            // samples per integration
+    int n_chan;
+    int c_total_in, chan0_in;
+    int c_total_out, chan0_out;
+};
+
+struct MapKey {
+    const void* ptr;
+    int streams;           // M of the group the map addresses
+    int c_total, n_time, n_dump, box_rows;
+    bool operator==(const MapKey& o) const {
+        return ptr == o.ptr && streams == o.streams && c_total == o.c_total && n_time == o.n_time && n_dump == o.n_dump &&
+               box_rows == o.box_rows;
+    }
+};
+
 }  // namespace
 
 struct corr_plan {
     int N, P, C, T, dtype;
+    int C_total, chan0;    // channel window [chan0, chan0 + C) of buffers laid out for C_total channels (whole band: 0, C)
     int M;                 // N * P
     int Nb, Mb;            // rectangular cross-only plan (corr_create_cross): stations / streams of group B; 0 = HERK
-    long long B;           // N (N + 1) / 2
+    long long B;           // N (N + 1) / 2, or N * Nb for a cross plan
     int sample_bytes;      // 2 (ci8) or 4 (cf16)
     int device;
     int sm_count;
@@ -49,27 +71,27 @@ struct corr_plan {
     int kernel;            // requested CORR_KERNEL_*
     std::vector<xtc::TileDesc> h_tiles;
     xtc::TileDesc* d_tiles;
-    std::vector<xtc::PairGroup> h_groups[2];   // [0]: one pair per cluster, [1]: two pairs per cluster (multicast)
-    xtc::PairGroup* d_groups[2];
+    std::vector<xtc::PairTile> h_pair_tiles;
+    xtc::PairTile* d_pair_tiles;
     unsigned int* d_sched;                     // ring of tile-feed counters, one per launch (kSchedRing)
     unsigned int sched_seq;
-    int max_clusters[2];                       // co-resident clusters of 2 / 4 CTAs (cudaOccupancyMaxActiveClusters)
+    int max_clusters;                          // co-resident CTA pairs (cudaOccupancyMaxActiveClusters)
     EncodeTiledFn encode;
 
-    CUtensorMap tmap_in;     // 1-CTA kernel: box [128 B][Cfg::kKStage samples]
-    CUtensorMap tmap_pair;   // pair kernels: box [128 B][kPairStageK / kPairBoxes samples]
-    const void* tmap_in_ptr;
-    int tmap_dumps;          // n_dump the pair tensor map was encoded for
-    CUtensorMap tmap_b;      // cross plans: group B, pair-kernel box
-    const void* tmap_b_ptr;
+    // encoded tensor maps, least recently used replaced
+    MapKey map_key[kMapCache];
+    CUtensorMap map_val[kMapCache];
+    unsigned long long map_used[kMapCache];
+    unsigned long long map_clock;
 
     // corner-turn feed
     int Tp;                // padded time extent of the workspace
 
-    // corr_xengine_host staging
-    void* d_in_stage;
+    // corr_xengine_host: device staging (two input windows, the running output) and the copy pipeline
+    void* d_in_stage[2];
     void* d_out_stage;
-    cudaStream_t own_stream;
+    cudaStream_t st_h2d, st_run, st_d2h;
+    cudaEvent_t ev_h2d[2], ev_run[2];
 
     char err[512];
 };
@@ -122,144 +144,109 @@ void build_pair_tiles(int N, int P, std::vector<xtc::PairTile>& v) {
         for (int rb = cb; rb < R; ++rb) v.push_back(xtc::PairTile{rb * xtc::kPairRows, cb * xtc::kPairRows});
 }
 
-// Groups of ONE channel.  pairs_per_cluster == 1: one tile per group.  == 2: two tiles sharing their column
-// block (B multicast); the odd tile out of each column block lies in the last row block, and those are joined
-// two by two (A multicast); a last single tile is duplicated (computed twice, written once).
-void build_groups(int N, int P, int pairs_per_cluster, std::vector<xtc::PairGroup>& g) {
-    g.clear();
-    const int M2 = 2 * N * P;
-    const int R = (M2 + xtc::kPairRows - 1) / xtc::kPairRows;
-    if (pairs_per_cluster == 1) {
-        std::vector<xtc::PairTile> t;
-        build_pair_tiles(N, P, t);
-        for (const xtc::PairTile& x : t) g.push_back(xtc::PairGroup{{x, x}, 0, 0});
-        return;
-    }
-    std::vector<xtc::PairTile> odd;
-    for (int cb = 0; cb < R; ++cb) {
-        int rb = cb;
-        for (; rb + 1 < R; rb += 2)
-            g.push_back(xtc::PairGroup{{{rb * xtc::kPairRows, cb * xtc::kPairRows}, {(rb + 1) * xtc::kPairRows, cb * xtc::kPairRows}}, 2, 0});
-        if (rb < R) odd.push_back(xtc::PairTile{rb * xtc::kPairRows, cb * xtc::kPairRows});
-    }
-    size_t k = 0;
-    for (; k + 1 < odd.size(); k += 2) g.push_back(xtc::PairGroup{{odd[k], odd[k + 1]}, 1, 0});
-    if (k < odd.size()) g.push_back(xtc::PairGroup{{odd[k], odd[k]}, 3, 0});
-}
-
 // Rectangular cross-only plan: every 256 x 256 block of the [2 M_a] x [2 M_b] rectangle, column-block major.
-void build_groups_rect(int Na, int Nb, int P, std::vector<xtc::PairGroup>& g) {
-    g.clear();
+void build_pair_tiles_rect(int Na, int Nb, int P, std::vector<xtc::PairTile>& v) {
+    v.clear();
     const int Ra = (2 * Na * P + xtc::kPairRows - 1) / xtc::kPairRows;
     const int Rb = (2 * Nb * P + xtc::kPairRows - 1) / xtc::kPairRows;
     for (int cb = 0; cb < Rb; ++cb)
-        for (int rb = 0; rb < Ra; ++rb) {
-            const xtc::PairTile t{rb * xtc::kPairRows, cb * xtc::kPairRows};
-            g.push_back(xtc::PairGroup{{t, t}, 0, 0});
-        }
+        for (int rb = 0; rb < Ra; ++rb) v.push_back(xtc::PairTile{rb * xtc::kPairRows, cb * xtc::kPairRows});
 }
 
 int resolve_kernel(const corr_plan* h) {
     if (!h->tma_ok) return CORR_KERNEL_SIMT;
     if (h->kernel != CORR_KERNEL_AUTO) return h->kernel;
-    if (h->Nb) return h->max_clusters[0] > 0 ? CORR_KERNEL_PAIR : CORR_KERNEL_SIMT;
-    // CORR_KERNEL_QUAD (multicast between two pairs) is never chosen: measured 12 % slower than PAIR at config 4
-    // (profiles/): the multicast saves L2 reads but not delivered bytes, and couples the two pairs' pipelines.
+    if (h->Nb) return h->max_clusters > 0 ? CORR_KERNEL_PAIR : CORR_KERNEL_SIMT;
     // PAIR vs SINGLE by executed MACs per sample and channel: a pair MAC costs ~0.72 of a 1-CTA MAC (half the operand
     // bytes from L2), but 256 x 256 tiles pad ragged 2M far more than 128-row tiles do.  Measured crossover (T = 2048,
     // N = 72 .. 384): PAIR wins iff pair MACs / single MACs < 1.39.
-    if (h->max_clusters[0] <= 0 || 2 * h->M < 256) return CORR_KERNEL_SINGLE;
+    if (h->max_clusters <= 0 || 2 * h->M < 256) return CORR_KERNEL_SINGLE;
     double single_macs = 0.0;
     for (const xtc::TileDesc& t : h->h_tiles) single_macs += static_cast<double>(xtc::kTileRows) * t.ncols;
-    const double pair_macs = static_cast<double>(h->h_groups[0].size()) * xtc::kPairRows * xtc::kTileCols;
+    const double pair_macs = static_cast<double>(h->h_pair_tiles.size()) * xtc::kPairRows * xtc::kTileCols;
     return pair_macs < 1.39 * single_macs ? CORR_KERNEL_PAIR : CORR_KERNEL_SINGLE;
 }
 
+// sizes of the caller's buffers: always the WHOLE band (C_total channels), also for a window plan
 size_t input_bytes(const corr_plan* h) {
-    return static_cast<size_t>(h->T) * h->C * h->M * h->sample_bytes;
+    return static_cast<size_t>(h->T) * h->C_total * h->M * h->sample_bytes;
 }
 size_t output_bytes(const corr_plan* h) {
-    return static_cast<size_t>(h->C) * h->B * h->P * h->P * 8;
+    return static_cast<size_t>(h->C_total) * h->B * h->P * h->P * 8;
 }
 size_t workspace_bytes(const corr_plan* h) {
     return 2 * static_cast<size_t>(h->C) * h->M * h->Tp * h->sample_bytes;
 }
+View device_view(const corr_plan* h) { return View{h->T, h->C, h->C_total, h->chan0, h->C_total, h->chan0}; }
 
-int encode_map(corr_plan* h, CUtensorMap* map, const void* ptr, int M, int box_rows) {
+// Tensor map of `ptr` viewed as [n_dump][n_time][c_total * 2 streams] real components, box [128 B][box_rows samples][1]:
+// a box never crosses from one integration into the next, rows past an integration's end are zero-filled.  Encoded maps
+// are cached per (pointer, shape): a caller cycling a few input buffers (config 4: four) pays the encode once each.
+int get_map(corr_plan* h, const void* ptr, int streams, int c_total, int n_time, int n_dump, int box_rows,
+            const CUtensorMap** out) {
+    const MapKey key{ptr, streams, c_total, n_time, n_dump, box_rows};
+    int victim = 0;
+    for (int k = 0; k < kMapCache; ++k) {
+        if (h->map_used[k] && h->map_key[k] == key) {
+            h->map_used[k] = ++h->map_clock;
+            *out = &h->map_val[k];
+            return CORR_OK;
+        }
+        if (h->map_used[k] < h->map_used[victim]) victim = k;
+    }
     const int elt = h->sample_bytes / 2;                       // bytes per real component
-    const cuuint64_t W = static_cast<cuuint64_t>(h->C) * 2 * M;
-    cuuint64_t dims[2] = {W, static_cast<cuuint64_t>(h->T)};
-    cuuint64_t strides[1] = {W * elt};
-    cuuint32_t box[2] = {static_cast<cuuint32_t>(128 / elt), static_cast<cuuint32_t>(box_rows)};
-    cuuint32_t estr[2] = {1, 1};
-    const CUresult r = h->encode(map, elt == 1 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2,
-                                 const_cast<void*>(ptr), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                                 CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) return fail(h, CORR_ECUDA, "cuTensorMapEncodeTiled failed with CUresult %d", static_cast<int>(r));
-    return CORR_OK;
-}
-
-// Pair kernels: `ptr` viewed as [n_dump][T / n_dump][C*2M] (rank 3), box [128 B][stage samples][1]: a box never crosses
-// from one integration into the next, rows past an integration's end are zero-filled.
-int encode_map3(corr_plan* h, CUtensorMap* map, const void* ptr, int M, int box_rows, int n_dump) {
-    const int elt = h->sample_bytes / 2;
-    const cuuint64_t W = static_cast<cuuint64_t>(h->C) * 2 * M;
-    const cuuint64_t Ts = static_cast<cuuint64_t>(h->T / n_dump);
-    cuuint64_t dims[3] = {W, Ts, static_cast<cuuint64_t>(n_dump)};
-    cuuint64_t strides[2] = {W * elt, Ts * W * elt};
+    const cuuint64_t W = static_cast<cuuint64_t>(c_total) * 2 * streams;
+    cuuint64_t dims[3] = {W, static_cast<cuuint64_t>(n_time), static_cast<cuuint64_t>(n_dump)};
+    cuuint64_t strides[2] = {W * elt, static_cast<cuuint64_t>(n_time) * W * elt};
     cuuint32_t box[3] = {static_cast<cuuint32_t>(128 / elt), static_cast<cuuint32_t>(box_rows), 1};
     cuuint32_t estr[3] = {1, 1, 1};
-    const CUresult r = h->encode(map, elt == 1 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3,
-                                 const_cast<void*>(ptr), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+    const CUresult r = h->encode(&h->map_val[victim], elt == 1 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16,
+                                 3, const_cast<void*>(ptr), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                                  CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) return fail(h, CORR_ECUDA, "cuTensorMapEncodeTiled (rank 3) failed with CUresult %d", static_cast<int>(r));
+    if (r != CUDA_SUCCESS) {
+        h->map_used[victim] = 0;
+        return fail(h, CORR_ECUDA, "cuTensorMapEncodeTiled failed with CUresult %d", static_cast<int>(r));
+    }
+    h->map_key[victim] = key;
+    h->map_used[victim] = ++h->map_clock;
+    *out = &h->map_val[victim];
     return CORR_OK;
 }
 
-// Tensor maps of `in` viewed as [T][C*2M]: box [128 B][stage samples] for the 1-CTA kernel and for the pair kernels.
-int encode_input_map(corr_plan* h, const void* in, int n_dump = 1) {
-    if (h->tmap_in_ptr == in && h->tmap_dumps == n_dump) return CORR_OK;
-    h->tmap_in_ptr = nullptr;
-    const int elt = h->sample_bytes / 2;
-    int rc = encode_map(h, &h->tmap_in, in, h->M, elt == 1 ? xtc::Cfg<1>::kKStage : xtc::Cfg<2>::kKStage);
-    if (rc == CORR_OK)
-        rc = encode_map3(h, &h->tmap_pair, in, h->M, (elt == 1 ? xtc::kPairStageK<1> : xtc::kPairStageK<2>) / xtc::kPairBoxes, n_dump);
-    if (rc == CORR_OK) { h->tmap_in_ptr = in; h->tmap_dumps = n_dump; }
-    return rc;
-}
-
-int encode_input_map_b(corr_plan* h, const void* in_b) {
-    if (h->tmap_b_ptr == in_b) return CORR_OK;
-    h->tmap_b_ptr = nullptr;
-    h->tmap_dumps = 1;
-    const int elt = h->sample_bytes / 2;
-    const int rc = encode_map3(h, &h->tmap_b, in_b, h->Mb, (elt == 1 ? xtc::kPairStageK<1> : xtc::kPairStageK<2>) / xtc::kPairBoxes, 1);
-    if (rc == CORR_OK) h->tmap_b_ptr = in_b;
-    return rc;
-}
-
-int launch_direct(corr_plan* h, const void* in, void* out, int accumulate, cudaStream_t st) {
-    int rc = encode_input_map(h, in);
-    if (rc != CORR_OK) return rc;
-    xtc::Params prm;
-    prm.tiles = h->d_tiles;
-    prm.tiles_per_chan = static_cast<int>(h->h_tiles.size());
-    prm.n_tiles = static_cast<long long>(h->h_tiles.size()) * h->C;
+void fill_params(const corr_plan* h, const View& v, void* out, int accumulate, int n_dump, xtc::Params& prm) {
+    prm.tiles = nullptr;
+    prm.tiles_per_chan = 0;
+    prm.n_tiles = 0;
     prm.n_station = h->N;
     prm.n_pol = h->P;
-    prm.n_chan = h->C;
-    prm.n_time = h->T;
+    prm.n_chan = v.n_chan;
+    prm.n_time = v.n_time;
+    prm.n_dump = n_dump;
     prm.M = h->M;
     prm.n_baseline = h->B;
-    prm.n_station_b = 0;
-    prm.M_b = 0;
-    prm.n_dump = 1;
+    prm.n_station_b = h->Nb;
+    prm.M_b = h->Mb;
     prm.out = out;
     prm.accumulate = accumulate ? 1 : 0;
     // samples per TMEM accumulation pass: everything for int32 (exact); 1024 for fp32 (see xengine_tc.cuh)
-    prm.k_chunk = h->dtype == CORR_CI8 ? (1 << 30) : xtc::kFloatChunk;      // int32 sums are exact: one pass
+    prm.k_chunk = h->dtype == CORR_CI8 ? (1 << 30) : xtc::kFloatChunk;
+    prm.chan0 = v.chan0_in;
+    prm.chan0_out = v.chan0_out;
+    prm.n_chan_total = v.c_total_out;
+    prm.n_stages = prm.stage_bytes = prm.b_chunks = 0;
+}
+
+int launch_direct(corr_plan* h, const View& v, const void* in, void* out, int accumulate, cudaStream_t st) {
+    const CUtensorMap* map = nullptr;
+    const int rc = get_map(h, in, h->M, v.c_total_in, v.n_time, 1,
+                           h->dtype == CORR_CI8 ? xtc::Cfg<1>::kKStage : xtc::Cfg<2>::kKStage, &map);
+    if (rc != CORR_OK) return rc;
+    xtc::Params prm;
+    fill_params(h, v, out, accumulate, 1, prm);
+    prm.tiles = h->d_tiles;
+    prm.tiles_per_chan = static_cast<int>(h->h_tiles.size());
+    prm.n_tiles = static_cast<long long>(h->h_tiles.size()) * v.n_chan;
     {   // operand ring geometry: widest B of any tile, plus separate A chunks only if some tile is off the diagonal
         const int chunk_elems = h->dtype == CORR_CI8 ? 128 : 64;
         const int chunk_bytes = 128 * (h->dtype == CORR_CI8 ? xtc::Cfg<1>::kKStage : xtc::Cfg<2>::kKStage);
@@ -277,97 +264,61 @@ int launch_direct(corr_plan* h, const void* in, void* out, int accumulate, cudaS
     }
     const long long grid = prm.n_tiles < h->sm_count ? prm.n_tiles : h->sm_count;
     if (h->dtype == CORR_CI8)
-        xtc::xengine_direct_kernel<1><<<static_cast<unsigned>(grid), xtc::kNumThreads, xtc::kSmemBytes, st>>>(h->tmap_in, prm);
+        xtc::xengine_direct_kernel<1><<<static_cast<unsigned>(grid), xtc::kNumThreads, xtc::kSmemBytes, st>>>(*map, prm);
     else
-        xtc::xengine_direct_kernel<2><<<static_cast<unsigned>(grid), xtc::kNumThreads, xtc::kSmemBytes, st>>>(h->tmap_in, prm);
+        xtc::xengine_direct_kernel<2><<<static_cast<unsigned>(grid), xtc::kNumThreads, xtc::kSmemBytes, st>>>(*map, prm);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail_cuda(h, e, "xengine_direct_kernel launch");
     h->last_launches += 1;
     return CORR_OK;
 }
 
-template <int kElt, int kPairs>
+template <int kElt>
 cudaError_t launch_pair_kernel(const CUtensorMap& tmap, const CUtensorMap& tmap_b, const xtc::PairParams& pp, unsigned clusters,
                                cudaStream_t st) {
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(clusters * 2 * kPairs);
+    cfg.gridDim = dim3(clusters * 2);
     cfg.blockDim = dim3(xtc::kNumThreads);
     cfg.dynamicSmemBytes = xtc::kPairSmemBytes;
     cfg.stream = st;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeClusterDimension;
-    at[0].val.clusterDim.x = 2 * kPairs;
+    at[0].val.clusterDim.x = 2;
     at[0].val.clusterDim.y = 1;
     at[0].val.clusterDim.z = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, xtc::xengine_pair_kernel<kElt, kPairs>, tmap, tmap_b, pp);
+    return cudaLaunchKernelEx(&cfg, xtc::xengine_pair_kernel<kElt>, tmap, tmap_b, pp);
 }
 
-int launch_pair(corr_plan* h, const void* in, const void* in_b, void* out, int accumulate, cudaStream_t st,
-                int pairs_per_cluster, int n_dump = 1) {
-    int rc = encode_input_map(h, in, n_dump);
-    if (rc == CORR_OK && h->Nb) rc = encode_input_map_b(h, in_b);
+int launch_pair(corr_plan* h, const View& v, const void* in, const void* in_b, void* out, int accumulate, cudaStream_t st,
+                int n_dump = 1) {
+    const int box_rows = (h->dtype == CORR_CI8 ? xtc::kPairStageK<1> : xtc::kPairStageK<2>) / xtc::kPairBoxes;
+    const CUtensorMap* map_a = nullptr;
+    const CUtensorMap* map_b = nullptr;
+    int rc = get_map(h, in, h->M, v.c_total_in, v.n_time, n_dump, box_rows, &map_a);
+    if (rc == CORR_OK && h->Nb) rc = get_map(h, in_b, h->Mb, v.c_total_in, v.n_time, 1, box_rows, &map_b);
     if (rc != CORR_OK) return rc;
-    const CUtensorMap& map_b = h->Nb ? h->tmap_b : h->tmap_pair;
-    const int v = pairs_per_cluster - 1;
+    if (!h->Nb) map_b = map_a;
     xtc::PairParams pp;
-    pp.base.tiles = nullptr;
-    pp.base.tiles_per_chan = 0;
-    pp.base.n_tiles = 0;
-    pp.base.n_station = h->N;
-    pp.base.n_pol = h->P;
-    pp.base.n_chan = h->C;
-    pp.base.n_time = h->T / n_dump;
-    pp.base.n_dump = n_dump;
-    pp.base.M = h->M;
-    pp.base.n_baseline = h->B;
-    pp.base.n_station_b = h->Nb;
-    pp.base.M_b = h->Mb;
-    pp.base.out = out;
-    pp.base.accumulate = accumulate ? 1 : 0;
-    pp.base.k_chunk = h->dtype == CORR_CI8 ? (1 << 30) : xtc::kFloatChunk;      // int32 sums are exact: one pass
-#ifdef CORR_STATS
-    static unsigned long long* d_stats = nullptr;
-    if (!d_stats) cudaMalloc(&d_stats, 8 * 160 * sizeof(unsigned long long));
-    cudaMemsetAsync(d_stats, 0, 8 * 160 * sizeof(unsigned long long), st);
-    pp.base.stats = d_stats;
-#endif
-    pp.groups = h->d_groups[v];
-    pp.groups_per_chan = static_cast<int>(h->h_groups[v].size());
-    pp.n_groups = static_cast<long long>(pp.groups_per_chan) * h->C * n_dump;
-    const unsigned clusters = static_cast<unsigned>(pp.n_groups < h->max_clusters[v] ? pp.n_groups : h->max_clusters[v]);
-    if (pp.n_groups > (1ll << 31) - 4096) return fail(h, CORR_EINVAL, "xengine_pair_kernel: %lld tiles exceed the tile feed's range", pp.n_groups);
+    fill_params(h, v, out, accumulate, n_dump, pp.base);
+    pp.tiles = h->d_pair_tiles;
+    pp.tiles_per_chan = static_cast<int>(h->h_pair_tiles.size());
+    pp.n_tiles = static_cast<long long>(pp.tiles_per_chan) * v.n_chan * n_dump;
+    if (pp.n_tiles > (1ll << 31) - 4096)
+        return fail(h, CORR_EINVAL, "xengine_pair_kernel: %lld tiles exceed the tile feed's range", pp.n_tiles);
+    const unsigned clusters = static_cast<unsigned>(pp.n_tiles < h->max_clusters ? pp.n_tiles : h->max_clusters);
     pp.sched_counter = h->d_sched + (h->sched_seq++ % kSchedRing);
     cudaError_t e = cudaMemsetAsync(pp.sched_counter, 0, sizeof(unsigned int), st);
     if (e != cudaSuccess) return fail_cuda(h, e, "tile-feed counter reset");
-    if (h->dtype == CORR_CI8)
-        e = v ? launch_pair_kernel<1, 2>(h->tmap_pair, map_b, pp, clusters, st) : launch_pair_kernel<1, 1>(h->tmap_pair, map_b, pp, clusters, st);
-    else
-        e = v ? launch_pair_kernel<2, 2>(h->tmap_pair, map_b, pp, clusters, st) : launch_pair_kernel<2, 1>(h->tmap_pair, map_b, pp, clusters, st);
+    e = h->dtype == CORR_CI8 ? launch_pair_kernel<1>(*map_a, *map_b, pp, clusters, st)
+                             : launch_pair_kernel<2>(*map_a, *map_b, pp, clusters, st);
     if (e != cudaSuccess) return fail_cuda(h, e, "xengine_pair_kernel launch");
-#ifdef CORR_STATS
-    if (getenv("CORR_STATS_PRINT")) {
-        static unsigned long long hs[8 * 160];
-        cudaStreamSynchronize(st);
-        cudaMemcpy(hs, d_stats, sizeof(hs), cudaMemcpyDeviceToHost);
-        const int nb = static_cast<int>(clusters) * 2 * pairs_per_cluster;
-        double a[8] = {0};
-        for (int b = 0; b < nb; ++b) for (int k = 0; k < 8; ++k) a[k] += static_cast<double>(hs[b * 8 + k]) / nb;
-        double lead_tempty = 0, lead_full = 0;
-        for (int b = 0; b < nb; b += 2) { lead_tempty += hs[b * 8 + 2] / (nb / 2.0); lead_full += hs[b * 8 + 3] / (nb / 2.0); }
-        double tmin = 1e30, tmax = 0;
-        for (int b = 0; b < nb; ++b) { if (hs[b * 8] < tmin) tmin = hs[b * 8]; if (hs[b * 8] > tmax) tmax = hs[b * 8]; }
-        fprintf(stderr, "[corr stats] producer loop clk: min %.0f max %.0f (spread %.1f %%)\n", tmin, tmax, 100.0 * (tmax - tmin) / tmax);
-        fprintf(stderr, "[corr stats] clk/CTA: total %.0f | producer wait empty %.0f | mma wait tmem-empty %.0f, wait full %.0f | epi(warp2) wait tmem-full %.0f, drain %.0f\n",
-                a[0], a[1], lead_tempty, lead_full, a[4], a[5]);
-    }
-#endif
     h->last_launches += 1;
     return CORR_OK;
 }
 
-int launch_simt(corr_plan* h, const void* in, const void* in_b, void* out, int accumulate, cudaStream_t st) {
+int launch_simt(corr_plan* h, const View& v, const void* in, const void* in_b, void* out, int accumulate, cudaStream_t st) {
     xsimt::Params prm;
     prm.in = in;
     prm.in_b = in_b;
@@ -375,11 +326,14 @@ int launch_simt(corr_plan* h, const void* in, const void* in_b, void* out, int a
     prm.out = out;
     prm.n_station = h->N;
     prm.n_pol = h->P;
-    prm.n_chan = h->C;
-    prm.n_time = h->T;
+    prm.n_chan = v.n_chan;
+    prm.n_time = v.n_time;
     prm.n_baseline = h->B;
-    prm.n_vis = static_cast<long long>(h->C) * h->B * h->P * h->P;
+    prm.n_vis = static_cast<long long>(v.n_chan) * h->B * h->P * h->P;
     prm.accumulate = accumulate ? 1 : 0;
+    prm.chan0 = v.chan0_in;
+    prm.n_chan_total = v.c_total_in;
+    prm.chan0_out = v.chan0_out;
     long long blocks = (prm.n_vis + 127) / 128;
     const long long cap = static_cast<long long>(h->sm_count) * 16;
     if (blocks > cap) blocks = cap;
@@ -415,6 +369,15 @@ int launch_corner_turn(corr_plan* h, const void* in, void* ws, cudaStream_t st) 
     return CORR_OK;
 }
 
+// One X-engine launch on a view, on whichever kernel the plan resolves to.
+int launch_xengine(corr_plan* h, const View& v, const void* in, const void* in_b, void* out, int accumulate, cudaStream_t st) {
+    switch (resolve_kernel(h)) {
+        case CORR_KERNEL_PAIR: return launch_pair(h, v, in, in_b, out, accumulate, st);
+        case CORR_KERNEL_SINGLE: return launch_direct(h, v, in, out, accumulate, st);
+        default: return launch_simt(h, v, in, in_b, out, accumulate, st);
+    }
+}
+
 }  // namespace
 
 extern "C" {
@@ -431,15 +394,10 @@ int corr_tile_schedule(int n_station, int n_pol, int dtype, int kernel, int* til
         std::vector<xtc::TileDesc> v;
         build_schedule_direct(n_station, n_pol, v);
         for (const xtc::TileDesc& t : v) { flat.push_back(t.row0); flat.push_back(t.col0); flat.push_back(t.ncols); }
-    } else if (kernel == CORR_KERNEL_PAIR || kernel == CORR_KERNEL_QUAD) {
-        std::vector<xtc::PairGroup> g;
-        build_groups(n_station, n_pol, kernel == CORR_KERNEL_QUAD ? 2 : 1, g);
-        for (const xtc::PairGroup& x : g)
-            for (int k = 0; k < (kernel == CORR_KERNEL_QUAD ? 2 : 1); ++k) {
-                flat.push_back(x.t[k].row0);
-                flat.push_back(x.t[k].col0);
-                flat.push_back(k == 1 && x.share == 3 ? 0 : xtc::kTileCols);     // 0: duplicate, computed but not written
-            }
+    } else if (kernel == CORR_KERNEL_PAIR) {
+        std::vector<xtc::PairTile> v;
+        build_pair_tiles(n_station, n_pol, v);
+        for (const xtc::PairTile& t : v) { flat.push_back(t.row0); flat.push_back(t.col0); flat.push_back(xtc::kTileCols); }
     } else {
         return CORR_EINVAL;
     }
@@ -449,16 +407,18 @@ int corr_tile_schedule(int n_station, int n_pol, int dtype, int kernel, int* til
     return n;
 }
 
-static corr_handle create_plan(int n_station, int n_station_b, int n_pol, int n_chan, int n_time, int dtype) {
+static corr_handle create_plan(int n_station, int n_station_b, int n_pol, int n_chan_total, int chan0, int n_chan, int n_time,
+                               int dtype) {
     g_create_error[0] = 0;
-    if (!valid_geometry(n_station, n_pol, dtype) || n_station_b < 0 || n_chan < 1 || n_time < 1) {
-        fail(nullptr, CORR_EINVAL, "corr_create: invalid geometry N=%d Nb=%d P=%d C=%d T=%d dtype=%d", n_station, n_station_b,
-             n_pol, n_chan, n_time, dtype);
+    if (!valid_geometry(n_station, n_pol, dtype) || n_station_b < 0 || n_chan < 1 || n_time < 1 || chan0 < 0 ||
+        n_chan_total < 1 || static_cast<long long>(chan0) + n_chan > n_chan_total) {
+        fail(nullptr, CORR_EINVAL, "corr_create: invalid geometry N=%d Nb=%d P=%d C=%d (window %d..+%d) T=%d dtype=%d", n_station,
+             n_station_b, n_pol, n_chan_total, chan0, n_chan, n_time, dtype);
         return nullptr;
     }
     const long long M = static_cast<long long>(n_station) * n_pol;
     const long long Mb = static_cast<long long>(n_station_b) * n_pol;
-    const long long W = static_cast<long long>(n_chan) * 2 * (M > Mb ? M : Mb);
+    const long long W = static_cast<long long>(n_chan_total) * 2 * (M > Mb ? M : Mb);
     if (M > (1 << 20) || Mb > (1 << 20) || W > (1ll << 31) - 1024 || n_time > (1 << 24)) {
         fail(nullptr, CORR_EINVAL, "corr_create: geometry too large (N*P=%lld, C*2*N*P=%lld, T=%d)", M, W, n_time);
         return nullptr;
@@ -475,7 +435,7 @@ static corr_handle create_plan(int n_station, int n_station_b, int n_pol, int n_
         fail(nullptr, CORR_EUNSUPPORTED, "corr_create: cudaGetDeviceProperties: %s", cudaGetErrorString(e));
         return nullptr;
     }
-    if (prop.major != 10) {
+    if (prop.major != 10 || prop.minor != 0) {       // the library carries sm_100a SASS only (no PTX): B200 / GB200
         fail(nullptr, CORR_EUNSUPPORTED, "corr_create: device %d (%s) is sm_%d%d; this library is built for sm_100a only",
              dev, prop.name, prop.major, prop.minor);
         return nullptr;
@@ -488,6 +448,8 @@ static corr_handle create_plan(int n_station, int n_station_b, int n_pol, int n_
     h->N = n_station;
     h->P = n_pol;
     h->C = n_chan;
+    h->C_total = n_chan_total;
+    h->chan0 = chan0;
     h->T = n_time;
     h->dtype = dtype;
     h->M = static_cast<int>(M);
@@ -499,21 +461,22 @@ static corr_handle create_plan(int n_station, int n_station_b, int n_pol, int n_
     h->device = dev;
     h->sm_count = prop.multiProcessorCount;
     h->tma_ok = (M * h->sample_bytes) % 16 == 0 && (Mb * h->sample_bytes) % 16 == 0;
-    h->tmap_b_ptr = nullptr;
     h->t_total = 0;
     h->last_launches = 0;
     h->d_tiles = nullptr;
+    h->d_pair_tiles = nullptr;
     h->kernel = CORR_KERNEL_AUTO;
-    h->d_groups[0] = h->d_groups[1] = nullptr;
     h->d_sched = nullptr;
     h->sched_seq = 0;
-    h->max_clusters[0] = h->max_clusters[1] = 0;
+    h->max_clusters = 0;
     h->encode = nullptr;
-    h->tmap_in_ptr = nullptr;
+    for (int k = 0; k < kMapCache; ++k) h->map_used[k] = 0;
+    h->map_clock = 0;
     h->Tp = (n_time + 63) / 64 * 64;
-    h->d_in_stage = nullptr;
+    h->d_in_stage[0] = h->d_in_stage[1] = nullptr;
     h->d_out_stage = nullptr;
-    h->own_stream = nullptr;
+    h->st_h2d = h->st_run = h->st_d2h = nullptr;
+    h->ev_h2d[0] = h->ev_h2d[1] = h->ev_run[0] = h->ev_run[1] = nullptr;
     h->err[0] = 0;
 
     build_schedule_direct(h->N, h->P, h->h_tiles);
@@ -551,33 +514,29 @@ static corr_handle create_plan(int n_station, int n_station_b, int n_pol, int n_
             corr_destroy(h);
             return nullptr;
         }
-        // CTA-pair kernels: group tables and the number of co-resident clusters (the persistent grid)
-        for (int v = 0; v < (h->Nb ? 1 : 2) && e == cudaSuccess; ++v) {
-            if (h->Nb) build_groups_rect(h->N, h->Nb, h->P, h->h_groups[v]);
-            else build_groups(h->N, h->P, v + 1, h->h_groups[v]);
-            const size_t bytes = h->h_groups[v].size() * sizeof(xtc::PairGroup);
-            e = cudaMalloc(&h->d_groups[v], bytes);
-            if (e == cudaSuccess) e = cudaMemcpy(h->d_groups[v], h->h_groups[v].data(), bytes, cudaMemcpyHostToDevice);
-            const void* fn_ptr = h->dtype == CORR_CI8
-                                     ? (v ? (const void*)xtc::xengine_pair_kernel<1, 2> : (const void*)xtc::xengine_pair_kernel<1, 1>)
-                                     : (v ? (const void*)xtc::xengine_pair_kernel<2, 2> : (const void*)xtc::xengine_pair_kernel<2, 1>);
-            if (e == cudaSuccess) e = cudaFuncSetAttribute(fn_ptr, cudaFuncAttributeMaxDynamicSharedMemorySize, xtc::kPairSmemBytes);
-            if (e == cudaSuccess) {
-                cudaLaunchConfig_t cfg = {};
-                cfg.gridDim = dim3(static_cast<unsigned>(h->sm_count / (2 * (v + 1)) * (2 * (v + 1))));
-                cfg.blockDim = dim3(xtc::kNumThreads);
-                cfg.dynamicSmemBytes = xtc::kPairSmemBytes;
-                cudaLaunchAttribute at[1];
-                at[0].id = cudaLaunchAttributeClusterDimension;
-                at[0].val.clusterDim.x = 2 * (v + 1);
-                at[0].val.clusterDim.y = 1;
-                at[0].val.clusterDim.z = 1;
-                cfg.attrs = at;
-                cfg.numAttrs = 1;
-                int n = 0;
-                if (cudaOccupancyMaxActiveClusters(&n, fn_ptr, &cfg) == cudaSuccess) h->max_clusters[v] = n;
-                else cudaGetLastError();          // pair kernels unavailable: resolve_kernel falls back
-            }
+        // CTA-pair kernel: tile table and the number of co-resident pairs (the persistent grid)
+        if (h->Nb) build_pair_tiles_rect(h->N, h->Nb, h->P, h->h_pair_tiles);
+        else build_pair_tiles(h->N, h->P, h->h_pair_tiles);
+        const size_t bytes = h->h_pair_tiles.size() * sizeof(xtc::PairTile);
+        e = cudaMalloc(&h->d_pair_tiles, bytes);
+        if (e == cudaSuccess) e = cudaMemcpy(h->d_pair_tiles, h->h_pair_tiles.data(), bytes, cudaMemcpyHostToDevice);
+        const void* fn_ptr = h->dtype == CORR_CI8 ? (const void*)xtc::xengine_pair_kernel<1> : (const void*)xtc::xengine_pair_kernel<2>;
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(fn_ptr, cudaFuncAttributeMaxDynamicSharedMemorySize, xtc::kPairSmemBytes);
+        if (e == cudaSuccess) {
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3(static_cast<unsigned>(h->sm_count / 2 * 2));
+            cfg.blockDim = dim3(xtc::kNumThreads);
+            cfg.dynamicSmemBytes = xtc::kPairSmemBytes;
+            cudaLaunchAttribute at[1];
+            at[0].id = cudaLaunchAttributeClusterDimension;
+            at[0].val.clusterDim.x = 2;
+            at[0].val.clusterDim.y = 1;
+            at[0].val.clusterDim.z = 1;
+            cfg.attrs = at;
+            cfg.numAttrs = 1;
+            int n = 0;
+            if (cudaOccupancyMaxActiveClusters(&n, fn_ptr, &cfg) == cudaSuccess) h->max_clusters = n;
+            else cudaGetLastError();          // pair kernel unavailable: resolve_kernel falls back
         }
         if (e != cudaSuccess) {
             fail(nullptr, e == cudaErrorMemoryAllocation ? CORR_ENOMEM : CORR_ECUDA, "corr_create: pair kernel setup: %s",
@@ -590,7 +549,11 @@ static corr_handle create_plan(int n_station, int n_station_b, int n_pol, int n_
 }
 
 corr_handle corr_create(int n_station, int n_pol, int n_chan, int n_time, int dtype) {
-    return create_plan(n_station, 0, n_pol, n_chan, n_time, dtype);
+    return create_plan(n_station, 0, n_pol, n_chan, 0, n_chan, n_time, dtype);
+}
+
+corr_handle corr_create_window(int n_station, int n_pol, int n_chan_total, int chan0, int n_chan, int n_time, int dtype) {
+    return create_plan(n_station, 0, n_pol, n_chan_total, chan0, n_chan, n_time, dtype);
 }
 
 corr_handle corr_create_cross(int n_station_a, int n_station_b, int n_pol, int n_chan, int n_time, int dtype) {
@@ -599,18 +562,23 @@ corr_handle corr_create_cross(int n_station_a, int n_station_b, int n_pol, int n
         fail(nullptr, CORR_EINVAL, "corr_create_cross: invalid geometry Na=%d Nb=%d", n_station_a, n_station_b);
         return nullptr;
     }
-    return create_plan(n_station_a, n_station_b, n_pol, n_chan, n_time, dtype);
+    return create_plan(n_station_a, n_station_b, n_pol, n_chan, 0, n_chan, n_time, dtype);
 }
 
 void corr_destroy(corr_handle h) {
     if (!h) return;
     if (h->d_tiles) cudaFree(h->d_tiles);
     if (h->d_sched) cudaFree(h->d_sched);
-    if (h->d_groups[0]) cudaFree(h->d_groups[0]);
-    if (h->d_groups[1]) cudaFree(h->d_groups[1]);
-    if (h->d_in_stage) cudaFree(h->d_in_stage);
+    if (h->d_pair_tiles) cudaFree(h->d_pair_tiles);
+    for (int k = 0; k < 2; ++k) {
+        if (h->d_in_stage[k]) cudaFree(h->d_in_stage[k]);
+        if (h->ev_h2d[k]) cudaEventDestroy(h->ev_h2d[k]);
+        if (h->ev_run[k]) cudaEventDestroy(h->ev_run[k]);
+    }
     if (h->d_out_stage) cudaFree(h->d_out_stage);
-    if (h->own_stream) cudaStreamDestroy(h->own_stream);
+    if (h->st_h2d) cudaStreamDestroy(h->st_h2d);
+    if (h->st_run) cudaStreamDestroy(h->st_run);
+    if (h->st_d2h) cudaStreamDestroy(h->st_d2h);
     delete h;
 }
 
@@ -629,10 +597,10 @@ int corr_set_kernel(corr_handle h, int kernel) {
     if (kernel != CORR_KERNEL_AUTO && kernel != CORR_KERNEL_SIMT && !h->tma_ok)
         return fail(h, CORR_EUNSUPPORTED, "corr_set_kernel: per-channel row of %lld B is not a multiple of 16, only the SIMT kernel applies",
                     static_cast<long long>(h->M) * h->sample_bytes);
-    if (h->Nb && (kernel == CORR_KERNEL_SINGLE || kernel == CORR_KERNEL_QUAD))
+    if (h->Nb && kernel == CORR_KERNEL_SINGLE)
         return fail(h, CORR_EUNSUPPORTED, "corr_set_kernel: cross plans run on the PAIR or the SIMT kernel");
-    if ((kernel == CORR_KERNEL_PAIR && h->max_clusters[0] <= 0) || (kernel == CORR_KERNEL_QUAD && h->max_clusters[1] <= 0))
-        return fail(h, CORR_EUNSUPPORTED, "corr_set_kernel: no co-resident clusters for kernel %d on this device", kernel);
+    if (kernel == CORR_KERNEL_PAIR && h->max_clusters <= 0)
+        return fail(h, CORR_EUNSUPPORTED, "corr_set_kernel: no co-resident CTA pairs for the PAIR kernel on this device");
     h->kernel = kernel;
     return CORR_OK;
 }
@@ -671,7 +639,7 @@ int corr_fengine_ci8(const void* in, void* out, int n_stream, long long n_spectr
 
 int corr_corner_turn(corr_handle h, const void* in, void* ws, void* stream) {
     if (!h) return CORR_EINVAL;
-    if (h->Nb) return fail(h, CORR_EINVAL, "corr_corner_turn: not available on cross plans");
+    if (h->Nb || h->C != h->C_total) return fail(h, CORR_EINVAL, "corr_corner_turn: not available on cross or window plans");
     if (!in || !ws) return fail(h, CORR_EINVAL, "corr_corner_turn: NULL pointer");
     if ((reinterpret_cast<uintptr_t>(in) & 15) || (reinterpret_cast<uintptr_t>(ws) & 127))
         return fail(h, CORR_EINVAL, "corr_corner_turn: `in` must be 16-byte and `ws` 128-byte aligned");
@@ -682,7 +650,19 @@ int corr_corner_turn(corr_handle h, const void* in, void* ws, void* stream) {
     return launch_corner_turn(h, in, ws, static_cast<cudaStream_t>(stream));
 }
 
-static int run_xengine(corr_handle h, const void* in, const void* in_b, void* out, int accumulate, void* stream);
+static int run_xengine(corr_handle h, const void* in, const void* in_b, void* out, int accumulate, void* stream) {
+    if (!in || !out) return fail(h, CORR_EINVAL, "corr_xengine: NULL pointer");
+    if ((reinterpret_cast<uintptr_t>(in) & 15) || (reinterpret_cast<uintptr_t>(out) & 15))
+        return fail(h, CORR_EINVAL, "corr_xengine: `in` and `out` must be 16-byte aligned");
+    const long long t_next = accumulate ? h->t_total + h->T : h->T;
+    if (h->dtype == CORR_CI8 && t_next > kMaxIntegrationCi8)
+        return fail(h, CORR_EOVERFLOW, "corr_xengine: integrating %lld samples would overflow int32 (limit %lld)", t_next,
+                    kMaxIntegrationCi8);
+    h->last_launches = 0;
+    const int rc = launch_xengine(h, device_view(h), in, in_b, out, accumulate, static_cast<cudaStream_t>(stream));
+    if (rc == CORR_OK) h->t_total = t_next;
+    return rc;
+}
 
 int corr_xengine(corr_handle h, const void* in, void* out, int accumulate, void* stream) {
     if (!h) return CORR_EINVAL;
@@ -702,19 +682,16 @@ int corr_xengine_dumps(corr_handle h, const void* in, void* out, int n_dump, voi
     if (h->dtype == CORR_CI8 && Ts > kMaxIntegrationCi8)
         return fail(h, CORR_EOVERFLOW, "corr_xengine_dumps: integrating %d samples would overflow int32", Ts);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    h->last_launches = 0;
-    h->t_total = Ts;
-    const int kernel = resolve_kernel(h);
-    if (kernel != CORR_KERNEL_SIMT && h->max_clusters[0] > 0)
-        return launch_pair(h, in, nullptr, out, 0, st, 1, n_dump);       // any TMA-addressable geometry runs on the pair kernel
+    h->last_launches = 0;       // (the running-integration count t_total of corr_xengine is not touched: dumps never accumulate)
+    View v = device_view(h);
+    v.n_time = Ts;
+    if (resolve_kernel(h) != CORR_KERNEL_SIMT && h->max_clusters > 0)
+        return launch_pair(h, v, in, nullptr, out, 0, st, n_dump);        // any TMA-addressable geometry runs on the pair kernel
     // SIMT: one launch per integration on slices of `in` and `out`
-    const int T_full = h->T;
     int rc = CORR_OK;
-    h->T = Ts;
     for (int d = 0; d < n_dump && rc == CORR_OK; ++d)
-        rc = launch_simt(h, static_cast<const uint8_t*>(in) + d * input_bytes(h), nullptr,
+        rc = launch_simt(h, v, static_cast<const uint8_t*>(in) + d * (input_bytes(h) / n_dump), nullptr,
                          static_cast<uint8_t*>(out) + d * output_bytes(h), 0, st);
-    h->T = T_full;
     return rc;
 }
 
@@ -726,55 +703,80 @@ int corr_xengine_cross(corr_handle h, const void* in_a, const void* in_b, void* 
     return run_xengine(h, in_a, in_b, out, accumulate, stream);
 }
 
-static int run_xengine(corr_handle h, const void* in, const void* in_b, void* out, int accumulate, void* stream) {
-    if (!in || !out) return fail(h, CORR_EINVAL, "corr_xengine: NULL pointer");
-    if ((reinterpret_cast<uintptr_t>(in) & 15) || (reinterpret_cast<uintptr_t>(out) & 15))
-        return fail(h, CORR_EINVAL, "corr_xengine: `in` and `out` must be 16-byte aligned");
-    const long long t_next = accumulate ? h->t_total + h->T : h->T;
-    if (h->dtype == CORR_CI8 && t_next > kMaxIntegrationCi8)
-        return fail(h, CORR_EOVERFLOW, "corr_xengine: integrating %lld samples would overflow int32 (limit %lld)", t_next,
-                    kMaxIntegrationCi8);
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    h->last_launches = 0;
-    int rc;
-    switch (resolve_kernel(h)) {
-        case CORR_KERNEL_QUAD: rc = launch_pair(h, in, in_b, out, accumulate, st, 2); break;
-        case CORR_KERNEL_PAIR: rc = launch_pair(h, in, in_b, out, accumulate, st, 1); break;
-        case CORR_KERNEL_SINGLE: rc = launch_direct(h, in, out, accumulate, st); break;
-        default: rc = launch_simt(h, in, in_b, out, accumulate, st); break;
-    }
-    if (rc == CORR_OK) h->t_total = t_next;
-    return rc;
-}
-
+// Host-buffer entry point: the plan's channels are cut into up to kHostWindows windows that flow through a three-stage
+// pipeline on three streams -- H2D of window w+1 (a strided 2-D copy straight out of the caller's [T][C][M] buffer into
+// one of two compact staging slots), the X-engine on window w (reading the slot, writing its slab of the device-resident
+// running sum), D2H of window w-1's slab -- so the PCIe link runs in both directions while the kernel computes.
 int corr_xengine_host(corr_handle h, const void* in_host, void* out_host, int accumulate) {
     if (!h) return CORR_EINVAL;
     if (h->Nb) return fail(h, CORR_EINVAL, "corr_xengine_host: not available on cross plans");
     if (!in_host) return fail(h, CORR_EINVAL, "corr_xengine_host: NULL input pointer");
-    cudaError_t e;
-    if (!h->own_stream) {
-        e = cudaStreamCreateWithFlags(&h->own_stream, cudaStreamNonBlocking);
-        if (e != cudaSuccess) return fail_cuda(h, e, "cudaStreamCreate");
+    const long long t_next = accumulate ? h->t_total + h->T : h->T;
+    if (h->dtype == CORR_CI8 && t_next > kMaxIntegrationCi8)
+        return fail(h, CORR_EOVERFLOW, "corr_xengine_host: integrating %lld samples would overflow int32 (limit %lld)", t_next,
+                    kMaxIntegrationCi8);
+    cudaError_t e = cudaSuccess;
+    const int n_win = h->C < kHostWindows ? h->C : kHostWindows;
+    const int win_max = (h->C + n_win - 1) / n_win;
+    const size_t chan_in_bytes = static_cast<size_t>(h->M) * h->sample_bytes;             // one channel of one time sample
+    const size_t chan_out_bytes = static_cast<size_t>(h->B) * h->P * h->P * 8;            // one channel's visibilities
+    if (!h->st_h2d) {
+        e = cudaStreamCreateWithFlags(&h->st_h2d, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&h->st_run, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&h->st_d2h, cudaStreamNonBlocking);
+        for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
+            e = cudaEventCreateWithFlags(&h->ev_h2d[k], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_run[k], cudaEventDisableTiming);
+        }
+        if (e != cudaSuccess) return fail_cuda(h, e, "corr_xengine_host: streams / events");
     }
-    if (!h->d_in_stage) {
-        e = cudaMalloc(&h->d_in_stage, input_bytes(h));
-        if (e != cudaSuccess) return fail(h, CORR_ENOMEM, "corr_xengine_host: input staging: %s", cudaGetErrorString(e));
-    }
+    for (int k = 0; k < 2; ++k)
+        if (!h->d_in_stage[k]) {
+            e = cudaMalloc(&h->d_in_stage[k], static_cast<size_t>(h->T) * win_max * chan_in_bytes);
+            if (e != cudaSuccess) return fail(h, CORR_ENOMEM, "corr_xengine_host: input staging: %s", cudaGetErrorString(e));
+        }
     if (!h->d_out_stage) {
         if (accumulate) return fail(h, CORR_EINVAL, "corr_xengine_host: accumulate without a previous call");
-        e = cudaMalloc(&h->d_out_stage, output_bytes(h));
+        e = cudaMalloc(&h->d_out_stage, static_cast<size_t>(h->C) * chan_out_bytes);
         if (e != cudaSuccess) return fail(h, CORR_ENOMEM, "corr_xengine_host: output staging: %s", cudaGetErrorString(e));
     }
-    e = cudaMemcpyAsync(h->d_in_stage, in_host, input_bytes(h), cudaMemcpyHostToDevice, h->own_stream);
-    if (e != cudaSuccess) return fail_cuda(h, e, "H2D copy");
-    const int rc = corr_xengine(h, h->d_in_stage, h->d_out_stage, accumulate, h->own_stream);
-    if (rc != CORR_OK) return rc;
-    if (out_host) {
-        e = cudaMemcpyAsync(out_host, h->d_out_stage, output_bytes(h), cudaMemcpyDeviceToHost, h->own_stream);
-        if (e != cudaSuccess) return fail_cuda(h, e, "D2H copy");
+    h->last_launches = 0;
+    const uint8_t* src = static_cast<const uint8_t*>(in_host);
+    uint8_t* dst = static_cast<uint8_t*>(out_host);
+    const int base = h->C / n_win, extra = h->C % n_win;
+    int c0 = 0;
+    for (int w = 0; w < n_win; ++w) {
+        const int wn = base + (w < extra ? 1 : 0);
+        const int slot = w & 1;
+        if (w >= 2) {                                     // the kernel of window w - 2 has finished reading this slot
+            e = cudaStreamWaitEvent(h->st_h2d, h->ev_run[slot], 0);
+            if (e != cudaSuccess) return fail_cuda(h, e, "corr_xengine_host: wait for the staging slot");
+        }
+        e = cudaMemcpy2DAsync(h->d_in_stage[slot], wn * chan_in_bytes, src + static_cast<size_t>(h->chan0 + c0) * chan_in_bytes,
+                              static_cast<size_t>(h->C_total) * chan_in_bytes, wn * chan_in_bytes, h->T, cudaMemcpyHostToDevice,
+                              h->st_h2d);
+        if (e == cudaSuccess) e = cudaEventRecord(h->ev_h2d[slot], h->st_h2d);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(h->st_run, h->ev_h2d[slot], 0);
+        if (e != cudaSuccess) return fail_cuda(h, e, "corr_xengine_host: H2D copy");
+        const View v{h->T, wn, wn, 0, h->C, c0};
+        const int rc = launch_xengine(h, v, h->d_in_stage[slot], nullptr, h->d_out_stage, accumulate, h->st_run);
+        if (rc != CORR_OK) return rc;
+        e = cudaEventRecord(h->ev_run[slot], h->st_run);
+        if (e == cudaSuccess && dst) {
+            e = cudaStreamWaitEvent(h->st_d2h, h->ev_run[slot], 0);
+            if (e == cudaSuccess)
+                e = cudaMemcpyAsync(dst + static_cast<size_t>(h->chan0 + c0) * chan_out_bytes,
+                                    static_cast<uint8_t*>(h->d_out_stage) + static_cast<size_t>(c0) * chan_out_bytes,
+                                    wn * chan_out_bytes, cudaMemcpyDeviceToHost, h->st_d2h);
+        }
+        if (e != cudaSuccess) return fail_cuda(h, e, "corr_xengine_host: D2H copy");
+        c0 += wn;
     }
-    e = cudaStreamSynchronize(h->own_stream);
+    e = cudaStreamSynchronize(h->st_run);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->st_d2h);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->st_h2d);
     if (e != cudaSuccess) return fail_cuda(h, e, "corr_xengine_host: stream synchronize");
+    h->t_total = t_next;
     return CORR_OK;
 }
 

@@ -37,14 +37,15 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
         : "memory");
     return ok != 0;
 }
-// Blocking wait.  A pipeline bug must surface as a launch failure, never as a hung GPU: after
-// ~2^31 SM clocks (about a second) without progress the kernel traps.
+// Blocking wait.  A pipeline bug must surface as a launch failure, never as a hung GPU: after 2^33 SM clocks
+// (4 - 7 s at 1.2 - 2 GHz; the longest legitimate wait is one tile, microseconds) without progress the kernel traps,
+// and the caller sees CORR_ECUDA (documented in corr.h: the context is then unusable, as after any device fault).
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     if (mbar_try_wait(bar, parity)) return;
     const long long t0 = clock64();
     uint32_t spins = 0;
     while (!mbar_try_wait(bar, parity)) {
-        if ((++spins & 0x3ffu) == 0 && clock64() - t0 > (1ll << 32)) __trap();
+        if ((++spins & 0x3ffu) == 0 && clock64() - t0 > (1ll << 33)) __trap();
     }
 }
 
@@ -52,14 +53,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 __device__ __forceinline__ void prefetch_tensormap(const CUtensorMap* map) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(map)) : "memory");
 }
-// 2-D tiled load global -> shared, completion on an mbarrier (complete_tx::bytes).
-__device__ __forceinline__ void tma_load_2d(uint32_t dst_smem, const CUtensorMap* map, uint32_t bar,
-                                            int c0, int c1) {
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
-        ::"r"(dst_smem), "l"(reinterpret_cast<uint64_t>(map)), "r"(bar), "r"(c0), "r"(c1)
-        : "memory");
-}
+// 3-D tiled load global -> shared, completion on an mbarrier (complete_tx::bytes).
 __device__ __forceinline__ void tma_load_3d(uint32_t dst_smem, const CUtensorMap* map, uint32_t bar,
                                             int c0, int c1, int c2) {
     asm volatile(
@@ -204,8 +198,6 @@ __device__ __forceinline__ uint32_t mapa(uint32_t addr, uint32_t rank) {
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
     asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
-// In a CTA pair the two CTAs' shared::cluster windows differ in one address bit; clearing it turns the
-// address of a barrier in this CTA into the address of the same barrier in the pair's even (leader) CTA.
 // ---- cluster-scope pieces of the dynamic tile feed (xengine_pair.cuh) ----------------------------------------
 __device__ __forceinline__ void st_shared_cluster_u32(uint32_t cluster_addr, uint32_t v) {
     asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(cluster_addr), "r"(v) : "memory");
@@ -238,42 +230,19 @@ __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity)
     const long long t0 = clock64();
     uint32_t spins = 0;
     while (!mbar_try_wait_cluster(bar, parity)) {
-        if ((++spins & 0x3ffu) == 0 && clock64() - t0 > (1ll << 32)) __trap();
+        if ((++spins & 0x3ffu) == 0 && clock64() - t0 > (1ll << 33)) __trap();
     }
 }
+// In a CTA pair the two CTAs' shared::cluster windows differ in one address bit; clearing it turns the
+// address of a barrier in this CTA into the address of the same barrier in the pair's even (leader) CTA.
 constexpr uint32_t kPeerBitMask = 0xFEFFFFFFu;
-// 2-D tiled load into THIS CTA's shared memory whose completion bytes are counted on the PAIR LEADER's mbarrier.
-__device__ __forceinline__ void tma_load_2d_pair(uint32_t dst_smem, const CUtensorMap* map, uint32_t bar,
-                                                 int c0, int c1) {
-    asm volatile(
-        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
-        ::"r"(dst_smem), "l"(reinterpret_cast<uint64_t>(map)), "r"(bar & kPeerBitMask), "r"(c0), "r"(c1)
-        : "memory");
-}
-// The same, delivered to the same offset of every CTA in `cta_mask` (bit k = cluster rank k); each destination
-// CTA's bytes are counted on ITS pair leader's mbarrier.
-__device__ __forceinline__ void tma_load_2d_pair_mc(uint32_t dst_smem, const CUtensorMap* map, uint32_t bar,
-                                                    int c0, int c1, uint16_t cta_mask) {
-    asm volatile(
-        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster"
-        " [%0], [%1, {%4, %5}], [%2], %3;"
-        ::"r"(dst_smem), "l"(reinterpret_cast<uint64_t>(map)), "r"(bar & kPeerBitMask), "h"(cta_mask), "r"(c0), "r"(c1)
-        : "memory");
-}
-// 3-D forms (coordinates: component column, time sample within the integration, integration index)
+// 3-D tiled load into THIS CTA's shared memory whose completion bytes are counted on the PAIR LEADER's mbarrier
+// (coordinates: component column, time sample within the integration, integration index)
 __device__ __forceinline__ void tma_load_3d_pair(uint32_t dst_smem, const CUtensorMap* map, uint32_t bar,
                                                  int c0, int c1, int c2) {
     asm volatile(
         "cp.async.bulk.tensor.3d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
         ::"r"(dst_smem), "l"(reinterpret_cast<uint64_t>(map)), "r"(bar & kPeerBitMask), "r"(c0), "r"(c1), "r"(c2)
-        : "memory");
-}
-__device__ __forceinline__ void tma_load_3d_pair_mc(uint32_t dst_smem, const CUtensorMap* map, uint32_t bar,
-                                                    int c0, int c1, int c2, uint16_t cta_mask) {
-    asm volatile(
-        "cp.async.bulk.tensor.3d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster"
-        " [%0], [%1, {%4, %5, %6}], [%2], %3;"
-        ::"r"(dst_smem), "l"(reinterpret_cast<uint64_t>(map)), "r"(bar & kPeerBitMask), "h"(cta_mask), "r"(c0), "r"(c1), "r"(c2)
         : "memory");
 }
 __device__ __forceinline__ void tmem_alloc_pair(uint32_t dst_smem, uint32_t ncols) {
@@ -306,7 +275,8 @@ __device__ __forceinline__ void mma_f16_pair(uint32_t d_tmem, uint64_t adesc, ui
         ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
         : "memory");
 }
-// Arrive on the mbarrier at this offset in every CTA of `cta_mask` once all MMAs issued so far have completed.
+// Arrive on the mbarrier at this offset in every CTA of `cta_mask` (bit k = cluster rank k) once all MMAs issued so far
+// have completed.
 __device__ __forceinline__ void mma_commit_pair_mc(uint32_t bar, uint16_t cta_mask) {
     asm volatile(
         "tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"

@@ -1,5 +1,5 @@
-// xengine_pair.cuh -- the X-engine HERK on CTA PAIRS (tcgen05 cta_group::2) with optional TMA multicast
-// between two pairs of a 4-CTA cluster.  Same mathematics and same direct feed as xengine_tc.cuh
+// xengine_pair.cuh -- the X-engine HERK on CTA PAIRS (tcgen05 cta_group::2).  Same mathematics and same direct feed
+// as xengine_tc.cuh
 // (Sec. 2 Eq. 2; lower station triangle incl. autocorrelations PAPER.md:79, 144).
 //
 // Why (profiles/r1a_cfg4_ncu_1cta_kernel.md): with 128 x 256 tiles per CTA every time sample costs
@@ -7,15 +7,15 @@
 // call = the L2 slice throughput cap; the tensor pipe idles 60 % of the time.  A CTA pair computes a
 // 256 x 256 tile of G with one M = 256 instruction: each CTA holds 128 rows of A and only HALF of B's
 // columns (the hardware feeds both halves to both tensor cores), so a sample costs 128 + 128 bytes per CTA
-// for the same 32768 MACs (and half the shared-memory operand reads).  Two pairs that work on tiles of one
-// channel sharing a column block (or a row block) form a 4-CTA cluster and fetch the shared operand ONCE
-// with a multicast TMA load: 128 + 64 bytes per CTA and sample.
+// for the same 32768 MACs (and half the shared-memory operand reads).  (A 4-CTA cluster of two pairs with a
+// multicast load of the operand their tiles share was built and measured in round 1: 12 % slower at config 4 --
+// the multicast saves L2 reads, not bytes delivered to each SM, and couples the two pipelines -- and removed.)
 //
 // Roles per CTA (320 threads, one CTA per SM, persistent; the tiles come from the dynamic TileFeed below):
 //   warp 0      TMA producer (one lane): its 128 A rows and its 128 B columns of every pipeline stage; completion
 //               bytes of both CTAs are counted on the pair LEADER's `full` barrier
 //   warp 1      TMEM allocator (both CTAs) + tcgen05.mma.cta_group::2 issuer (one lane of the leader CTA);
-//               tcgen05.commit multicasts the `empty` (all CTAs of the cluster) and `tmem full` (the pair) arrivals;
+//               tcgen05.commit multicasts the `empty` and `tmem full` arrivals to both CTAs;
 //               in cluster rank 1 (no MMAs to issue) the same lane is the tile-feed writer
 //   warps 2..9  epilogue of this CTA's 128 TMEM lanes (drain_accumulator in xengine_tc.cuh); they release the
 //               accumulator by arriving on the leader's `tmem empty` barrier through shared::cluster
@@ -25,11 +25,6 @@
 namespace xtc {
 
 constexpr int kPairRows = 256;                 // G rows per pair tile
-#ifdef CORR_NO_DIAG_REUSE                       // developer A/B switch (CORR_DEFINES=-DCORR_NO_DIAG_REUSE): measured
-constexpr bool kDiagReuse = false;              // 1.86 M instead of 1.55 M cycles per config-4 call without the reuse
-#else
-constexpr bool kDiagReuse = true;
-#endif
 constexpr int kPairBoxes = 1;                  // TMA boxes stacked along time per 128-byte chunk of a pipeline stage
 constexpr int kPairStageBytes = 32 * 1024;     // per CTA and stage: A 128 components + B 128 components, kPairStageK samples
 template <int kElt> constexpr int kPairStageK = kPairStageBytes / (2 * 128 * kElt);    // 128 (ci8) / 64 (cf16) samples
@@ -46,31 +41,24 @@ struct PairTile {
     int row0;   // first G row    (multiple of 256), real components u within the channel
     int col0;   // first G column (multiple of 256)
 };
-// Work item of one cluster: one tile per pair, all of the same channel.
-struct PairGroup {
-    PairTile t[2];
-    int share;   // bit 0: both tiles have the same rows (A multicast), bit 1: the same columns (B multicast);
-                 // 3: t[1] duplicates t[0] (odd tile out) and is computed but not written
-    int pad;
-};
 
 struct PairParams {
     Params base;                 // geometry, output, accumulate, k_chunk (tiles/tiles_per_chan/n_tiles unused)
-    const PairGroup* groups;     // DEVICE: per-channel group table
-    int groups_per_chan;
-    long long n_groups;          // groups_per_chan * n_chan (< 2^31 - grid)
-    unsigned int* sched_counter; // DEVICE, zeroed before the launch: groups handed out beyond the first one per cluster
+    const PairTile* tiles;       // DEVICE: per-channel tile table (triangle: column-block major; rectangle: all blocks)
+    int tiles_per_chan;
+    long long n_tiles;           // tiles_per_chan * n_chan * n_dump (< 2^31 - grid)
+    unsigned int* sched_counter; // DEVICE, zeroed before the launch: tiles handed out beyond the first one per cluster
 };
 
-// Dynamic tile feed.  Every cluster starts on group `cluster id`; further groups are claimed in order from one
-// global counter, so all clusters work on neighbouring groups (= the same few channels: their input stays in L2) and a
-// slow cluster simply takes fewer groups (a static round robin ended 9.5 % later on its slowest cluster).  The
-// otherwise idle MMA-warp lane of cluster rank 1 (the pair's second CTA issues no MMAs) is the writer: it claims groups
-// with atomicAdd and publishes each into a small slot ring in the shared memory of EVERY CTA of the cluster
-// (st.shared::cluster + cluster-scope fence + remote mbarrier arrive); producers, MMA issuers and epilogue warps read
-// their CTA's copy and report the slot read on rank 1's `slot free` barrier.  A value >= n_groups ends every loop.
+// Dynamic tile feed.  Every cluster starts on tile `cluster id`; further tiles are claimed in order from one
+// global counter, so all clusters work on neighbouring tiles (= the same few channels: their input stays in L2) and a
+// slow cluster simply takes fewer tiles (a static round robin ended 9.5 % later on its slowest cluster).  The
+// otherwise idle MMA-warp lane of cluster rank 1 (the pair's second CTA issues no MMAs) is the writer: it claims tiles
+// with atomicAdd and publishes each into a small slot ring in the shared memory of BOTH CTAs
+// (st.shared::cluster + cluster-scope fence + remote mbarrier arrive); producers, the MMA issuer and epilogue warps read
+// their CTA's copy and report the slot read on rank 1's `slot free` barrier.  A value >= n_tiles ends every loop.
 // (Claiming from the TMA producer thread instead cost 1500 clk per tile of load issue: measured 13 % slower.)
-constexpr int kFeedSlots = 3;      // the writer claims at most this many groups ahead of the cluster's slowest reader
+constexpr int kFeedSlots = 3;      // the writer claims at most this many tiles ahead of the cluster's slowest reader
 struct TileFeed {
     uint32_t full0;           // this CTA's  slot-filled barriers  [kFeedSlots]
     uint32_t slot0;           // this CTA's  slot values (u32)     [kFeedSlots]
@@ -100,16 +88,16 @@ struct TileFeed {
         return g;
     }
     // the writer (one thread of cluster rank 1; `free0_local` is its own barrier): same slot/phase bookkeeping
-    __device__ __forceinline__ void publish(uint32_t g, int n_ctas, uint32_t free0_local) {
+    __device__ __forceinline__ void publish(uint32_t g, uint32_t free0_local) {
         ptx::mbar_wait(free0_local + 8u * slot, phase ^ 1u);         // every consumer of the cluster has read the old value
-        for (int r = 0; r < n_ctas; ++r) ptx::st_shared_cluster_u32(ptx::mapa(slot0 + 4u * slot, r), g);
+        for (uint32_t r = 0; r < 2; ++r) ptx::st_shared_cluster_u32(ptx::mapa(slot0 + 4u * slot, r), g);
         ptx::fence_acq_rel_cluster();
-        for (int r = 0; r < n_ctas; ++r) ptx::mbar_arrive_cluster(ptx::mapa(full0 + 8u * slot, r));
+        for (uint32_t r = 0; r < 2; ++r) ptx::mbar_arrive_cluster(ptx::mapa(full0 + 8u * slot, r));
         advance();
     }
 };
 
-template <int kElt, int kPairs>
+template <int kElt>
 __global__ void __launch_bounds__(kNumThreads, 1)
 xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const __grid_constant__ CUtensorMap tmap_b,
                     const PairParams pp) {
@@ -126,11 +114,12 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const __grid_co
     static_assert(2 * kOpChunks * kChunkBytes == kPairStageBytes, "stage size");
     // M = 256 (16 << 24), N = 256 (32 << 17); formats and MN-major bits as for the 1-CTA kernel
     constexpr uint32_t kIdesc = (C::kIdesc & ~(0x1fu << 24)) | (16u << 24) | (32u << 17);
-    constexpr uint16_t kAllMask = static_cast<uint16_t>((1u << (2 * kPairs)) - 1u);
+    constexpr uint16_t kPairMask = 3;
 
     extern __shared__ uint8_t smem_raw[];
-    // the SAME offsets in every CTA of the cluster (multicast and cta_group::2 address by offset): the dynamic
-    // shared memory window starts at the same offset in all CTAs of a launch, so the rounding is identical
+    // the SAME offsets in both CTAs of the pair (cta_group::2 addresses by offset): the dynamic shared memory
+    // window starts at the same offset in all CTAs of a launch.  SWIZZLE_128B needs 1024-byte alignment; a kernel
+    // without static shared memory gets it (corr_create verifies the launch works; a violation traps).
     const uint32_t smem_base = ptx::smem_u32(smem_raw);
     if (smem_base & 1023u) __trap();
     const uint32_t epi_base = smem_base + kPairStages * kPairStageBytes;
@@ -144,16 +133,13 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const __grid_co
     const uint32_t feed_free0 = feed_full0 + 8u * kFeedSlots;
     const uint32_t feed_slot0 = feed_free0 + 8u * kFeedSlots;
     static_assert(8 * (2 * kPairStages + 5 + 2 * kFeedSlots) + 4 * kFeedSlots <= 256, "barrier region");
-    // readers of a feed slot per cluster: 8 epilogue warps and the TMA producer of every CTA, one MMA issuer per pair
-    constexpr uint32_t kFeedReaders = 2 * kPairs * kNumEpiWarps + kPairs + 2 * kPairs;
+    // readers of a feed slot per cluster: 8 epilogue warps and the TMA producer of each CTA, and the MMA issuer
+    constexpr uint32_t kFeedReaders = 2 * kNumEpiWarps + 2 + 1;
     uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - ptx::smem_u32(smem_raw)));
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
-    const uint32_t rank = ptx::cluster_ctarank();          // 0 .. 2 kPairs - 1
-    const int pair = static_cast<int>(rank >> 1);
-    const int half = static_cast<int>(rank & 1u);          // 0 = pair leader (issues the MMAs)
-    const uint16_t pair_mask = static_cast<uint16_t>(3u << (2 * pair));
+    const int half = static_cast<int>(ptx::cluster_ctarank());      // 0 = pair leader (issues the MMAs)
     const long long cluster_id = ptx::cluster_id_x();
     const long long n_clusters = ptx::cluster_count_x();
 
@@ -162,7 +148,7 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const __grid_co
         ptx::prefetch_tensormap(&tmap_b);
         for (int s = 0; s < kPairStages; ++s) {
             ptx::mbar_init(full_bar(s), 1);                  // leader: its own arrive.expect_tx
-            ptx::mbar_init(empty_bar(s), kPairs);            // one tcgen05.commit arrival per pair of the cluster
+            ptx::mbar_init(empty_bar(s), 1);                 // the tcgen05.commit arrival
         }
         for (int a = 0; a < 2; ++a) {
             ptx::mbar_init(tfull_bar(a), 1);
@@ -179,7 +165,7 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const __grid_co
         ptx::tmem_relinquish_pair();
     }
     ptx::tc_fence_before();
-    ptx::cluster_sync();                 // barriers of every CTA initialised before anyone signals them
+    ptx::cluster_sync();                 // barriers of both CTAs initialised before anyone signals them
     ptx::tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
 
@@ -195,64 +181,37 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const __grid_co
         if (lane == 0) {
             int stage = 0;
             uint32_t phase = 0;
-            [[maybe_unused]] long long st_empty = 0;
-            [[maybe_unused]] const long long st_begin = clock64();
             TileFeed feed(feed_full0, feed_free0, feed_slot0);
-            for (long long g = cluster_id; g < pp.n_groups; g = feed.next()) {
-                const int cd = static_cast<int>(g / pp.groups_per_chan);            // integration * C + channel
-                const PairGroup gd = pp.groups[g - static_cast<long long>(cd) * pp.groups_per_chan];
-                const PairTile td = (kPairs == 2 && pair == 1) ? gd.t[1] : gd.t[0];
-                const int dump = cd / prm.n_chan, c = cd - dump * prm.n_chan;
+            for (long long g = cluster_id; g < pp.n_tiles; g = feed.next()) {
+                const int cd = static_cast<int>(g / pp.tiles_per_chan);             // integration * C + channel
+                const PairTile td = pp.tiles[g - static_cast<long long>(cd) * pp.tiles_per_chan];
+                const int dump = cd / prm.n_chan, c = prm.chan0 + (cd - dump * prm.n_chan);
                 const int w_a = c * M2 + td.row0 + 128 * half;      // this CTA's A rows in the [n_dump][T][C*2M] view
                 const int w_b = c * M2b + td.col0 + 128 * half;     // this CTA's half of the B columns
-                // a shared operand is fetched once, by pair 0's CTA, and multicast to the same-half CTA of pair 1
-                const bool mc_a = kPairs == 2 && (gd.share & 1);
-                const bool mc_b = kPairs == 2 && (gd.share & 2);
                 // diagonal tile: this CTA's half of the B columns IS its 128 A rows -> one load serves both operands
-                const bool diag = kPairs == 1 && !rect && td.row0 == td.col0 && kDiagReuse;
-                const uint16_t mc_mask = static_cast<uint16_t>((1u << half) | (4u << half));
+                const bool diag = !rect && td.row0 == td.col0;
                 for (int kb = 0; kb < num_kb; ++kb) {
-                    {
-                        CORR_STAT_T0();
-                        ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
-                        CORR_STAT_ADD(st_empty);
-                    }
+                    ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
                     const uint32_t sa = smem_base + stage * kPairStageBytes;
                     const uint32_t sb = sa + kOpChunks * kChunkBytes;
                     if (half == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), diag ? kPairStageBytes : 2u * kPairStageBytes);
 #pragma unroll
                     for (int ch = 0; ch < kOpChunks; ++ch)
 #pragma unroll
-                        for (int b = 0; b < kPairBoxes; ++b) {
-                            if (!mc_a)
-                                ptx::tma_load_3d_pair(sa + ch * kChunkBytes + b * kBoxBytes, &tmap_in, full_bar(stage),
-                                                      w_a + ch * kChunkElems, kb * kStageK + b * kBoxRows, dump);
-                            else if (pair == 0)
-                                ptx::tma_load_3d_pair_mc(sa + ch * kChunkBytes + b * kBoxBytes, &tmap_in, full_bar(stage),
-                                                         w_a + ch * kChunkElems, kb * kStageK + b * kBoxRows, dump, mc_mask);
-                        }
-                    if (diag) {
-                        if (++stage == kPairStages) { stage = 0; phase ^= 1u; }
-                        continue;
-                    }
+                        for (int b = 0; b < kPairBoxes; ++b)
+                            ptx::tma_load_3d_pair(sa + ch * kChunkBytes + b * kBoxBytes, &tmap_in, full_bar(stage),
+                                                  w_a + ch * kChunkElems, kb * kStageK + b * kBoxRows, dump);
+                    if (!diag) {
 #pragma unroll
-                    for (int ch = 0; ch < kOpChunks; ++ch)
+                        for (int ch = 0; ch < kOpChunks; ++ch)
 #pragma unroll
-                        for (int b = 0; b < kPairBoxes; ++b) {
-                            if (!mc_b)
+                            for (int b = 0; b < kPairBoxes; ++b)
                                 ptx::tma_load_3d_pair(sb + ch * kChunkBytes + b * kBoxBytes, &tmap_b, full_bar(stage),
                                                       w_b + ch * kChunkElems, kb * kStageK + b * kBoxRows, dump);
-                            else if (pair == 0)
-                                ptx::tma_load_3d_pair_mc(sb + ch * kChunkBytes + b * kBoxBytes, &tmap_b, full_bar(stage),
-                                                         w_b + ch * kChunkElems, kb * kStageK + b * kBoxRows, dump, mc_mask);
-                        }
+                    }
                     if (++stage == kPairStages) { stage = 0; phase ^= 1u; }
                 }
             }
-#ifdef CORR_STATS
-            prm.stats[blockIdx.x * 8 + 0] = clock64() - st_begin;
-            prm.stats[blockIdx.x * 8 + 1] = st_empty;
-#endif
         }
     } else if (warp == 1) {
         // ===================== MMA issuer (pair leader only) =====================
@@ -261,26 +220,17 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const __grid_co
             uint32_t phase = 0;
             int acc = 0;
             uint32_t acc_phase = 0;
-            [[maybe_unused]] long long st_tempty = 0, st_full = 0;
             TileFeed feed(feed_full0, feed_free0, feed_slot0);
-            for (long long g = cluster_id; g < pp.n_groups; g = feed.next()) {
-                const PairGroup gd = pp.groups[g % pp.groups_per_chan];
-                const bool diag = kPairs == 1 && !rect && gd.t[0].row0 == gd.t[0].col0 && kDiagReuse;      // B operand = the A buffer
+            for (long long g = cluster_id; g < pp.n_tiles; g = feed.next()) {
+                const PairTile td = pp.tiles[g % pp.tiles_per_chan];
+                const bool diag = !rect && td.row0 == td.col0;      // B operand = the A buffer
                 for (int kb0 = 0; kb0 < num_kb; kb0 += kb_per_chunk) {
                     const int kb1 = kb0 + kb_per_chunk < num_kb ? kb0 + kb_per_chunk : num_kb;
                     const uint32_t d_tmem = tmem_base + acc * kTileCols;
-                    {
-                        CORR_STAT_T0();
-                        ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1u);     // both CTAs' epilogues have drained it
-                        CORR_STAT_ADD(st_tempty);
-                    }
+                    ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1u);     // both CTAs' epilogues have drained it
                     ptx::tc_fence_after();
                     for (int kb = kb0; kb < kb1; ++kb) {
-                        {
-                            CORR_STAT_T0();
-                            ptx::mbar_wait(full_bar(stage), phase);          // both CTAs' operand bytes have landed
-                            CORR_STAT_ADD(st_full);
-                        }
+                        ptx::mbar_wait(full_bar(stage), phase);          // both CTAs' operand bytes have landed
                         ptx::tc_fence_after();
                         const uint32_t sa = smem_base + stage * kPairStageBytes;
                         const uint32_t sb = diag ? sa : sa + kOpChunks * kChunkBytes;
@@ -292,24 +242,20 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const __grid_co
                             if constexpr (C::kFloat) ptx::mma_f16_pair(d_tmem, adesc, bdesc, kIdesc, accum);
                             else ptx::mma_i8_pair(d_tmem, adesc, bdesc, kIdesc, accum);
                         }
-                        ptx::mma_commit_pair_mc(empty_bar(stage), kAllMask);   // slot free in every CTA that fills it
+                        ptx::mma_commit_pair_mc(empty_bar(stage), kPairMask);  // slot free in both CTAs
                         if (++stage == kPairStages) { stage = 0; phase ^= 1u; }
                     }
-                    ptx::mma_commit_pair_mc(tfull_bar(acc), pair_mask);        // accumulator complete in both CTAs
+                    ptx::mma_commit_pair_mc(tfull_bar(acc), kPairMask);        // accumulator complete in both CTAs
                     if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
                 }
             }
-#ifdef CORR_STATS
-            prm.stats[blockIdx.x * 8 + 2] = st_tempty;
-            prm.stats[blockIdx.x * 8 + 3] = st_full;
-#endif
-        } else if (lane == 0 && rank == 1) {
+        } else if (lane == 0 && half == 1) {
             // ===================== tile-feed writer (this CTA issues no MMAs) =====================
             TileFeed feed(feed_full0, feed_free0, feed_slot0);
             for (;;) {
                 const uint32_t g_next = atomicAdd(pp.sched_counter, 1u) + static_cast<uint32_t>(n_clusters);
-                feed.publish(g_next, 2 * kPairs, feed_free0);
-                if (g_next >= pp.n_groups) break;
+                feed.publish(g_next, feed_free0);
+                if (g_next >= pp.n_tiles) break;
             }
         }
     } else {
@@ -318,22 +264,21 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const __grid_co
         const int quarter = warp & 3;                // TMEM lanes [32*quarter, 32*quarter+32) belong to this warp
         const int chalf = ew >> 2;                   // column half of the tile handled by this warp
         const uint32_t stage_smem = epi_base + ew * kPairEpiWarpBytes;
-        const uint32_t leader = rank & ~1u;
         int acc = 0;
         uint32_t acc_phase = 0;
         int buf = 0;
-        [[maybe_unused]] long long st_tfull = 0, st_drain = 0;
         TileFeed feed(feed_full0, feed_free0, feed_slot0);
-        for (long long g = cluster_id; g < pp.n_groups; g = feed.next_warp(lane)) {
-            const int c = static_cast<int>(g / pp.groups_per_chan);
-            const PairGroup gd = pp.groups[g - static_cast<long long>(c) * pp.groups_per_chan];
-            const PairTile td = (kPairs == 2 && pair == 1) ? gd.t[1] : gd.t[0];
+        for (long long g = cluster_id; g < pp.n_tiles; g = feed.next_warp(lane)) {
+            const int cd = static_cast<int>(g / pp.tiles_per_chan);
+            const PairTile td = pp.tiles[g - static_cast<long long>(cd) * pp.tiles_per_chan];
+            const int dump = cd / prm.n_chan;
+            const int c_out = dump * prm.n_chan_total + prm.chan0_out + (cd - dump * prm.n_chan);   // output slab index
             const int r0 = td.row0 + 128 * half;                   // first G row of this CTA
             const int u0 = r0 + quarter * 32;                      // first G row of this warp
             // columns this CTA's rows need: up to the last station of its rows (s_j <= s_i), none for rows past the
-            // channel's 2M components or for the duplicate tile of an odd group
+            // channel's 2M components
             int need = 0;
-            if (r0 < M2 && !(kPairs == 2 && pair == 1 && gd.share == 3)) {
+            if (r0 < M2) {
                 int i_max = (r0 + 127) / (2 * prm.n_pol);
                 if (i_max > prm.n_station - 1) i_max = prm.n_station - 1;
                 need = (rect ? M2b : (i_max + 1) * 2 * prm.n_pol) - td.col0;
@@ -344,32 +289,19 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const __grid_co
             const int h_end = need < h_begin + kTileCols / 2 ? need : h_begin + kTileCols / 2;
             for (int kc = 0; kc < n_kchunks; ++kc) {
                 const bool reduce = prm.accumulate != 0 || kc != 0;
-                {
-                    CORR_STAT_T0();
-                    ptx::mbar_wait(tfull_bar(acc), acc_phase);
-                    CORR_STAT_ADD(st_tfull);
-                }
+                ptx::mbar_wait(tfull_bar(acc), acc_phase);
                 ptx::tc_fence_after();
                 const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + acc * kTileCols;
-                {
-                    CORR_STAT_T0();
-                    drain_accumulator<C::kFloat, true, kPairEpiBufs>(prm, c, u0, td.col0, h_begin, h_end, taddr,
-                                                       ptx::mapa(tempty_bar(acc), leader), reduce, kc == 0, stage_smem, buf, lane);
-                    CORR_STAT_ADD(st_drain);
-                }
+                drain_accumulator<C::kFloat, true, kPairEpiBufs>(prm, c_out, u0, td.col0, h_begin, h_end, taddr,
+                                                                 ptx::mapa(tempty_bar(acc), 0), reduce, kc == 0,
+                                                                 stage_smem, buf, lane);
                 if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
             }
         }
         if (lane < 8) ptx::bulk_wait<0>();           // all bulk stores performed before the CTA retires
-#ifdef CORR_STATS
-        if (warp == 2 && lane == 0) {
-            prm.stats[blockIdx.x * 8 + 4] = st_tfull;
-            prm.stats[blockIdx.x * 8 + 5] = st_drain;
-        }
-#endif
     }
 
-    // no CTA may exit (or free TMEM) while a peer can still signal its barriers or read its operands
+    // no CTA may exit (or free TMEM) while its peer can still signal its barriers or read its operands
     ptx::tc_fence_before();
     ptx::cluster_sync();
     if (warp == 1) {

@@ -18,6 +18,9 @@ struct Params {
     // n_station * n_station_b and visibilities are ordered [c][i][j][p][q].  n_station_b == 0: packed triangle of `in`.
     const void* in_b;
     int n_station_b;
+    // channel window: n_chan channels starting at channel chan0 of inputs laid out for n_chan_total channels, written to
+    // the output slabs chan0_out ..
+    int chan0, n_chan_total, chan0_out;
 };
 
 __device__ __forceinline__ void decode_baseline(long long b, int& i, int& j) {
@@ -31,14 +34,16 @@ __device__ __forceinline__ void decode_baseline(long long b, int& i, int& j) {
 
 template <bool kFloat>
 __global__ void xengine_simt_kernel(const Params prm) {
-    const int P = prm.n_pol, N = prm.n_station, C = prm.n_chan;
-    for (long long v = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; v < prm.n_vis;
-         v += static_cast<long long>(gridDim.x) * blockDim.x) {
-        const int q = static_cast<int>(v % P);
-        const int p = static_cast<int>((v / P) % P);
-        const long long cb = v / (P * P);
+    const int P = prm.n_pol, N = prm.n_station, C = prm.n_chan_total;
+    const long long v_out0 = static_cast<long long>(prm.chan0_out) * prm.n_baseline * P * P;    // first word of the window
+    for (long long w = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; w < prm.n_vis;
+         w += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const long long v = v_out0 + w;                                                         // output word
+        const int q = static_cast<int>(w % P);
+        const int p = static_cast<int>((w / P) % P);
+        const long long cb = w / (P * P);
         const long long b = cb % prm.n_baseline;
-        const int c = static_cast<int>(cb / prm.n_baseline);
+        const int c = prm.chan0 + static_cast<int>(cb / prm.n_baseline);                        // input channel
         int i, j;
         const bool rect = prm.n_station_b > 0;
         if (rect) {

@@ -71,20 +71,14 @@ struct Params {
     // pair kernels: number of separate integrations of n_time samples in one call (corr_xengine_dumps); the input is
     // [n_dump][n_time][C][...], the output [n_dump][C][...]: integration d, channel c is handled as "channel" d*C + c
     int n_dump;
+    // channel window (corr_create_window; "separating frequency channels prior to the CMAC stage"): the
+    // call integrates n_chan channels starting at channel chan0 of the input (whose row pitch the tensor map carries)
+    // into the output slabs chan0_out .. of an output laid out for n_chan_total channels (integration d of a dump call
+    // starts at slab d * n_chan_total).  Whole-band plans: 0, 0 and n_chan.
+    int chan0, chan0_out, n_chan_total;
     // 1-CTA kernel: a stage holds [b_chunks 128-byte-wide B chunks][A chunks, only if some tile is off the diagonal]
     int n_stages, stage_bytes, b_chunks;
-#ifdef CORR_STATS
-    unsigned long long* stats;   // DEVICE, 8 counters per CTA (developer build only: python -m ...build with CORR_STATS=1)
-#endif
 };
-
-#ifdef CORR_STATS
-#define CORR_STAT_T0() const long long stat_t0_ = clock64()
-#define CORR_STAT_ADD(var) (var) += clock64() - stat_t0_
-#else
-#define CORR_STAT_T0() do {} while (0)
-#define CORR_STAT_ADD(var) do {} while (0)
-#endif
 
 template <int kElt> struct Cfg;
 template <> struct Cfg<1> {                      // complex int8 -> int32
@@ -135,7 +129,7 @@ __device__ __forceinline__ void combine_chunk(const uint32_t (&v)[32], int ri, u
 
 // Drain one TMEM accumulator pass of one tile through this epilogue warp: tcgen05.ld -> Re/Im combine ->
 // packed-baseline writer (+ accumulate).  The warp owns TMEM lanes [32 quarter, +32) = G rows u0 .. u0 + 31 of
-// channel c and the tile columns [h_begin, h_end) (G columns col0 + h); `taddr` addresses lane 32 quarter,
+// output slab c (global channel, or integration * n_chan_total + channel) and the tile columns [h_begin, h_end) (G columns col0 + h); `taddr` addresses lane 32 quarter,
 // column 0 of the accumulator.  `release_bar` is arrived on (by lane 0; `kRemote`: it lives in the pair leader
 // CTA and is a shared::cluster address) as soon as the warp's last TMEM column is in registers.
 // first_pass: no earlier pass of this tile wrote the same output addresses (else wait for those writes).
@@ -329,8 +323,8 @@ xengine_direct_kernel(const __grid_constant__ CUtensorMap tmap_in, const Params 
             for (long long tile = blockIdx.x; tile < prm.n_tiles; tile += gridDim.x) {
                 const int c = static_cast<int>(tile / prm.tiles_per_chan);
                 const TileDesc td = prm.tiles[tile - static_cast<long long>(c) * prm.tiles_per_chan];
-                const int w_row = c * M2 + td.row0;        // element coordinate in the [T][C*2M] view
-                const int w_col = c * M2 + td.col0;
+                const int w_row = (prm.chan0 + c) * M2 + td.row0;        // element coordinate in the [T][C*2M] view
+                const int w_col = (prm.chan0 + c) * M2 + td.col0;
                 const int nb = (td.ncols + kChunkElems - 1) / kChunkElems;
                 // tile on the diagonal: the 128 A rows are among the loaded B columns -> A is not loaded at all
                 const bool a_in_b = td.row0 >= td.col0 && td.row0 + kTileRows <= td.col0 + nb * kChunkElems;
@@ -343,13 +337,13 @@ xengine_direct_kernel(const __grid_constant__ CUtensorMap tmap_in, const Params 
 #pragma unroll
                     for (int a = 0; a < kAChunks; ++a)
                         if (!a_in_b)
-                            ptx::tma_load_2d(sa + a * kChunkBytes, &tmap_in, full_bar(stage),
-                                         w_row + a * kChunkElems, kb * C::kKStage);
+                            ptx::tma_load_3d(sa + a * kChunkBytes, &tmap_in, full_bar(stage),
+                                             w_row + a * kChunkElems, kb * C::kKStage, 0);
 #pragma unroll
                     for (int b = 0; b < kBChunksMax; ++b)
                         if (b < nb)
-                            ptx::tma_load_2d(sb + b * kChunkBytes, &tmap_in, full_bar(stage),
-                                             w_col + b * kChunkElems, kb * C::kKStage);
+                            ptx::tma_load_3d(sb + b * kChunkBytes, &tmap_in, full_bar(stage),
+                                             w_col + b * kChunkElems, kb * C::kKStage, 0);
                     if (++stage == kNumStages) { stage = 0; phase ^= 1u; }
                 }
             }
@@ -416,8 +410,8 @@ xengine_direct_kernel(const __grid_constant__ CUtensorMap tmap_in, const Params 
                 ptx::mbar_wait(tfull_bar(acc), acc_phase);
                 ptx::tc_fence_after();
                 const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + acc * kTileCols;
-                drain_accumulator<C::kFloat, false>(prm, c, u0, td.col0, h_begin, h_end, taddr, tempty_bar(acc), reduce,
-                                                    kc == 0, stage_smem, buf, lane);
+                drain_accumulator<C::kFloat, false>(prm, prm.chan0_out + c, u0, td.col0, h_begin, h_end, taddr, tempty_bar(acc),
+                                                    reduce, kc == 0, stage_smem, buf, lane);
                 if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
             }
         }

@@ -82,6 +82,20 @@ def test_layout_and_fp16_rounding():
     assert (np.abs(x[..., 0].astype(np.float64) - S.real) <= 0.5 * np.spacing(np.abs(x[..., 0]).astype(np.float16)).astype(np.float64) + 1e-12).all()
 
 
+def test_to_xengine_input_rounds_both_components_to_nearest_even():
+    """Hand-written half-way cases (binary16 has 11 significant bits: spacing 2 in [2048, 4096), 4 in [4096, 8192)):
+    2049 -> 2048 and 2051 -> 2052 (ties to even), 2050 exact, 4098 -> 4096, 4102 -> 4104, -2049 -> -2048; the real and the
+    imaginary part are rounded independently and land in [..., 0] and [..., 1]."""
+    S = np.array([[[2049 + 2051j, 2051 - 2049j, 2050 + 4098j, -2049 + 4102j, 0.1 - 65504j, 1e-9 + 3j]]])        # [1, 1, 6]
+    x = fo.to_xengine_input(S)
+    assert x.shape == (1, 1, 6, 2) and x.dtype == np.float16
+    want = [[2048, 2052], [2052, -2048], [2050, 4096], [-2048, 4104], [float(np.float16(0.1)), -65504], [0.0, 3]]
+    got = x[0, 0].astype(np.float64)
+    assert got[:5].tolist() == want[:5]
+    assert got[5, 1] == 3 and abs(got[5, 0] - 1e-9) < 6e-8 and got[5, 0] in (0.0, float(np.float16(1e-9)))     # below the subnormal step
+    assert float(np.float16(0.1)) == 0.0999755859375            # 0.1 -> nearest binary16, written out
+
+
 def test_rejects_bad_input():
     with pytest.raises(ValueError):
         fo.fengine(np.zeros((2, 100), np.int8))

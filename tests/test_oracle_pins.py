@@ -113,12 +113,20 @@ def test_cf16_reduces_to_zgemm(oracle):
     ref = pack(full_matrix_numpy(x), N, P)
     scale = np.abs(ref).max()
     assert np.max(np.abs(V[..., 0] + 1j * V[..., 1] - ref)) <= 1e-12 * scale
+    # the single-visibility routine on fp16 input (xo_pair_cf16) against the same ZGEMM entries, every (c, i, p, j, q)
+    for c in range(C):
+        for i in range(N):
+            for j in range(i + 1):
+                for p in range(P):
+                    for q in range(P):
+                        re, im = oracle.visibility(x, c, i, p, j, q)
+                        assert abs(complex(re, im) - ref[c, oracle.baseline_index(i, j), p, q]) <= 1e-12 * scale
 
 
 def test_half_conversion_all_patterns(oracle):
     bits = np.arange(65536, dtype=np.uint16)
     lib = bits.view(np.float16).astype(np.float64)           # numpy's converter, independent
-    for b in list(range(0, 65536, 7)) + [0x0001, 0x03FF, 0x0400, 0x7BFF, 0x7C00, 0xFC00, 0x8000]:
+    for b in range(65536):                                   # every binary16 pattern, NaNs and subnormals included
         got = oracle.half_to_double(b)
         assert (np.isnan(got) and np.isnan(lib[b])) or got == lib[b]
     assert np.signbit(oracle.half_to_double(0x8000))
@@ -209,6 +217,9 @@ def test_delayed_tone_exact_quarter_turns(oracle):
                 assert abs(complex(got[0], got[1]) - want) < 1e-12
                 goti = Vi[c, oracle.baseline_index(i, j), 0, 0]
                 assert abs(complex(goti[0], goti[1]) - 1e4 * want) < 1e-9
+                # xo_pair_cf16 / xo_pair_ci8 straight from the ungathered input: the same closed form (sign of Im pinned)
+                assert abs(complex(*oracle.visibility(x, c, i, 0, j, 0)) - want) < 1e-12
+                assert abs(complex(*oracle.visibility((x * 100).astype(np.int8), c, i, 0, j, 0)) - 1e4 * want) < 1e-9
 
 
 def test_delayed_tone_phase_slope(oracle):

@@ -101,12 +101,12 @@ def test_ci8_bit_exact_small(corr, oracle, N, P, C, T):
 
 
 # every tensor-core kernel variant on geometries that span ragged pair tiles, several row / column blocks,
-# odd group counts (duplicate tile of the quad kernel), ragged T and both polarisation counts
+# ragged T and both polarisation counts
 KERNEL_CASES = [(16, 2, 5, 100), (64, 2, 9, 200), (72, 2, 3, 130), (96, 2, 4, 64), (128, 2, 5, 257),
                 (136, 1, 3, 96), (200, 2, 2, 128), (256, 2, 3, 192), (320, 2, 2, 64)]
 
 
-@pytest.mark.parametrize("kernel", ["single", "pair", "quad", "simt"])
+@pytest.mark.parametrize("kernel", ["single", "pair", "simt"])
 @pytest.mark.parametrize("N,P,C,T", KERNEL_CASES)
 def test_ci8_bit_exact_every_kernel(corr, oracle, kernel, N, P, C, T):
     x = inputs.gauss_ci8(T, C, N, P, 40.0, seed=7100 + N + T)
@@ -115,7 +115,7 @@ def test_ci8_bit_exact_every_kernel(corr, oracle, kernel, N, P, C, T):
     assert_bit_exact(got, want)
 
 
-@pytest.mark.parametrize("kernel", ["single", "pair", "quad", "simt"])
+@pytest.mark.parametrize("kernel", ["single", "pair", "simt"])
 @pytest.mark.parametrize("N,P,C,T", [(24, 2, 3, 100), (64, 2, 3, 1100), (96, 1, 2, 64), (160, 2, 2, 2100)])
 def test_cf16_within_tolerance_every_kernel(corr, oracle, kernel, N, P, C, T):
     x = inputs.corr_phase_cf16(T, C, N, P, seed=7200 + N)
@@ -228,22 +228,28 @@ def test_stream_argument_is_honoured(corr, oracle):
 
 
 def test_corner_turn_kernel(corr):
-    """Piece (a): ws[c][m][t] = in[t][c][m], ws_rot = (im, -re), time zero-padded -- against torch ops."""
+    """Piece (a): ws[c][m][t] = in[t][c][m], ws_rot = (im, -re), time zero-padded -- against oracle.corner_turn (plain
+    loops, pinned in tests/test_oracle_corner_turn_pins.py).  The int8 case carries -128: the rotated plane saturates
+    -(-128) to +127 (corr.h), everything else is exact."""
+    from oracle import corner_turn as oc
     for dtype, N, P, C, T in [("ci8", 24, 2, 5, 100), ("ci8", 64, 2, 3, 256), ("cf16", 20, 2, 3, 70)]:
         if dtype == "ci8":
             x = inputs.gauss_ci8(T, C, N, P, 30.0, seed=7700)
+            x[0, 0, 0, 0, 0] = -128
+            x[T - 1, C - 1, N - 1, P - 1] = -128
         else:
             x = inputs.corr_phase_cf16(T, C, N, P, seed=7701)
         with corr.Correlator(N, P, C, T, dtype) as h:
             ws = h.corner_turn(x.cuda())
             torch.cuda.synchronize()
             Tp = h.workspace_time
-            planes = ws.cpu().view(torch.int8 if dtype == "ci8" else torch.float16).view(2, C, N * P, Tp, 2)
-        ref = x.reshape(T, C, N * P, 2).permute(1, 2, 0, 3)                       # [C, M, T, 2]
-        assert torch.equal(planes[0, :, :, :T], ref)
-        rot = torch.stack([ref[..., 1], -ref[..., 0]], dim=-1)
-        assert torch.equal(planes[1, :, :, :T], rot)
-        assert (planes[:, :, :, T:] == 0).all()
+            planes = ws.cpu().view(torch.int8 if dtype == "ci8" else torch.float16).view(2, C, N * P, Tp, 2).numpy()
+        want_ws, want_rot = oc.corner_turn(x.numpy(), Tp)
+        if dtype == "ci8":
+            assert (want_rot == 128).sum() == 2                      # the two re = -128 samples
+            want_rot = np.minimum(want_rot, 127)
+        assert np.array_equal(planes[0].astype(want_ws.dtype), want_ws)
+        assert np.array_equal(planes[1].astype(want_rot.dtype), want_rot)
 
 
 # ---------------------------------------------------------------------------------------------
@@ -320,9 +326,119 @@ def test_config4_full_size_four_calls(corr, oracle):
     check_full_config(corr, oracle, "cfg4", 8)
 
 
-@pytest.mark.parametrize("N", [32, 128, 512, 1024])
+def test_config1_own_recipe_every_word(corr, oracle):
+    """BASELINE.json config 1 with its own recipe (sigma 16, seed 1001): every word of all 64 channels."""
+    cfg = inputs.CONFIGS["cfg1"]
+    x = inputs.make_input(cfg)
+    got, tc = run_gpu(corr, [x], "ci8")
+    assert tc and got.shape == (64, 136, 2, 2, 2)
+    assert_bit_exact(got, run_oracle(oracle, [x]))
+
+
+@pytest.mark.parametrize("N", [32, 64, 128, 256, 512, 1024])
 def test_config5_sweep_points(corr, oracle, N):
     check_full_config(corr, oracle, "cfg5_n%d" % N, 4 if N <= 128 else 2)
+
+
+# ---------------------------------------------------------------------------------------------
+# channel windows (corr_create_window; SURVEY 8(f) rank 3): windows of ONE input into ONE output
+# ---------------------------------------------------------------------------------------------
+def _windows(C, world):
+    from paper_1305_5639_b200.shard import channel_range
+    return [channel_range(C, world, r) for r in range(world)]
+
+
+@pytest.mark.parametrize("world", [2, 3, 8])
+@pytest.mark.parametrize("N,P,C,T,dtype,kernel", [(72, 2, 11, 200, "ci8", "pair"), (40, 2, 9, 130, "ci8", "single"),
+                                                  (33, 2, 8, 50, "ci8", "simt"), (136, 1, 10, 96, "ci8", None),
+                                                  (64, 2, 9, 1100, "cf16", None)])
+def test_channel_windows_equal_the_unsharded_launch(corr, oracle, world, N, P, C, T, dtype, kernel):
+    """`world` window plans over one [T][C][N][P] buffer, each writing its own slabs of one output (two calls: store, then
+    accumulate): word for word the unsharded launch, and the oracle; a canary value in a window's foreign slabs survives."""
+    x = (inputs.gauss_ci8(T, C, N, P, 40.0, seed=7900 + N) if dtype == "ci8" else inputs.corr_phase_cf16(T, C, N, P, seed=7900 + N))
+    xd = x.cuda()
+    with corr.Correlator(N, P, C, T, dtype) as h:
+        if kernel:
+            h.set_kernel(kernel)
+        whole = h.xengine(xd)
+        whole = h.xengine(xd, whole, accumulate=True)
+        torch.cuda.synchronize()
+    canary = 0x5a5a5a5a if dtype == "ci8" else 12345.0
+    out = torch.full_like(whole, canary)
+    for c0, c1 in _windows(C, world):
+        if c1 == c0:
+            continue
+        with corr.Correlator(N, P, C, T, dtype, window=(c0, c1 - c0)) as hw:
+            if kernel:
+                hw.set_kernel(kernel)
+            assert hw.input_bytes == xd.numel() * xd.element_size() and hw.output_bytes == out.numel() * 4
+            before = out.clone()
+            hw.xengine(xd, out)
+            hw.xengine(xd, out, accumulate=True)
+            torch.cuda.synchronize()
+            keep = torch.ones(C, dtype=torch.bool, device="cuda"); keep[c0:c1] = False
+            assert torch.equal(out[keep], before[keep])              # nothing outside the window's slabs was touched
+    assert torch.equal(out, whole)                                   # word for word (also fp32: same kernel, same order)
+    want = oracle.xengine(x.numpy())
+    if dtype == "ci8":
+        assert_bit_exact(out.cpu().numpy(), 2 * want)
+    else:
+        assert fp16_normalised_error(out.cpu().numpy(), 2 * want, N, P) <= FP16_TOL
+
+
+def test_channel_windows_dumps_and_host_path(corr, oracle):
+    """A window plan through corr_xengine_dumps and corr_xengine_host: only the window's columns / slabs are used."""
+    N, P, C, T = 48, 2, 7, 192
+    x = inputs.gauss_ci8(T, C, N, P, 40.0, seed=7950)
+    want = oracle.xengine(x.numpy())
+    c0, n = 2, 3
+    with corr.Correlator(N, P, C, T, "ci8", window=(c0, n)) as h:
+        out = torch.full((4,) + tuple(h.output_shape()), 77, dtype=torch.int32, device="cuda")
+        h.xengine_dumps(x.cuda(), 4, out)
+        torch.cuda.synchronize()
+        got = out.cpu().numpy()
+        for d in range(4):
+            assert_bit_exact(np.ascontiguousarray(got[d, c0:c0 + n]), oracle.xengine(x[d * 48:(d + 1) * 48].numpy(), chans=list(range(c0, c0 + n))))
+        assert (got[:, :c0] == 77).all() and (got[:, c0 + n:] == 77).all()
+        oh = torch.full(h.output_shape(), 99, dtype=torch.int32)
+        h.xengine_host(x, None)
+        h.xengine_host(x, oh, accumulate=True)
+        assert_bit_exact(np.ascontiguousarray(oh.numpy()[c0:c0 + n]), 2 * want[c0:c0 + n])
+        assert (oh[:c0] == 99).all() and (oh[c0 + n:] == 99).all()
+
+
+def test_window_argument_errors(corr):
+    L = corr.lib()
+    assert not L.corr_create_window(8, 2, 4, 3, 2, 16, 0)            # window runs past the band
+    assert b"window" in L.corr_last_error(None)
+    assert not L.corr_create_window(8, 2, 4, -1, 2, 16, 0)
+    assert not L.corr_create_window(8, 2, 4, 0, 0, 16, 0)
+    with corr.Correlator(8, 2, 4, 16, "ci8", window=(1, 2)) as h:
+        x = torch.zeros(h.input_shape(), dtype=torch.int8, device="cuda")
+        ws = torch.empty(max(h.workspace_bytes, 128), dtype=torch.uint8, device="cuda")
+        assert L.corr_corner_turn(h._h, x.data_ptr(), ws.data_ptr(), None) == corr.CORR_EINVAL
+
+
+@pytest.mark.parametrize("N,P,C,T,dtype", [(40, 2, 19, 300, "ci8"), (16, 2, 3, 64, "ci8"), (24, 2, 1, 100, "ci8"), (20, 2, 9, 260, "cf16")])
+def test_host_path_pipeline(corr, oracle, N, P, C, T, dtype):
+    """corr_xengine_host: the channel-window copy pipeline (8 windows, fewer when C < 8) from PINNED and from pageable
+    host memory, three calls (store, accumulate, accumulate with readback)."""
+    xs = [(inputs.gauss_ci8(T, C, N, P, 40.0, seed=7960 + k) if dtype == "ci8" else inputs.corr_phase_cf16(T, C, N, P, seed=7960 + k))
+          for k in range(3)]
+    want = run_oracle(oracle, xs)
+    for pinned in (True, False):
+        with corr.Correlator(N, P, C, T, dtype) as h:
+            oh = torch.empty(h.output_shape(), dtype=torch.int32 if dtype == "ci8" else torch.float32)
+            if pinned:
+                oh = oh.pin_memory()
+            for k, x in enumerate(xs):
+                xh = x.pin_memory() if pinned else x
+                h.xengine_host(xh, oh if k == 2 else None, accumulate=k > 0)
+            assert h.last_launch_count == min(C, 8)
+            if dtype == "ci8":
+                assert_bit_exact(oh.numpy(), want)
+            else:
+                assert fp16_normalised_error(oh.numpy(), want, N, P) <= FP16_TOL
 
 
 # ---------------------------------------------------------------------------------------------

@@ -16,7 +16,7 @@ def _cases(seed, n):
     for it in range(n):
         P = int(rng.choice([1, 2])); N = int(rng.integers(1, 300)); C = int(rng.integers(1, 5)); T = int(rng.integers(1, 600))
         mode = str(rng.choice(["herk", "cross", "dumps"]))
-        kern = str(rng.choice(["auto", "pair", "single", "quad", "simt"]))
+        kern = str(rng.choice(["auto", "pair", "single", "simt"]))
         Nb = int(rng.integers(1, 200))
         nd = int(rng.choice([d for d in range(1, 9) if T % d == 0]))
         out.append((mode, kern, N, Nb, P, C, T, nd, it))
