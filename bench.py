@@ -9,18 +9,26 @@ of N=256 stations, 2 pol, 1024 channels, accumulated over 4 successive corr_xeng
 T=2048 samples each (accumulate = 0, 1, 1, 1) on four different 2 GiB input buffers, i.e. the
 triangular tcgen05 HERK + cross-call accumulation + packed-baseline writer, all inside libcorr.so.
 
-value    device-resident inputs, CUDA events on the launching stream, max over ranks.
-e2e      the same metric through corr_xengine_host (HOST pinned buffers; H2D of every call's
-         input and D2H of the integrated visibilities inside the timed region).
-roofline dominant kernel (the only kernel of a call) against the tensor peak for its dtype:
-         MEASURED_PEAKS.json bf16 x nominal ratio (int8 2x, fp16 1x) -- see DESIGN.md.
+value     device-resident inputs, CUDA events on the launching stream, max over ranks.
+e2e       the same metric through corr_xengine_host (HOST pinned buffers; H2D of every call's
+          input and D2H of the integrated visibilities inside the timed region).
+roofline  the dominant (only) kernel of a call against the SLOWER of its two roofs (north_star):
+          tensor = algorithmic ops / dense tensor peak of its dtype (MEASURED_PEAKS.json bf16 x nominal
+          ratio: int8 2x, fp16 1x), hbm = algorithmic bytes (input + output, + output again when a call
+          accumulates) / measured copy bandwidth.  Both sides are always reported.
+sustained the same step timed back to back for >= 2 s (power-capped clocks), with its own clock record,
+          against the sustained peaks.
+workloads (N = 1 only) short runs of every other BASELINE.json config point, the cross / dump modes and the
+          standalone corner-turn and F-engine kernels, so that the driver-run line carries them too.
 cpu_baseline / --impl reference: the CPU oracle (oracle/) as it stands, on the host cores, on a
-         bounded sample of the same workload (whole channels: all baselines, full T).
+          bounded sample of the same workload (whole channels: all baselines, full T).
 
 N > 1 (torchrun): the path does not shard (north_star: one GPU, no collectives) -> N independent
 replicas, "scaling": "weak"; the barrier and the max over ranks are the only communication.
+`--shard channels` instead splits ONE seeded workload by channel windows (corr_create_window), no collective.
 """
 import argparse
+import hashlib
 import json
 import os
 import statistics
@@ -36,17 +44,20 @@ if ROOT not in sys.path:
 METRIC = "xengine_tops_8ops_per_cmac"
 UNIT = "TOPS"
 NOMINAL_RATIO = {"ci8": 2.0, "cf16": 1.0}     # dense tensor peak relative to bf16 (guide: 4.5 / 2.25 / 2.25 PF)
+NOMINAL_BF16 = 2250.0
 FALLBACK_BF16_TFLOPS = 1590.0                  # B200_PROFILING.md fallback
 FALLBACK_HBM_GBS = 6650.0
-# DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum) of ONE xengine_direct_kernel launch from
-# the committed `ncu --set full` capture of this workload (profiles/), or None where not captured.
-NCU_TRAFFIC_BYTES = {
-    # profiles/r1c_final_ncu_pair_feed.md (dram__bytes_read.sum + dram__bytes_write.sum of one launch)
-    "cfg4": (3.198e9 + 3 * 4.275e9) / 4,          # accumulate = 0 once, accumulate = 1 three times per step
-    "cfg3": 4.651e9,
-    "cfg5_n64": 1.200e9,
-    "cfg5_n32": 1.139e9,
+# DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum, bytes per launch averaged over the step's calls) from the
+# committed `ncu --set full` captures of the SAME kernel and geometry -- not measured by this run, and emitted only when
+# the kernel that ran is the one that was captured: workload -> (kernel, bytes, capture file)
+NCU_TRAFFIC = {
+    "cfg4": ("pair", (3.198e9 + 3 * 4.275e9) / 4, "profiles/r1c_final_ncu_pair_feed.md"),
+    "cfg3": ("pair", 4.651e9, "profiles/r1c_final_ncu_pair_feed.md"),
+    "cfg5_n64": ("pair", 1.200e9, "profiles/r1c_final_ncu_pair_feed.md"),
+    "cfg5_n32": ("single", 1.139e9, "profiles/r1c_final_ncu_pair_feed.md"),
 }
+KERNEL_NAMES = {"single": "xtc::xengine_direct_kernel<%d>", "pair": "xtc::xengine_pair_kernel<%d>",
+                "simt": "xsimt::xengine_simt_kernel<%d>"}
 
 
 def parse_args():
@@ -56,18 +67,21 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="cfg4")
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
-    ap.add_argument("--kernel", default="auto", choices=["auto", "single", "pair", "quad", "simt"],
+    ap.add_argument("--kernel", default="auto", choices=["auto", "single", "pair", "simt"],
                     help="force a kernel variant (default: the library's own choice)")
     ap.add_argument("--piece", default="xengine", choices=["xengine", "corner_turn", "fengine"],
                     help="corner_turn: time the standalone corner-turn kernel (SURVEY 8(a) a1) on the workload's input; "
                          "fengine: time corr_fengine (SURVEY 8(f) rank 2) on 512 streams x 8192 spectra of 256 real int8 samples")
     ap.add_argument("--shard", default="none", choices=["none", "channels"],
-                    help="channels: the N ranks split the workload's channels (strong scaling, SURVEY 8(f) rank 3); "
+                    help="channels: the N ranks split ONE workload's channels into windows (strong scaling, SURVEY 8(f) rank 3); "
                          "default: N independent replicas (north_star: the path does not shard)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-gemm-peak", action="store_true",
                     help="skip the cuBLAS int8 / fp16 GEMM measured beside the kernel (context for the tensor peak)")
+    ap.add_argument("--no-sustained", action="store_true", help="skip the >= 2 s back-to-back sub-record")
+    ap.add_argument("--no-others", action="store_true", help="skip the short runs of the other workloads and pieces")
+    ap.add_argument("--no-sha", action="store_true", help="skip the SHA-256 of the input buffers")
     ap.add_argument("--e2e-steps", type=int, default=0, help="steps of the host-buffer leg (default min(K, 5))")
     return ap.parse_args()
 
@@ -93,8 +107,8 @@ def peaks():
         with open(path) as f:
             p = json.load(f)
         return dict(bf16=float(p["bf16_tflops"]), bf16_sustained=float(p.get("bf16_tflops_sustained", p["bf16_tflops"])),
-                    hbm=float(p["hbm_gbs"]), source="measured")
-    return dict(bf16=FALLBACK_BF16_TFLOPS, bf16_sustained=1400.0, hbm=FALLBACK_HBM_GBS, source="fallback")
+                    hbm=float(p["hbm_gbs"]), source="MEASURED_PEAKS.json")
+    return dict(bf16=FALLBACK_BF16_TFLOPS, bf16_sustained=1400.0, hbm=FALLBACK_HBM_GBS, source="B200_PROFILING.md fallback")
 
 
 # ------------------------------------------------------------------------------------------------
@@ -111,7 +125,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except OSError:
             self.proc = None
@@ -151,6 +165,16 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------
 # CPU oracle legs (the ONLY places bench.py touches oracle/)
 # ------------------------------------------------------------------------------------------------
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 def oracle_sample_rate(cfg, x_host, min_seconds, xb_host=None):
     """Times oracle.xengine on whole channels of `x_host` ([T, n, N, P, 2] numpy) -> (CMAC/s, seconds, channels)."""
     import oracle
@@ -177,11 +201,33 @@ def cpu_sample_input(cfg, n_chan):
     return inputs.make_input(cfg, call=0, device="cpu", C=n_chan).numpy()
 
 
+def cpu_baseline_record(cfg, x_host, xb_host, min_seconds=10.0):
+    """The oracle as it stands on the host cores: all threads on `x_host`'s channels, then ONE thread on the first
+    channel; CPU model and compiler flags recorded."""
+    import oracle
+    from oracle import build as obuild
+    cores = oracle.max_threads()
+    rate, secs, done = oracle_sample_rate(cfg, x_host, min_seconds, xb_host)
+    oracle.set_threads(1)
+    try:
+        rate1, secs1, done1 = oracle_sample_rate(cfg, x_host[:, :1], min(3.0, min_seconds), None if xb_host is None else xb_host[:, :1])
+    finally:
+        oracle.set_threads(cores)
+    return {"value": 8.0 * rate / 1e12, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": "channels 0..%d of call 0 (all %d baselines x %d pol products, full T=%d), %d channel passes in %.1f s"
+                      % (x_host.shape[1] - 1, cfg["n_baseline"], cfg["P"] ** 2, cfg["T"], done, secs),
+            "gcmac_per_s": rate / 1e9,
+            "threads_1": {"value": 8.0 * rate1 / 1e12, "unit": UNIT, "gcmac_per_s": rate1 / 1e9,
+                          "sample": "channel 0, %d passes in %.1f s" % (done1, secs1)},
+            "cpu_model": cpu_model(), "compiler": "gcc " + " ".join(obuild.CFLAGS)}
+
+
 def run_reference(args):
     """--impl reference: the oracle as it stands on the host cores; rank 0 only."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
     import oracle
+    from oracle import build as obuild
     cfg = workload(args.workload)
     cores = oracle.max_threads()
     n_chan = max(1, min(cfg["C"], cores))
@@ -207,7 +253,8 @@ def run_reference(args):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "int64" if cfg["dtype"] == "ci8" else "f64", "data": "synthetic",
         "config": {"workload": describe(cfg), "sample": sample},
-        "cpu_baseline": {"value": tops, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": tops, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                         "cpu_model": cpu_model(), "compiler": "gcc " + " ".join(obuild.CFLAGS)},
         "e2e": {"value": tops, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -276,53 +323,96 @@ def whole_job_value(units_per_rank_step, steps, world, total_ms):
     return world * steps * units_per_rank_step / (total_ms * 1e-3)
 
 
+def bytes_per_call(cfg):
+    """Algorithmic HBM bytes of one launch, averaged over the step's calls: input once, output written once, and read
+    once more by every call that accumulates."""
+    calls = cfg["calls"]
+    return cfg["in_bytes"] + cfg["out_bytes"] * (1.0 + (calls - 1) / calls)
+
+
+def roofline_record(cfg, kernel, kernel_ms, pk, sustained):
+    """The dominant kernel against the slower of its two roofs; both sides reported (north_star's definition)."""
+    dtype = cfg["dtype"]
+    ratio = NOMINAL_RATIO[dtype]
+    bf16 = pk["bf16_sustained"] if sustained else pk["bf16"]
+    peak_tensor = bf16 * ratio                                     # TOPS / TFLOP/s
+    ops, nbytes = cfg["ops_per_call"], bytes_per_call(cfg)
+    t_tensor_ms = ops / (peak_tensor * 1e12) * 1e3
+    t_hbm_ms = nbytes / (pk["hbm"] * 1e9) * 1e3
+    ach_tensor = ops / (kernel_ms * 1e-3) / 1e12
+    ach_hbm = nbytes / (kernel_ms * 1e-3) / 1e9
+    bound = "tensor" if t_tensor_ms >= t_hbm_ms else "hbm"
+    tunit = "TOPS" if dtype == "ci8" else "TFLOP/s"
+    traffic, traffic_source = None, None
+    if cfg["name"] in NCU_TRAFFIC and NCU_TRAFFIC[cfg["name"]][0] == kernel and not cfg.get("sharded"):
+        traffic = NCU_TRAFFIC[cfg["name"]][1]
+        traffic_source = "%s (ncu --set full capture of this kernel and geometry; NOT measured by this run)" % NCU_TRAFFIC[cfg["name"]][2]
+    return {
+        "bound": bound,
+        "achieved": ach_tensor if bound == "tensor" else ach_hbm,
+        "peak": peak_tensor if bound == "tensor" else pk["hbm"],
+        "unit": tunit if bound == "tensor" else "GB/s",
+        "frac": max(t_tensor_ms, t_hbm_ms) / kernel_ms,
+        "traffic": traffic, "traffic_source": traffic_source,
+        "kernel": KERNEL_NAMES[kernel] % (1 if dtype == "ci8" else 2), "kernel_ms": kernel_ms,
+        "roof_ms": {"tensor": t_tensor_ms, "hbm": t_hbm_ms},
+        "peak_source": "%s: bf16 %s %.1f TFLOP/s x nominal %s/bf16 ratio %.0f; HBM copy %.1f GB/s" % (
+            pk["source"], "sustained" if sustained else "burst", bf16, dtype, ratio, pk["hbm"]),
+        "tensor": {"algorithmic_ops_per_launch": ops, "achieved": ach_tensor, "unit": tunit, "peak": peak_tensor,
+                   "frac": ach_tensor / peak_tensor, "frac_of_burst": ach_tensor / (pk["bf16"] * ratio),
+                   "frac_of_sustained": ach_tensor / (pk["bf16_sustained"] * ratio),
+                   "frac_of_nominal": ach_tensor / (NOMINAL_BF16 * ratio)},
+        "hbm": {"algorithmic_bytes_per_launch": nbytes, "achieved_gbs": ach_hbm, "peak_gbs": pk["hbm"],
+                "frac": ach_hbm / pk["hbm"]},
+    }
+
+
+def sha256_tensor(t):
+    """SHA-256 of a tensor's bytes (copied to the host in 256 MiB slices)."""
+    import torch
+    h = hashlib.sha256()
+    flat = t.reshape(-1).view(torch.uint8)
+    step = 1 << 28
+    for k in range(0, flat.numel(), step):
+        h.update(flat[k:k + step].cpu().numpy().tobytes())
+    return h.hexdigest()
+
+
 # ------------------------------------------------------------------------------------------------
 # piece (a): the standalone corner-turn kernel, HBM-bound (read in + write two planes)
 # ------------------------------------------------------------------------------------------------
-def run_corner_turn(args):
+def time_corner_turn(cfg, pk, K, W):
     import torch
     from paper_1305_5639_b200 import binding, inputs
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py needs a CUDA device")
-    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
-    cfg = workload(args.workload)
-    pk = peaks()
     x = inputs.make_input(cfg, call=0, device="cuda")
-    h = binding.Correlator(cfg["N"], cfg["P"], cfg["C"], cfg["T"], cfg["dtype"])
-    ws = torch.empty((h.workspace_bytes,), dtype=torch.uint8, device="cuda")
-    K, W = args.steps, max(args.warmup, 3)
-    for _ in range(W):
-        h.corner_turn(x, ws)
-    torch.cuda.synchronize()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
-    for a, b in ev:
-        a.record(); h.corner_turn(x, ws); b.record()
-    torch.cuda.synchronize()
-    ms = sum(a.elapsed_time(b) for a, b in ev) / K
-    nbytes = cfg["in_bytes"] + h.workspace_bytes          # read the input once, write ws and ws_rot
+    with binding.Correlator(cfg["N"], cfg["P"], cfg["C"], cfg["T"], cfg["dtype"]) as h:
+        ws = torch.empty((h.workspace_bytes,), dtype=torch.uint8, device="cuda")
+        for _ in range(W):
+            h.corner_turn(x, ws)
+        torch.cuda.synchronize()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+        for a, b in ev:
+            a.record(); h.corner_turn(x, ws); b.record()
+        torch.cuda.synchronize()
+        ms = sum(a.elapsed_time(b) for a, b in ev) / K
+        nbytes = cfg["in_bytes"] + h.workspace_bytes          # read the input once, write ws and ws_rot
     gbs = nbytes / (ms * 1e-3) / 1e9
-    print(json.dumps({"metric": "corner_turn_gbs", "value": gbs, "unit": "GB/s", "n_gpus": 1, "steps": K, "warmup": W,
-                      "ms_per_step": ms, "higher_is_better": True, "dtype": "u8", "data": "synthetic",
-                      "config": {"workload": describe(cfg), "l2": "input + workspace (%.0f MiB) larger than L2" % (nbytes / 2 ** 20)},
-                      "gpu_launches": K,
-                      "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s", "frac": gbs / pk["hbm"],
-                                   "traffic": None, "kernel": "cturn::corner_turn_kernel", "kernel_ms": ms,
-                                   "algorithmic_bytes_per_launch": nbytes}}), flush=True)
+    return {"metric": "corner_turn_gbs", "value": gbs, "unit": "GB/s", "n_gpus": 1, "steps": K, "warmup": W,
+            "ms_per_step": ms, "higher_is_better": True, "dtype": "u8", "data": "synthetic",
+            "config": {"workload": describe(cfg), "l2": "input + workspace (%.0f MiB) larger than L2" % (nbytes / 2 ** 20)},
+            "gpu_launches": K,
+            "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s", "frac": gbs / pk["hbm"],
+                         "traffic": None, "kernel": "cturn::corner_turn_kernel", "kernel_ms": ms,
+                         "algorithmic_bytes_per_launch": nbytes}}
 
 
-def run_fengine(args):
+def time_fengine(pk, K, W, M=512, A=8192):
     """corr_fengine alone: HBM-bound (1 byte read + 2 bytes written per real sample)."""
     import torch
     from paper_1305_5639_b200 import binding
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py needs a CUDA device")
-    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
-    pk = peaks()
-    M, A = 512, 8192
     g = torch.Generator(device="cuda"); g.manual_seed(1700)
     s = torch.clamp(torch.round(torch.randn((M, A * 256), generator=g, device="cuda") * 20.0), -127, 127).to(torch.int8)
     out = binding.fengine(s)
-    K, W = args.steps, max(args.warmup, 3)
     for _ in range(W):
         binding.fengine(s, out)
     torch.cuda.synchronize()
@@ -333,16 +423,130 @@ def run_fengine(args):
     ms = sum(a.elapsed_time(b) for a, b in ev) / K
     nbytes = s.numel() + out.numel() * 2
     gbs = nbytes / (ms * 1e-3) / 1e9
-    print(json.dumps({"metric": "fengine_gbs", "value": gbs, "unit": "GB/s", "n_gpus": 1, "steps": K, "warmup": W,
-                      "ms_per_step": ms, "higher_is_better": True, "dtype": "f32", "data": "synthetic",
-                      "config": {"workload": "F-engine: %d streams x %d spectra of 256 real int8 samples (sigma 20) -> 128 complex fp16 "
-                                             "channels in the X-engine layout" % (M, A),
-                                 "l2": "input + output (%.0f MiB) larger than L2" % (nbytes / 2 ** 20),
-                                 "gsamples_per_s": s.numel() / (ms * 1e-3) / 1e9},
-                      "gpu_launches": K,
-                      "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s", "frac": gbs / pk["hbm"],
-                                   "traffic": None, "kernel": "feng::fengine_kernel", "kernel_ms": ms,
-                                   "algorithmic_bytes_per_launch": nbytes}}), flush=True)
+    return {"metric": "fengine_gbs", "value": gbs, "unit": "GB/s", "n_gpus": 1, "steps": K, "warmup": W,
+            "ms_per_step": ms, "higher_is_better": True, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "F-engine: %d streams x %d spectra of 256 real int8 samples (sigma 20) -> 128 complex fp16 "
+                                   "channels in the X-engine layout" % (M, A),
+                       "l2": "input + output (%.0f MiB) larger than L2" % (nbytes / 2 ** 20),
+                       "gsamples_per_s": s.numel() / (ms * 1e-3) / 1e9},
+            "gpu_launches": K,
+            "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s", "frac": gbs / pk["hbm"],
+                         "traffic": None, "kernel": "feng::fengine_kernel", "kernel_ms": ms,
+                         "algorithmic_bytes_per_launch": nbytes}}
+
+
+def run_piece(args):
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device")
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    K, W = args.steps, max(args.warmup, 3)
+    rec = time_corner_turn(workload(args.workload), peaks(), K, W) if args.piece == "corner_turn" else time_fengine(peaks(), K, W)
+    print(json.dumps(rec), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------
+# timing of one X-engine workload on resident inputs
+# ------------------------------------------------------------------------------------------------
+class Resident:
+    """A workload with its inputs resident in HBM and a plan on them."""
+
+    def __init__(self, cfg, kernel="auto", window=None):
+        import torch
+        from paper_1305_5639_b200 import binding, inputs
+        self.cfg, self.torch = cfg, torch
+        self.cross = bool(cfg.get("Nb"))
+        self.xs = [inputs.make_input(cfg, call=k, device="cuda") for k in range(cfg["calls"])]
+        self.xbs = [inputs.make_input_b(cfg, call=k, device="cuda") for k in range(cfg["calls"])] if self.cross else None
+        N, P, C, T, dtype = cfg["N"], cfg["P"], cfg["C"], cfg["T"], cfg["dtype"]
+        self.h = (binding.CrossCorrelator(N, cfg["Nb"], P, C, T, dtype) if self.cross
+                  else binding.Correlator(N, P, C, T, dtype, window=window))
+        if kernel != "auto":
+            self.h.set_kernel(kernel)
+        self.out = self.h.empty_output()
+        # inputs smaller than ~4x L2 (126 MB) are (partly) re-read from L2 unless it is flushed between steps
+        self.flush = None
+        if cfg["in_bytes"] * cfg["calls"] < 512 * 2 ** 20:
+            self.flush = torch.empty(256 * 2 ** 20, dtype=torch.uint8, device="cuda")
+
+    def step(self, ev=None):
+        for k in range(self.cfg["calls"]):
+            if ev is not None:
+                ev[2 * k].record()
+            if self.cross:
+                self.h.xengine_cross(self.xs[k], self.xbs[k], self.out, accumulate=k > 0)
+            else:
+                self.h.xengine(self.xs[k], self.out, accumulate=k > 0)
+            if ev is not None:
+                ev[2 * k + 1].record()
+
+    def timed(self, K, cold=True):
+        """K steps, per-call CUDA events on the launching stream -> list of per-call ms (flush kernels excluded)."""
+        torch, calls = self.torch, self.cfg["calls"]
+        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(2 * calls)] for _ in range(K)]
+        for s in range(K):
+            if cold and self.flush is not None:
+                self.flush.fill_(s & 1)
+            self.step(evs[s])
+        torch.cuda.synchronize()
+        return [evs[s][2 * k].elapsed_time(evs[s][2 * k + 1]) for s in range(K) for k in range(calls)]
+
+    def close(self):
+        self.h.close()
+        self.xs = self.xbs = self.out = self.flush = None
+        self.torch.cuda.empty_cache()
+
+
+def short_run(name, pk, K=10, W=3, sha=True):
+    """A short run of another workload for the `workloads` list of the headline line."""
+    cfg = workload(name)
+    r = Resident(cfg)
+    try:
+        for _ in range(W):
+            if r.flush is not None:
+                r.flush.fill_(1)
+            r.step()
+        r.torch.cuda.synchronize()
+        ms = r.timed(K, cold=True)
+        kernel_ms = sum(ms) / len(ms)
+        rec = {"workload": describe(cfg), "kernel": r.h.kernel, "steps": K, "ms_per_call": kernel_ms,
+               "value": cfg["ops_per_call"] / (kernel_ms * 1e-3) / 1e12, "unit": UNIT,
+               "visibilities_per_s": cfg["C"] * cfg["n_baseline"] * cfg["P"] ** 2 / (kernel_ms * 1e-3),
+               "l2": "flushed between steps (cold)" if r.flush is not None else "inputs larger than L2",
+               "roofline": roofline_record(cfg, r.h.kernel, kernel_ms, pk, sustained=False)}
+        if r.flush is not None:                                  # small inputs: also the L2-warm figure
+            warm = r.timed(K, cold=False)
+            wms = sum(warm) / len(warm)
+            rec["l2_warm"] = {"ms_per_call": wms, "value": cfg["ops_per_call"] / (wms * 1e-3) / 1e12, "unit": UNIT}
+        if sha:
+            rec["input_sha256"] = [sha256_tensor(x) for x in r.xs]
+        return rec
+    finally:
+        r.close()
+
+
+def dumps_run(pk, K=10, W=3):
+    """Short-integration mode (corr_xengine_dumps): N=256, C=256, T=2048 in 16 integrations of 128 samples."""
+    import torch
+    from paper_1305_5639_b200 import binding, inputs
+    N, P, C, T, nd = 256, 2, 256, 2048, 16
+    x = inputs.gauss_ci8(T, C, N, P, 20.0, seed=1800, device="cuda")
+    with binding.Correlator(N, P, C, T, "ci8") as h:
+        out = h.xengine_dumps(x, nd)
+        for _ in range(W):
+            h.xengine_dumps(x, nd, out)
+        torch.cuda.synchronize()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+        for a, b in ev:
+            a.record(); h.xengine_dumps(x, nd, out); b.record()
+        torch.cuda.synchronize()
+    ms = sum(a.elapsed_time(b) for a, b in ev) / K
+    ops = 8.0 * C * T * (N * (N + 1) // 2) * P * P
+    nbytes = x.numel() + out.numel() * 4
+    return {"workload": "dumps: N=%d, %d pol, %d channels, T=%d cut into %d integrations of %d samples, int8" % (N, P, C, T, nd, T // nd),
+            "ms_per_call": ms, "value": ops / (ms * 1e-3) / 1e12, "unit": UNIT,
+            "hbm": {"algorithmic_bytes_per_launch": nbytes, "achieved_gbs": nbytes / (ms * 1e-3) / 1e9,
+                    "frac": nbytes / (ms * 1e-3) / 1e9 / pk["hbm"]}}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -351,7 +555,7 @@ def run_fengine(args):
 def run_native(args):
     import torch
     import torch.distributed as dist
-    from paper_1305_5639_b200 import binding, inputs
+    from paper_1305_5639_b200 import binding
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -365,98 +569,92 @@ def run_native(args):
 
     cfg = workload(args.workload)
     sharded = args.shard == "channels" and world > 1
+    window = None
+    share = 1.0                                     # this rank's share of the workload's ops / bytes
     if sharded:
-        # this rank owns a contiguous block of channels: a smaller, otherwise identical problem with its own output slab
+        # every rank holds the SAME seeded whole-band input and a whole-band output; its window plan integrates its
+        # contiguous block of channels in place (corr_create_window) -- one workload, disjoint output slabs, no collective
         from paper_1305_5639_b200.shard import channel_range
+        if cfg.get("Nb"):
+            raise RuntimeError("--shard channels applies to the triangle workloads")
         c0, c1 = channel_range(cfg["C"], world, rank)
-        frac = (c1 - c0) / cfg["C"]
-        for key in ("cmacs_per_call", "ops_per_call", "in_bytes", "out_bytes"):
-            cfg[key] = int(cfg[key] * frac)
-        cfg["C_total"], cfg["C"] = cfg["C"], c1 - c0
-        cfg["seed"] = cfg["seed"] + 7 * rank            # each slab gets its own noise
-    N, P, C, T, dtype, calls = cfg["N"], cfg["P"], cfg["C"], cfg["T"], cfg["dtype"], cfg["calls"]
+        window = (c0, c1 - c0) if c1 > c0 else None
+        share = (c1 - c0) / cfg["C"]
+        cfg["sharded"] = True
+    P, C, dtype, calls = cfg["P"], cfg["C"], cfg["dtype"], cfg["calls"]
     K, W = args.steps, max(args.warmup, 3)
     pk = peaks()
+    idle = sharded and window is None               # more ranks than channels: this rank has nothing to integrate
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    # every rank is an independent replica on its own seeded inputs (replicas only; no sharding)
-    xs = [inputs.make_input(cfg, call=k, device="cuda") for k in range(calls)]
-    cross = bool(cfg.get("Nb"))
-    xbs = [inputs.make_input_b(cfg, call=k, device="cuda") for k in range(calls)] if cross else None
-    h = binding.CrossCorrelator(N, cfg["Nb"], P, C, T, dtype) if cross else binding.Correlator(N, P, C, T, dtype)
-    if args.kernel != "auto":
-        h.set_kernel(args.kernel)
-    kernel = h.kernel
-    if not h.uses_tensor_cores and args.kernel != "simt":
+    r = None if idle else Resident(cfg, args.kernel, window)
+    kernel = "pair" if idle else r.h.kernel
+    if r is not None and not r.h.uses_tensor_cores and args.kernel != "simt":
         raise RuntimeError("workload %s does not run on the tcgen05 kernel" % cfg["name"])
-    out = h.empty_output()
-    # inputs smaller than L2 (126 MB) are re-read from DRAM only if L2 is flushed between steps
-    flush = None
-    in_total = cfg["in_bytes"] * calls
-    if in_total < 512 * 2 ** 20:
-        flush = torch.empty(256 * 2 ** 20, dtype=torch.uint8, device="cuda")
-
-    def step(ev=None):
-        for k in range(calls):
-            if ev is not None:
-                ev[2 * k].record()
-            if cross:
-                h.xengine_cross(xs[k], xbs[k], out, accumulate=k > 0)
-            else:
-                h.xengine(xs[k], out, accumulate=k > 0)
-            if ev is not None:
-                ev[2 * k + 1].record()
-
     for _ in range(W):
-        if flush is not None:
-            flush.fill_(1)
-        step()
-    launches_per_call = h.last_launch_count
+        if r is not None:
+            if r.flush is not None:
+                r.flush.fill_(1)
+            r.step()
+    launches_per_call = 0 if idle else r.h.last_launch_count
     barrier()
 
     # ---- timed region: device-resident inputs ---------------------------------------------------
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(2 * calls)] for _ in range(K)]
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
         time.sleep(0.25)
     barrier()
     w0 = time.time()
-    for s in range(K):
-        if flush is not None:
-            flush.fill_(s & 1)
-        step(evs[s])
+    call_ms = [] if idle else r.timed(K, cold=True)
     barrier()
     w1 = time.time()
     clocks = sampler.stop(w0, w1) if rank == 0 else None
-    call_ms = [evs[s][2 * k].elapsed_time(evs[s][2 * k + 1]) for s in range(K) for k in range(calls)]
-    step_ms = [sum(call_ms[s * calls:(s + 1) * calls]) for s in range(K)]
-    total_ms = sum(step_ms)          # device time of exactly K steps (flush kernels excluded)
-    total_ms = max_over_ranks(total_ms, dist, world, "cuda")
+    total_ms = max_over_ranks(sum(call_ms), dist, world, "cuda")          # device time of exactly K steps, slowest rank
     ops_step = cfg["ops_per_call"] * calls
     if sharded:
-        # strong scaling: the job is ONE workload; sum the ranks' (nearly equal) shares
-        t_ops = torch.tensor([float(ops_step)], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t_ops, op=dist.ReduceOp.SUM)
-        value = whole_job_value(float(t_ops.item()), K, 1, total_ms) / 1e12
+        value = whole_job_value(ops_step, K, 1, total_ms) / 1e12          # strong scaling: the job is ONE workload
     else:
         value = whole_job_value(ops_step, K, world, total_ms) / 1e12
-    kernel_ms = sum(call_ms) / len(call_ms)          # average launch duration of the dominant (only) kernel
+    kernel_ms = sum(call_ms) / max(1, len(call_ms))          # average launch duration of the dominant (only) kernel
+
+    # ---- sustained: the same step back to back for >= 2 s (power-capped clocks), its own clock record -----------
+    sustained = None
+    if not args.no_sustained and not idle:
+        est = max(kernel_ms * calls, 1e-3)
+        Ks = max(K, int(2200.0 / est) + 1)
+        s2 = ClockSampler(local)
+        if rank == 0:
+            s2.start()
+            time.sleep(0.1)
+        barrier()
+        t0 = time.time()
+        ms2 = r.timed(Ks, cold=True)
+        barrier()
+        t1 = time.time()
+        tot2 = max_over_ranks(sum(ms2), dist, world, "cuda")
+        k_ms = sum(ms2) / len(ms2)
+        sustained = {"steps": Ks, "seconds": tot2 * 1e-3, "ms_per_step": tot2 / Ks,
+                     "value": whole_job_value(ops_step, Ks, 1 if sharded else world, tot2) / 1e12, "unit": UNIT,
+                     "clocks": s2.stop(t0, t1) if rank == 0 else None,
+                     "roofline": None if sharded else roofline_record(cfg, kernel, k_ms, pk, sustained=True)}
 
     # ---- e2e: HOST pinned buffers through corr_xengine_host --------------------------------------
-    e2e = None
-    if not args.no_e2e and not cross:          # the host-buffer entry point exists for corr_xengine only
+    e2e, sha = None, None
+    if not args.no_e2e and not r is None and not r.cross and not sharded:
         Ke = args.e2e_steps or min(K, 5)
-        xh = [x.cpu().pin_memory() for x in xs]
-        oh = torch.empty(h.output_shape(), dtype=out.dtype).pin_memory()
+        xh = [x.cpu().pin_memory() for x in r.xs]
+        oh = torch.empty(r.h.output_shape(), dtype=r.out.dtype).pin_memory()
+        if not args.no_sha and rank == 0:
+            sha = [hashlib.sha256(x.numpy()).hexdigest() for x in xh]
 
         def host_step():
             for k in range(calls):
-                h.xengine_host(xh[k], oh if k == calls - 1 else None, accumulate=k > 0)
+                r.h.xengine_host(xh[k], oh if k == calls - 1 else None, accumulate=k > 0)
 
         host_step()
         barrier()
@@ -469,39 +667,26 @@ def run_native(args):
             dist.all_reduce(te, op=dist.ReduceOp.MAX)
         e2e = {"value": world * Ke * ops_step / float(te.item()) / 1e12, "unit": UNIT,
                "h2d_bytes_per_step": cfg["in_bytes"] * calls, "d2h_bytes_per_step": cfg["out_bytes"],
-               "steps": Ke, "ms_per_step": 1e3 * float(te.item()) / Ke}
-        if not torch.equal(oh.cuda(), out):
+               "steps": Ke, "ms_per_step": 1e3 * float(te.item()) / Ke,
+               "how": "corr_xengine_host: 8 channel windows per call through an H2D / kernel / D2H pipeline on 3 streams"}
+        r.step()
+        torch.cuda.synchronize()
+        if not torch.equal(oh.cuda(), r.out):
             raise RuntimeError("host-buffer leg and device leg disagree")
         del xh, oh
+    elif not args.no_sha and rank == 0 and r is not None:
+        sha = [sha256_tensor(x) for x in r.xs]
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel ----------------------------------------------------------
-    ratio = NOMINAL_RATIO[dtype]
-    # a kernel timed back to back for longer than ~0.25 s runs under the 1 kW power cap: sustained peak; else burst
-    sustained = total_ms > 250.0
-    peak = (pk["bf16_sustained"] if sustained else pk["bf16"]) * ratio
-    achieved = cfg["ops_per_call"] / (kernel_ms * 1e-3) / 1e12
-    acc_calls = calls - 1
-    bytes_call = cfg["in_bytes"] + cfg["out_bytes"] * (1.0 + acc_calls / calls)      # avg over the step's calls
-    roofline = {
-        "bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TOPS" if dtype == "ci8" else "TFLOP/s",
-        "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg["name"]),
-        "kernel": {"single": "xtc::xengine_direct_kernel<%d>", "pair": "xtc::xengine_pair_kernel<%d, 1>",
-                   "quad": "xtc::xengine_pair_kernel<%d, 2>", "simt": "xsimt::xengine_simt_kernel<%d>"}[kernel]
-                  % (1 if dtype == "ci8" else 2), "kernel_ms": kernel_ms,
-        "peak_source": "%s bf16 %s %.1f TFLOP/s x nominal %s/bf16 ratio %.0f" % (
-            pk["source"], "sustained" if sustained else "burst", pk["bf16_sustained"] if sustained else pk["bf16"], dtype, ratio),
-        "frac_of_burst": achieved / (pk["bf16"] * ratio),
-        "frac_of_sustained": achieved / (pk["bf16_sustained"] * ratio),
-        "frac_of_nominal": achieved / (2250.0 * ratio),
-        "algorithmic_ops_per_launch": cfg["ops_per_call"],
-        "hbm": {"algorithmic_bytes_per_launch": bytes_call, "achieved_gbs": bytes_call / (kernel_ms * 1e-3) / 1e9,
-                "peak_gbs": pk["hbm"], "frac": bytes_call / (kernel_ms * 1e-3) / 1e9 / pk["hbm"]},
-    }
+    # ---- roofline of the dominant kernel: the timed region above decides burst vs sustained peaks -------------------
+    # (a kernel timed back to back for longer than ~0.25 s runs under the 1 kW power cap: sustained peak; else burst)
+    roofline = roofline_record(cfg, kernel, kernel_ms / max(share, 1e-9) if sharded else kernel_ms, pk, sustained=total_ms > 250.0)
+    if sharded:
+        roofline["note"] = "channel-sharded: kernel_ms scaled to the whole workload (this rank integrated %.3f of it)" % share
 
     # ---- the library GEMM of the same dtype, same protocol as MEASURED_PEAKS.json (context, not the denominator) --
     if world == 1 and not args.no_gemm_peak:
@@ -511,26 +696,43 @@ def run_native(args):
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         import oracle
-        cores = oracle.max_threads()
-        n_chan = max(1, min(C, cores))
-        x_host = xs[0][:, :n_chan].contiguous().cpu().numpy()      # the same bytes the GPU consumed
-        xb_host = xbs[0][:, :n_chan].contiguous().cpu().numpy() if cross else None
-        rate, secs, done = oracle_sample_rate(cfg, x_host, min_seconds=10.0, xb_host=xb_host)
-        cpu = {"value": 8.0 * rate / 1e12, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": "channels 0..%d of call 0 (all %d baselines x %d pol products, full T=%d), %d channel passes in %.1f s"
-                         % (n_chan - 1, cfg["n_baseline"], P * P, T, done, secs),
-               "gcmac_per_s": rate / 1e9}
+        n_chan = max(1, min(C, oracle.max_threads()))
+        x_host = r.xs[0][:, :n_chan].contiguous().cpu().numpy()      # the same bytes the GPU consumed
+        xb_host = r.xbs[0][:, :n_chan].contiguous().cpu().numpy() if r.cross else None
+        cpu = cpu_baseline_record(cfg, x_host, xb_host)
+
+    in_total = cfg["in_bytes"] * calls
+    flushed = r is not None and r.flush is not None
+    if r is not None:
+        r.close()
+
+    # ---- every other config point and piece, briefly (N = 1 only), so the driver-run line carries them --------------
+    others = None
+    if world == 1 and not args.no_others and args.workload == "cfg4" and args.kernel == "auto":
+        others = []
+        for name in ["cfg1", "cfg2", "cfg3"] + ["cfg5_n%d" % n for n in (32, 64, 128, 256, 512, 1024)] + ["cross_n256"]:
+            try:
+                others.append(short_run(name, pk, sha=not args.no_sha))
+            except Exception as e:                                    # a failed side run must not lose the headline
+                others.append({"workload": name, "error": repr(e)})
+        for fn in (lambda: dumps_run(pk), lambda: time_corner_turn(workload("cfg4"), pk, 10, 3), lambda: time_fengine(pk, 10, 3)):
+            try:
+                others.append(fn())
+            except Exception as e:
+                others.append({"error": repr(e)})
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
         "dtype": "s8 x s8 -> s32" if dtype == "ci8" else "f16 x f16 -> f32", "data": "synthetic",
-        "config": {"workload": describe(cfg), "l2": ("flushed between steps" if flush is not None else
+        "config": {"workload": describe(cfg), "l2": ("flushed between steps" if flushed else
                                                      "inputs (%.0f MiB per step) larger than L2" % (in_total / 2 ** 20)),
-                   "parallelism": ("channels sharded over %d ranks, no collective" % world) if sharded else "replicas only (x%d)" % world, "visibilities_per_s": world * K * C * cfg["n_baseline"] * P * P
-                   / (total_ms * 1e-3)},
+                   "parallelism": ("channel windows of one workload over %d ranks, no collective" % world) if sharded
+                   else "replicas only (x%d)" % world,
+                   "visibilities_per_s": (1 if sharded else world) * K * C * cfg["n_baseline"] * P * P / (total_ms * 1e-3),
+                   "input_sha256": sha},
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_call * calls * K,
-        "roofline": roofline, "cpu_baseline": cpu,
+        "roofline": roofline, "sustained": sustained, "cpu_baseline": cpu, "workloads": others,
     }
     print(json.dumps(line), flush=True)
     if world > 1:
@@ -541,10 +743,8 @@ def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
-    elif args.piece == "corner_turn":
-        run_corner_turn(args)
-    elif args.piece == "fengine":
-        run_fengine(args)
+    elif args.piece != "xengine":
+        run_piece(args)
     else:
         run_native(args)
 

@@ -13,6 +13,7 @@ import tempfile
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "xengine_oracle.c")
 LIB = os.path.join(HERE, "libxoracle.so")
+CFLAGS = ["-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra"]
 
 
 def _stale():
@@ -30,7 +31,7 @@ def build(force: bool = False) -> str:
                 return LIB
             fd, tmp = tempfile.mkstemp(prefix="libxoracle.", suffix=".so.tmp", dir=HERE)
             os.close(fd)
-            cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra", SRC, "-o", tmp, "-lm"]
+            cmd = ["gcc"] + CFLAGS + [SRC, "-o", tmp, "-lm"]
             subprocess.run(cmd, check=True)
             os.chmod(tmp, 0o755)
             os.replace(tmp, LIB)
