@@ -129,88 +129,137 @@ __device__ __forceinline__ void combine_chunk(const uint32_t (&v)[32], int ri, u
 
 // Drain one TMEM accumulator pass of one tile through this epilogue warp: tcgen05.ld -> Re/Im combine ->
 // packed-baseline writer (+ accumulate).  The warp owns TMEM lanes [32 quarter, +32) = G rows u0 .. u0 + 31 of
-// output slab c (global channel, or integration * n_chan_total + channel) and the tile columns [h_begin, h_end) (G columns col0 + h); `taddr` addresses lane 32 quarter,
-// column 0 of the accumulator.  `release_bar` is arrived on (by lane 0; `kRemote`: it lives in the pair leader
-// CTA and is a shared::cluster address) as soon as the warp's last TMEM column is in registers.
-// first_pass: no earlier pass of this tile wrote the same output addresses (else wait for those writes).
-template <bool kFloat, bool kRemote, int kBufs = 2>
+// output slab c (global channel, or integration * n_chan_total + channel) and the tile columns [h_begin, h_end)
+// (G columns col0 + h; at most 128 of them); `taddr` addresses lane 32 quarter, column 0 of the accumulator.
+// `release_bar` is arrived on (by lane 0; `kRemote`: it lives in the pair leader CTA and is a shared::cluster address)
+// as soon as the warp's last TMEM column is in registers.
+//
+// kFold (fp16 path, several TMEM passes per tile): the passes of one tile are summed in REGISTERS with IEEE
+// round-to-nearest fp32 adds and only the last pass touches memory:
+//   kFoldNone  single pass: combine -> stage -> store / reduce-add
+//   kFoldAdd   run[] += this pass; nothing is written
+//   kFoldLast  this pass + run[] -> stage -> store / reduce-add
+// run[k]: the warp's (re, im) values in the order they are produced: 32-column chunk q (0..3), then re[0..7], im[0..7].
+enum { kFoldNone = 0, kFoldAdd = 1, kFoldLast = 2 };
+
+template <bool kFloat, int kFold>
+__device__ __forceinline__ void fold_chunk(uint32_t (&re)[8], uint32_t (&im)[8], float (&run)[64], int q) {
+    if constexpr (kFloat && kFold != kFoldNone) {
+#pragma unroll
+        for (int y = 0; y < 8; ++y) {
+            const float r = __uint_as_float(re[y]) + run[q * 16 + y];
+            const float i = __uint_as_float(im[y]) + run[q * 16 + 8 + y];
+            if constexpr (kFold == kFoldAdd) {
+                run[q * 16 + y] = r;
+                run[q * 16 + 8 + y] = i;
+            } else {
+                re[y] = __float_as_uint(r);
+                im[y] = __float_as_uint(i);
+            }
+        }
+    }
+}
+
+template <bool kFloat, bool kRemote, int kBufs, int kFold>
 __device__ __forceinline__ void drain_accumulator(const Params& prm, int c, int u0, int col0, int h_begin, int h_end,
-                                                  uint32_t taddr, uint32_t release_bar, bool reduce, bool first_pass,
-                                                  uint32_t stage_smem, int& buf, int lane) {
-    auto release = [](uint32_t bar) {
-        if constexpr (kRemote) ptx::mbar_arrive_cluster(bar);
-        else ptx::mbar_arrive(bar);
+                                                  uint32_t taddr, uint32_t release_bar, bool reduce,
+                                                  uint32_t stage_smem, int& buf, int lane, float (&run)[64]) {
+    auto release = [&]() {
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) {
+            if constexpr (kRemote) ptx::mbar_arrive_cluster(release_bar);
+            else ptx::mbar_arrive(release_bar);
+        }
     };
     const int P = prm.n_pol;
     const int ri = lane & 1;                     // row parity: 0 = re row (u even), 1 = im row
     uint8_t* out8 = static_cast<uint8_t*>(prm.out);
-    struct { int col0; } td{col0};
-    const int kc = first_pass ? 0 : 1;
     const bool rect = prm.n_station_b > 0;
     const uint64_t policy = ptx::policy_evict_first();
+    if (h_begin >= h_end) {                      // nothing in this column half: just release
+        release();
+        return;
+    }
     if (P == 2) {
         // ---- fast path: station rows are 32-byte aligned runs; bulk async store / reduce-add ----
         const int il = lane >> 2;                        // station within the warp's 8
         const int p = (lane >> 1) & 1;
         const int i_row = (u0 >> 2) + lane;              // lanes 0..7: the station row this lane ships
-        // chunk kc - 1 wrote the same addresses: its bulk operations must be complete (not just read)
-        if (kc != 0 && lane < 8) ptx::bulk_wait<0>();
-        if (h_begin >= h_end) {                          // nothing in this column half: just release
-            ptx::tc_fence_before();
-            __syncwarp();
-            if (lane == 0) release(release_bar);
-        }
-        for (int h0 = h_begin; h0 < h_end; h0 += kEpiCols) {
-            if (lane < 8) ptx::bulk_wait_read<kBufs - 1>();   // staging[buf] (kBufs passes ago) has been read
-            __syncwarp();
+#pragma unroll
+        for (int it = 0; it < (kTileCols / 2) / kEpiCols; ++it) {
+            const int h0 = h_begin + it * kEpiCols;
+            if (h0 >= h_end) continue;                   // (no break: the loop must unroll so that run[] stays in registers)
             const uint32_t sbuf = stage_smem + buf * kEpiBufBytes;
-            // both 32-column TMEM loads of the pass are issued before the first wait (latency overlap)
-            uint32_t v0[32], v1[32];
-            const bool two = h0 + 32 < h_end;
-            ptx::tmem_ld_32x32(taddr + h0, v0);
-            if (two) ptx::tmem_ld_32x32(taddr + h0 + 32, v1);
-            ptx::tmem_ld_wait();
-            if (h0 + kEpiCols >= h_end) {                // all of this warp's columns are in registers
-                ptx::tc_fence_before();
+            if constexpr (kFold != kFoldAdd) {
+                if (lane < 8) ptx::bulk_wait_read<kBufs - 1>();   // staging[buf] (kBufs passes ago) has been read
                 __syncwarp();
-                if (lane == 0) release(release_bar);
             }
-            {
-                uint32_t re[8], im[8];
-                combine_chunk<kFloat>(v0, ri, re, im);
-                // (i, p) x (j = j0 + 8 half + y, q = ri): byte offset j*32 + p*16 + q*8 in the station row
-                const uint32_t dst = sbuf + il * kEpiRowBytes + p * 16 + ri * 8;
+            const bool two = h0 + 32 < h_end;
+            if constexpr (kFold == kFoldNone) {
+                // both 32-column TMEM loads of the pass are issued before the first wait (latency overlap)
+                uint32_t v0[32], v1[32];
+                ptx::tmem_ld_32x32(taddr + h0, v0);
+                if (two) ptx::tmem_ld_32x32(taddr + h0 + 32, v1);
+                ptx::tmem_ld_wait();
+                if (h0 + kEpiCols >= h_end) release();       // all of this warp's columns are in registers
+                {
+                    uint32_t re[8], im[8];
+                    combine_chunk<kFloat>(v0, ri, re, im);
+                    // (i, p) x (j = j0 + 8 half + y, q = ri): byte offset j*32 + p*16 + q*8 in the station row
+                    const uint32_t dst = sbuf + il * kEpiRowBytes + p * 16 + ri * 8;
 #pragma unroll
-                for (int y = 0; y < 8; ++y) ptx::st_shared_v2(dst + y * 32, re[y], im[y]);
-            }
-            if (two) {
-                uint32_t re[8], im[8];
-                combine_chunk<kFloat>(v1, ri, re, im);
-                const uint32_t dst = sbuf + il * kEpiRowBytes + 256 + p * 16 + ri * 8;
-#pragma unroll
-                for (int y = 0; y < 8; ++y) ptx::st_shared_v2(dst + y * 32, re[y], im[y]);
-            }
-            ptx::fence_proxy_async_smem();               // generic-proxy writes -> visible to the bulk copy
-            __syncwarp();
-            if (lane < 8) {
-                const int j0 = (td.col0 + h0) >> 2;                       // first station of this pass
-                int cnt = (h_end - h0) >> 2;                              // stations staged in this pass
-                if (cnt > kEpiCols / 4) cnt = kEpiCols / 4;
-                const int j_end = rect ? prm.n_station_b : i_row + 1;     // triangle: j <= i; rectangle: every j of group B
-                if (cnt > j_end - j0) cnt = j_end - j0;
-                if (i_row < prm.n_station && cnt > 0) {
-                    const long long row = rect ? (static_cast<long long>(c) * prm.n_station + i_row) * prm.n_station_b
-                                               : static_cast<long long>(c) * prm.n_baseline + static_cast<long long>(i_row) * (i_row + 1) / 2;
-                    uint8_t* dst = out8 + ((row + j0) << 5);
-                    const uint32_t src = sbuf + lane * kEpiRowBytes;
-                    const uint32_t bytes = static_cast<uint32_t>(cnt) << 5;
-                    if (!reduce) ptx::bulk_store(dst, src, bytes, policy);
-                    else if constexpr (kFloat) ptx::bulk_reduce_add_f32(dst, src, bytes, policy);
-                    else ptx::bulk_reduce_add_s32(dst, src, bytes, policy);
+                    for (int y = 0; y < 8; ++y) ptx::st_shared_v2(dst + y * 32, re[y], im[y]);
                 }
-                ptx::bulk_commit();
+                if (two) {
+                    uint32_t re[8], im[8];
+                    combine_chunk<kFloat>(v1, ri, re, im);
+                    const uint32_t dst = sbuf + il * kEpiRowBytes + 256 + p * 16 + ri * 8;
+#pragma unroll
+                    for (int y = 0; y < 8; ++y) ptx::st_shared_v2(dst + y * 32, re[y], im[y]);
+                }
+            } else {
+                // folding passes keep 64 running sums per thread: one 32-column chunk at a time (register budget: 168)
+#pragma unroll
+                for (int q = 0; q < 2; ++q) {
+                    if (q == 1 && !two) continue;
+                    uint32_t v[32];
+                    ptx::tmem_ld_32x32(taddr + h0 + 32 * q, v);
+                    ptx::tmem_ld_wait();
+                    if (h0 + 32 * (q + 1) >= h_end) release();
+                    uint32_t re[8], im[8];
+                    combine_chunk<kFloat>(v, ri, re, im);
+                    fold_chunk<kFloat, kFold>(re, im, run, 2 * it + q);
+                    if constexpr (kFold == kFoldLast) {
+                        const uint32_t dst = sbuf + il * kEpiRowBytes + 256 * q + p * 16 + ri * 8;
+#pragma unroll
+                        for (int y = 0; y < 8; ++y) ptx::st_shared_v2(dst + y * 32, re[y], im[y]);
+                    }
+                }
             }
-            if (kBufs == 2) buf ^= 1;
+            if constexpr (kFold != kFoldAdd) {
+                ptx::fence_proxy_async_smem();               // generic-proxy writes -> visible to the bulk copy
+                __syncwarp();
+                if (lane < 8) {
+                    const int j0 = (col0 + h0) >> 2;                          // first station of this pass
+                    int cnt = (h_end - h0) >> 2;                              // stations staged in this pass
+                    if (cnt > kEpiCols / 4) cnt = kEpiCols / 4;
+                    const int j_end = rect ? prm.n_station_b : i_row + 1;     // triangle: j <= i; rectangle: every j of group B
+                    if (cnt > j_end - j0) cnt = j_end - j0;
+                    if (i_row < prm.n_station && cnt > 0) {
+                        const long long row = rect ? (static_cast<long long>(c) * prm.n_station + i_row) * prm.n_station_b
+                                                   : static_cast<long long>(c) * prm.n_baseline + static_cast<long long>(i_row) * (i_row + 1) / 2;
+                        uint8_t* dst = out8 + ((row + j0) << 5);
+                        const uint32_t src = sbuf + lane * kEpiRowBytes;
+                        const uint32_t bytes = static_cast<uint32_t>(cnt) << 5;
+                        if (!reduce) ptx::bulk_store(dst, src, bytes, policy);
+                        else if constexpr (kFloat) ptx::bulk_reduce_add_f32(dst, src, bytes, policy);
+                        else ptx::bulk_reduce_add_s32(dst, src, bytes, policy);
+                    }
+                    ptx::bulk_commit();
+                }
+                if (kBufs == 2) buf ^= 1;
+            }
         }
     } else {
         // ---- general path (n_pol == 1): per-visibility 8-byte stores ----
@@ -223,38 +272,67 @@ __device__ __forceinline__ void drain_accumulator(const Params& prm, int c, int 
         const long long row_base = (row * P + p) * P * 2;
         const int n_cols = rect ? prm.M_b : prm.M;
         uint32_t* out = static_cast<uint32_t*>(prm.out);
-        if (h_begin >= h_end) {
-            ptx::tc_fence_before();
-            __syncwarp();
-            if (lane == 0) release(release_bar);
-        }
-        for (int h0 = h_begin; h0 < h_end; h0 += 32) {
+#pragma unroll
+        for (int it = 0; it < (kTileCols / 2) / 32; ++it) {
+            const int h0 = h_begin + it * 32;
+            if (h0 >= h_end) continue;
             uint32_t v[32];
             ptx::tmem_ld_32x32(taddr + h0, v);
             ptx::tmem_ld_wait();
-            if (h0 + 32 >= h_end) {
-                ptx::tc_fence_before();
-                __syncwarp();
-                if (lane == 0) release(release_bar);
-            }
+            if (h0 + 32 >= h_end) release();
             uint32_t re[8], im[8];
             combine_chunk<kFloat>(v, ri, re, im);
-            const int n0 = (td.col0 + h0) >> 1;
+            fold_chunk<kFloat, kFold>(re, im, run, it);
+            if constexpr (kFold != kFoldAdd) {
+                const int n0 = (col0 + h0) >> 1;
 #pragma unroll
-            for (int y = 0; y < 8; ++y) {
-                const int n = n0 + 2 * y + ri;
-                const int j = n / P, q = n - j * P;
-                if (row_ok && n < n_cols && (rect || j <= i)) {
-                    uint2* dst = reinterpret_cast<uint2*>(out + row_base + (static_cast<long long>(j) * P * P + q) * 2);
-                    uint2 val = make_uint2(re[y], im[y]);
-                    if (reduce) {
-                        const uint2 old = *dst;
-                        val.x = add_bits<kFloat>(old.x, val.x);
-                        val.y = add_bits<kFloat>(old.y, val.y);
+                for (int y = 0; y < 8; ++y) {
+                    const int n = n0 + 2 * y + ri;
+                    const int j = n / P, q = n - j * P;
+                    if (row_ok && n < n_cols && (rect || j <= i)) {
+                        uint2* dst = reinterpret_cast<uint2*>(out + row_base + (static_cast<long long>(j) * P * P + q) * 2);
+                        uint2 val = make_uint2(re[y], im[y]);
+                        if (reduce) {
+                            const uint2 old = *dst;
+                            val.x = add_bits<kFloat>(old.x, val.x);
+                            val.y = add_bits<kFloat>(old.y, val.y);
+                        }
+                        *dst = val;
                     }
-                    *dst = val;
                 }
             }
+        }
+    }
+}
+
+// All TMEM passes of one tile through this epilogue warp (see drain_accumulator): `wait_pass(kc)` blocks until pass kc
+// of the tile is complete in TMEM and returns {TMEM address, release barrier} of the accumulator it sits in.
+template <bool kFloat, bool kRemote, int kBufs, typename WaitPass>
+__device__ __forceinline__ void drain_tile(const Params& prm, int n_kchunks, int c, int u0, int col0, int h_begin, int h_end,
+                                           uint32_t stage_smem, int& buf, int lane, WaitPass&& wait_pass) {
+    float run[64];
+    const bool acc = prm.accumulate != 0;
+    if (!kFloat || n_kchunks == 1) {
+        for (int kc = 0; kc < n_kchunks; ++kc) {          // int32: one pass by construction
+            uint32_t taddr, bar;
+            wait_pass(kc, taddr, bar);
+            drain_accumulator<kFloat, kRemote, kBufs, kFoldNone>(prm, c, u0, col0, h_begin, h_end, taddr, bar, acc || kc != 0,
+                                                                 stage_smem, buf, lane, run);
+        }
+        return;
+    }
+    if constexpr (kFloat) {
+#pragma unroll
+        for (int k = 0; k < 64; ++k) run[k] = 0.0f;
+        for (int kc = 0; kc < n_kchunks; ++kc) {
+            uint32_t taddr, bar;
+            wait_pass(kc, taddr, bar);
+            if (kc + 1 < n_kchunks)
+                drain_accumulator<kFloat, kRemote, kBufs, kFoldAdd>(prm, c, u0, col0, h_begin, h_end, taddr, bar, false, stage_smem,
+                                                                    buf, lane, run);
+            else
+                drain_accumulator<kFloat, kRemote, kBufs, kFoldLast>(prm, c, u0, col0, h_begin, h_end, taddr, bar, acc, stage_smem,
+                                                                     buf, lane, run);
         }
     }
 }
@@ -405,15 +483,14 @@ xengine_direct_kernel(const __grid_constant__ CUtensorMap tmap_in, const Params 
             const int u0 = td.row0 + quarter * 32;                 // first G row of this warp
             const int h_begin = chalf * (kTileCols / 2);
             const int h_end = td.ncols < h_begin + kTileCols / 2 ? td.ncols : h_begin + kTileCols / 2;
-            for (int kc = 0; kc < n_kchunks; ++kc) {
-                const bool reduce = prm.accumulate != 0 || kc != 0;
+            drain_tile<C::kFloat, false, 2>(prm, n_kchunks, prm.chan0_out + c, u0, td.col0, h_begin, h_end, stage_smem, buf, lane,
+                                            [&](int, uint32_t& taddr, uint32_t& bar) {
                 ptx::mbar_wait(tfull_bar(acc), acc_phase);
                 ptx::tc_fence_after();
-                const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + acc * kTileCols;
-                drain_accumulator<C::kFloat, false>(prm, prm.chan0_out + c, u0, td.col0, h_begin, h_end, taddr, tempty_bar(acc),
-                                                    reduce, kc == 0, stage_smem, buf, lane);
+                taddr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + acc * kTileCols;
+                bar = tempty_bar(acc);
                 if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
-            }
+            });
         }
         if (lane < 8) ptx::bulk_wait<0>();           // all bulk stores performed before the CTA retires
     }
