@@ -228,6 +228,7 @@ void fill_params(const corr_plan* h, const View& v, void* out, int accumulate, i
     prm.n_station_b = h->Nb;
     prm.M_b = h->Mb;
     prm.out = out;
+    prm.out_bytes = static_cast<unsigned long long>(n_dump) * v.c_total_out * h->B * h->P * h->P * 8;
     prm.accumulate = accumulate ? 1 : 0;
     // samples per TMEM accumulation pass: everything for int32 (exact); 1024 for fp32 (see xengine_tc.cuh)
     prm.k_chunk = h->dtype == CORR_CI8 ? (1 << 30) : xtc::kFloatChunk;

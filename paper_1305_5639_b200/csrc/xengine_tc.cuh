@@ -63,6 +63,7 @@ struct Params {
     int M;                   // n_station * n_pol  (inputs per channel)
     long long n_baseline;    // N(N+1)/2
     void* out;               // DEVICE: packed output
+    unsigned long long out_bytes;   // extent of `out`: every bulk store / reduce-add is checked against it (a violation traps)
     int accumulate;
     int k_chunk;             // samples per TMEM accumulation pass (multiple of the pipeline stage)
     // rectangular cross-only mode: rows are the n_station streams of group A (conjugated), columns the
@@ -252,6 +253,10 @@ __device__ __forceinline__ void drain_accumulator(const Params& prm, int c, int 
                         uint8_t* dst = out8 + ((row + j0) << 5);
                         const uint32_t src = sbuf + lane * kEpiRowBytes;
                         const uint32_t bytes = static_cast<uint32_t>(cnt) << 5;
+                        // the writer's own bounds check (compute-sanitizer is not available on every box): a segment
+                        // outside the caller's buffer or the warp's staging row is a bug, never a silent write
+                        if (((row + j0) << 5) < 0 || static_cast<unsigned long long>((row + j0) << 5) + bytes > prm.out_bytes ||
+                            bytes > static_cast<uint32_t>(kEpiRowBytes)) __trap();
                         if (!reduce) ptx::bulk_store(dst, src, bytes, policy);
                         else if constexpr (kFloat) ptx::bulk_reduce_add_f32(dst, src, bytes, policy);
                         else ptx::bulk_reduce_add_s32(dst, src, bytes, policy);
@@ -290,7 +295,9 @@ __device__ __forceinline__ void drain_accumulator(const Params& prm, int c, int 
                     const int n = n0 + 2 * y + ri;
                     const int j = n / P, q = n - j * P;
                     if (row_ok && n < n_cols && (rect || j <= i)) {
-                        uint2* dst = reinterpret_cast<uint2*>(out + row_base + (static_cast<long long>(j) * P * P + q) * 2);
+                        const long long word = row_base + (static_cast<long long>(j) * P * P + q) * 2;
+                        if (word < 0 || static_cast<unsigned long long>(word + 2) * 4 > prm.out_bytes) __trap();
+                        uint2* dst = reinterpret_cast<uint2*>(out + word);
                         uint2 val = make_uint2(re[y], im[y]);
                         if (reduce) {
                             const uint2 old = *dst;
