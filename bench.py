@@ -82,6 +82,7 @@ def parse_args():
     ap.add_argument("--no-sustained", action="store_true", help="skip the >= 2 s back-to-back sub-record")
     ap.add_argument("--no-others", action="store_true", help="skip the short runs of the other workloads and pieces")
     ap.add_argument("--no-sha", action="store_true", help="skip the SHA-256 of the input buffers")
+    ap.add_argument("--planes", type=int, default=1, choices=[1, 2], help="--piece corner_turn: planes written (2 adds ws_rot)")
     ap.add_argument("--e2e-steps", type=int, default=0, help="steps of the host-buffer leg (default min(K, 5))")
     return ap.parse_args()
 
@@ -381,25 +382,26 @@ def sha256_tensor(t):
 # ------------------------------------------------------------------------------------------------
 # piece (a): the standalone corner-turn kernel, HBM-bound (read in + write two planes)
 # ------------------------------------------------------------------------------------------------
-def time_corner_turn(cfg, pk, K, W):
+def time_corner_turn(cfg, pk, K, W, planes=1):
     import torch
     from paper_1305_5639_b200 import binding, inputs
     x = inputs.make_input(cfg, call=0, device="cuda")
     with binding.Correlator(cfg["N"], cfg["P"], cfg["C"], cfg["T"], cfg["dtype"]) as h:
-        ws = torch.empty((h.workspace_bytes,), dtype=torch.uint8, device="cuda")
+        ws = torch.empty((h.workspace_bytes * planes // 2,), dtype=torch.uint8, device="cuda")
         for _ in range(W):
-            h.corner_turn(x, ws)
+            h.corner_turn(x, ws, planes=planes)
         torch.cuda.synchronize()
         ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
         for a, b in ev:
-            a.record(); h.corner_turn(x, ws); b.record()
+            a.record(); h.corner_turn(x, ws, planes=planes); b.record()
         torch.cuda.synchronize()
         ms = sum(a.elapsed_time(b) for a, b in ev) / K
-        nbytes = cfg["in_bytes"] + h.workspace_bytes          # read the input once, write ws and ws_rot
+        nbytes = cfg["in_bytes"] + ws.numel()                 # read the input once, write ws (and ws_rot)
     gbs = nbytes / (ms * 1e-3) / 1e9
     return {"metric": "corner_turn_gbs", "value": gbs, "unit": "GB/s", "n_gpus": 1, "steps": K, "warmup": W,
             "ms_per_step": ms, "higher_is_better": True, "dtype": "u8", "data": "synthetic",
-            "config": {"workload": describe(cfg), "l2": "input + workspace (%.0f MiB) larger than L2" % (nbytes / 2 ** 20)},
+            "config": {"workload": describe(cfg), "planes": planes,
+                       "l2": "input + workspace (%.0f MiB) larger than L2" % (nbytes / 2 ** 20)},
             "gpu_launches": K,
             "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s", "frac": gbs / pk["hbm"],
                          "traffic": None, "kernel": "cturn::corner_turn_kernel", "kernel_ms": ms,
@@ -441,7 +443,7 @@ def run_piece(args):
         raise RuntimeError("bench.py needs a CUDA device")
     torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
     K, W = args.steps, max(args.warmup, 3)
-    rec = time_corner_turn(workload(args.workload), peaks(), K, W) if args.piece == "corner_turn" else time_fengine(peaks(), K, W)
+    rec = time_corner_turn(workload(args.workload), peaks(), K, W, args.planes) if args.piece == "corner_turn" else time_fengine(peaks(), K, W)
     print(json.dumps(rec), flush=True)
 
 

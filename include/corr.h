@@ -214,6 +214,9 @@ int corr_uses_tensor_cores(corr_handle h);
  * Asynchronous on `stream`.  corr_xengine does NOT run it: its TMA feed reads `in` in place.
  */
 int corr_corner_turn(corr_handle h, const void* in, void* ws, void* stream);
+/* The same with a choice of planes: n_planes == 1 writes only `ws` (the first corr_workspace_bytes(h) / 2 bytes; a consumer
+ * that forms the imaginary part without the rotated copy needs no more), n_planes == 2 is corr_corner_turn. */
+int corr_corner_turn_planes(corr_handle h, const void* in, void* ws, int n_planes, void* stream);
 size_t corr_workspace_bytes(corr_handle h);
 int corr_workspace_time(corr_handle h);
 

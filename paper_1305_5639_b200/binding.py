@@ -39,6 +39,7 @@ SYMBOLS = {
     "corr_get_kernel": (_i, [_vp]),
     "corr_uses_tensor_cores": (_i, [_vp]),
     "corr_corner_turn": (_i, [_vp, _vp, _vp, _vp]),
+    "corr_corner_turn_planes": (_i, [_vp, _vp, _vp, _i, _vp]),
     "corr_workspace_bytes": (_sz, [_vp]),
     "corr_workspace_time": (_i, [_vp]),
     "corr_tile_schedule": (_i, [_i, _i, _i, _i, ctypes.POINTER(_i), _i]),
@@ -248,13 +249,13 @@ class Correlator:
                                               int(bool(accumulate))))
         return out_host
 
-    def corner_turn(self, x, ws=None, stream=None):
-        """corr_corner_turn: returns the uint8 workspace holding the planes ws, ws_rot."""
+    def corner_turn(self, x, ws=None, stream=None, planes=2):
+        """corr_corner_turn_planes: returns the uint8 workspace holding the plane ws (and ws_rot when planes == 2)."""
         import torch
         self._check_in(x, "cuda")
         if ws is None:
-            ws = torch.empty((self.workspace_bytes,), dtype=torch.uint8, device=x.device)
-        self._check(self._L.corr_corner_turn(self._h, x.data_ptr(), ws.data_ptr(), _stream_ptr(stream)))
+            ws = torch.empty((self.workspace_bytes * planes // 2,), dtype=torch.uint8, device=x.device)
+        self._check(self._L.corr_corner_turn_planes(self._h, x.data_ptr(), ws.data_ptr(), int(planes), _stream_ptr(stream)))
         return ws
 
     def close(self):

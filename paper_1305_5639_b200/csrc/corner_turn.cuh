@@ -22,17 +22,29 @@ constexpr int kPitch = 33;           // smem row pitch in words
 struct Params {
     const void* in;
     void* ws;            // plane 0
-    void* ws_rot;        // plane 1
+    void* ws_rot;        // plane 1 (nullptr: not written)
     long long n_cm;      // C * M
     int n_time;          // T
     int n_time_pad;      // Tp (multiple of 64)
 };
 
-__device__ __forceinline__ uint4 ldg_stream(const uint4* p) {
+__device__ __forceinline__ uint64_t policy_evict_first() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void stg_stream(void* p, const uint4& v, uint64_t policy) {
+    // written once, read by a later kernel: keep it out of L1, let L2 write it back early
+    asm volatile("st.global.L1::no_allocate.L2::cache_hint.v4.u32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z),
+                 "r"(v.w), "l"(policy)
+                 : "memory");
+}
+__device__ __forceinline__ uint4 ldg_stream(const uint4* p, uint64_t policy) {
     uint4 r;
-    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
+    // read once: no L1 allocation, first in line for L2 eviction
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.u32 {%0, %1, %2, %3}, [%4], %5;"
                  : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
-                 : "l"(p));
+                 : "l"(p), "l"(policy));
     return r;
 }
 
@@ -56,6 +68,7 @@ corner_turn_kernel(const Params prm) {
     const int tid = threadIdx.x;
     const long long in_pitch = prm.n_cm * kSampleBytes;          // bytes per time step
     const uint8_t* in = static_cast<const uint8_t*>(prm.in);
+    const uint64_t policy = policy_evict_first();
 
     if constexpr (kSampleBytes == 2) {
         // 64 t x 64 cm patch.  Thread (tp, chunk): rows 2tp, 2tp+1; streams chunk*8 .. +7 (16 bytes each).
@@ -65,8 +78,8 @@ corner_turn_kernel(const Params prm) {
         uint4 a = make_uint4(0, 0, 0, 0), b = make_uint4(0, 0, 0, 0);
         if (cm < prm.n_cm) {
             const int ta = t0 + 2 * tp;
-            if (ta < prm.n_time) a = ldg_stream(reinterpret_cast<const uint4*>(in + ta * in_pitch + cm * 2));
-            if (ta + 1 < prm.n_time) b = ldg_stream(reinterpret_cast<const uint4*>(in + (ta + 1) * in_pitch + cm * 2));
+            if (ta < prm.n_time) a = ldg_stream(reinterpret_cast<const uint4*>(in + ta * in_pitch + cm * 2), policy);
+            if (ta + 1 < prm.n_time) b = ldg_stream(reinterpret_cast<const uint4*>(in + (ta + 1) * in_pitch + cm * 2), policy);
         }
         const uint32_t aw[4] = {a.x, a.y, a.z, a.w}, bw[4] = {b.x, b.y, b.z, b.w};
 #pragma unroll
@@ -85,7 +98,7 @@ corner_turn_kernel(const Params prm) {
             const int tl = trow + 16 * pass;
             uint4 a = make_uint4(0, 0, 0, 0);
             if (cm < prm.n_cm && t0 + tl < prm.n_time)
-                a = ldg_stream(reinterpret_cast<const uint4*>(in + (t0 + tl) * in_pitch + cm * 4));
+                a = ldg_stream(reinterpret_cast<const uint4*>(in + (t0 + tl) * in_pitch + cm * 4), policy);
             tile[(chunk * 4 + 0) * kPitch + tl] = a.x;
             tile[(chunk * 4 + 1) * kPitch + tl] = a.y;
             tile[(chunk * 4 + 2) * kPitch + tl] = a.z;
@@ -107,11 +120,13 @@ corner_turn_kernel(const Params prm) {
         if (cm0 + row < prm.n_cm) {
             const uint32_t* src = tile + row * kPitch + 4 * tg;
             const uint4 v = make_uint4(src[0], src[1], src[2], src[3]);
-            const uint4 r = make_uint4(rotate_word<kSampleBytes>(v.x), rotate_word<kSampleBytes>(v.y),
-                                       rotate_word<kSampleBytes>(v.z), rotate_word<kSampleBytes>(v.w));
             const long long off = (cm0 + row) * out_pitch + seg + 16 * tg;
-            *reinterpret_cast<uint4*>(ws + off) = v;
-            *reinterpret_cast<uint4*>(wr + off) = r;
+            stg_stream(ws + off, v, policy);
+            if (wr != nullptr) {
+                const uint4 r = make_uint4(rotate_word<kSampleBytes>(v.x), rotate_word<kSampleBytes>(v.y),
+                                           rotate_word<kSampleBytes>(v.z), rotate_word<kSampleBytes>(v.w));
+                stg_stream(wr + off, r, policy);
+            }
         }
     }
 }

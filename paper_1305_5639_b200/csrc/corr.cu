@@ -348,11 +348,11 @@ int launch_simt(corr_plan* h, const View& v, const void* in, const void* in_b, v
     return CORR_OK;
 }
 
-int launch_corner_turn(corr_plan* h, const void* in, void* ws, cudaStream_t st) {
+int launch_corner_turn(corr_plan* h, const void* in, void* ws, int n_planes, cudaStream_t st) {
     cturn::Params prm;
     prm.in = in;
     prm.ws = ws;
-    prm.ws_rot = static_cast<uint8_t*>(ws) + workspace_bytes(h) / 2;
+    prm.ws_rot = n_planes == 2 ? static_cast<uint8_t*>(ws) + workspace_bytes(h) / 2 : nullptr;
     prm.n_cm = static_cast<long long>(h->C) * h->M;
     prm.n_time = h->T;
     prm.n_time_pad = h->Tp;
@@ -639,7 +639,12 @@ int corr_fengine_ci8(const void* in, void* out, int n_stream, long long n_spectr
 }
 
 int corr_corner_turn(corr_handle h, const void* in, void* ws, void* stream) {
+    return corr_corner_turn_planes(h, in, ws, 2, stream);
+}
+
+int corr_corner_turn_planes(corr_handle h, const void* in, void* ws, int n_planes, void* stream) {
     if (!h) return CORR_EINVAL;
+    if (n_planes != 1 && n_planes != 2) return fail(h, CORR_EINVAL, "corr_corner_turn_planes: n_planes must be 1 or 2");
     if (h->Nb || h->C != h->C_total) return fail(h, CORR_EINVAL, "corr_corner_turn: not available on cross or window plans");
     if (!in || !ws) return fail(h, CORR_EINVAL, "corr_corner_turn: NULL pointer");
     if ((reinterpret_cast<uintptr_t>(in) & 15) || (reinterpret_cast<uintptr_t>(ws) & 127))
@@ -648,7 +653,7 @@ int corr_corner_turn(corr_handle h, const void* in, void* ws, void* stream) {
         return fail(h, CORR_EUNSUPPORTED, "corr_corner_turn: per-channel row of %lld B is not a multiple of 16",
                     static_cast<long long>(h->M) * h->sample_bytes);
     h->last_launches = 0;
-    return launch_corner_turn(h, in, ws, static_cast<cudaStream_t>(stream));
+    return launch_corner_turn(h, in, ws, n_planes, static_cast<cudaStream_t>(stream));
 }
 
 static int run_xengine(corr_handle h, const void* in, const void* in_b, void* out, int accumulate, void* stream) {

@@ -250,6 +250,14 @@ def test_corner_turn_kernel(corr):
             want_rot = np.minimum(want_rot, 127)
         assert np.array_equal(planes[0].astype(want_ws.dtype), want_ws)
         assert np.array_equal(planes[1].astype(want_rot.dtype), want_rot)
+        # one plane only (corr_corner_turn_planes): the first half of the workspace, nothing beyond it
+        with corr.Correlator(N, P, C, T, dtype) as h:
+            half = h.workspace_bytes // 2
+            buf = torch.full((half + 4096,), 0x5a, dtype=torch.uint8, device="cuda")
+            h.corner_turn(x.cuda(), buf[:half], planes=1)
+            torch.cuda.synchronize()
+            one = buf[:half].cpu().view(torch.int8 if dtype == "ci8" else torch.float16).view(C, N * P, Tp, 2).numpy()
+            assert np.array_equal(one.astype(want_ws.dtype), want_ws) and (buf[half:] == 0x5a).all()
 
 
 # ---------------------------------------------------------------------------------------------
