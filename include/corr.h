@@ -163,8 +163,16 @@ int corr_xengine_dumps(corr_handle h, const void* in, void* out, int n_dump, voi
  *         (stream m = s * n_pol + p) this IS corr_xengine's CORR_CF16 input [n_time = n_spectra][n_chan = 128]
  *         [n_station][n_pol]: no corner turn between the engines.
  * Stateless (no handle), asynchronous on `stream`; CORR_OK or a negative code, message via corr_last_error(NULL).
+ * Kernels: with n_stream a multiple of 64 and a 16-byte aligned `out` the transform runs as a dense contraction on the
+ * tcgen05 tensor cores (the real-input DFT folded onto 128 samples, twiddle matrices split into fp16 hi + lo parts,
+ * fp32 accumulation: csrc/fengine_tc.cuh); every other geometry runs on the CUDA-core radix-16 x 16 FFT kernel
+ * (csrc/fengine.cuh).  Both meet the same bound against the fp64 definition: 0.5 ulp of the fp16 output plus
+ * 2e-6 sum_n |s[n]|.  corr_fengine_simt forces the CUDA-core kernel (cross-check); corr_fengine_uses_tensor_cores tells
+ * which one corr_fengine would launch (1 / 0).
  */
 int corr_fengine(const void* in, void* out, int n_stream, long long n_spectra, void* stream);
+int corr_fengine_simt(const void* in, void* out, int n_stream, long long n_spectra, void* stream);
+int corr_fengine_uses_tensor_cores(int n_stream, const void* out);
 
 /*
  * corr_fengine_ci8 -- the same transform with REQUANTISED complex int8 output, the input format of the int8 X-engine

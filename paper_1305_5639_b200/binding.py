@@ -28,6 +28,8 @@ SYMBOLS = {
     "corr_xengine_cross": (_i, [_vp, _vp, _vp, _vp, _i, _vp]),
     "corr_input_bytes_b": (_sz, [_vp]),
     "corr_fengine": (_i, [_vp, _vp, _i, _ll, _vp]),
+    "corr_fengine_simt": (_i, [_vp, _vp, _i, _ll, _vp]),
+    "corr_fengine_uses_tensor_cores": (_i, [_i, _vp]),
     "corr_fengine_ci8": (_i, [_vp, _vp, _i, _ll, ctypes.c_float, _vp]),
     "corr_xengine_dumps": (_i, [_vp, _vp, _vp, _i, _vp]),
     "corr_destroy": (None, [_vp]),
@@ -92,9 +94,10 @@ def _stream_ptr(stream):
     return ctypes.c_void_p(getattr(stream, "cuda_stream", stream))
 
 
-def fengine(samples, out=None, stream=None, scale=None):
+def fengine(samples, out=None, stream=None, scale=None, simt=False):
     """corr_fengine: int8 real samples [n_stream, n_spectra * 256] (CUDA) -> complex fp16 [n_spectra, 128, n_stream, 2];
-    with ``scale`` (corr_fengine_ci8): requantised complex int8 codes clip(rint(S * scale), +-127) of the same shape."""
+    with ``scale`` (corr_fengine_ci8): requantised complex int8 codes clip(rint(S * scale), +-127) of the same shape.
+    ``simt=True`` forces the CUDA-core kernel (corr_fengine_simt)."""
     import torch
     if scale is not None:
         return _fengine_ci8(samples, float(scale), out, stream)
@@ -107,10 +110,16 @@ def fengine(samples, out=None, stream=None, scale=None):
     if out.dtype != torch.float16 or tuple(out.shape) != (n_spec, 128, n_stream, 2) or not out.is_contiguous():
         raise ValueError("out must be a contiguous float16 tensor [n_spectra, 128, n_stream, 2]")
     L = lib()
-    rc = L.corr_fengine(samples.data_ptr(), out.data_ptr(), n_stream, n_spec, _stream_ptr(stream))
+    fn = L.corr_fengine_simt if simt else L.corr_fengine
+    rc = fn(samples.data_ptr(), out.data_ptr(), n_stream, n_spec, _stream_ptr(stream))
     if rc != CORR_OK:
         raise CorrError(rc, L.corr_last_error(None).decode())
     return out
+
+
+def fengine_uses_tensor_cores(n_stream, out=None):
+    """Which kernel corr_fengine launches for this stream count (and output alignment)."""
+    return bool(lib().corr_fengine_uses_tensor_cores(int(n_stream), None if out is None else out.data_ptr()))
 
 
 def _fengine_ci8(samples, scale, out, stream):

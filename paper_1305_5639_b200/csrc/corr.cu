@@ -10,12 +10,15 @@
 #include <cstdint>
 #include <cstdio>
 #include <cstdlib>
+#include <cmath>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
 #include "corner_turn.cuh"
 #include "fengine.cuh"
+#include "fengine_tc.cuh"
 #include "xengine_simt.cuh"
 #include "xengine_tc.cuh"
 #include "xengine_pair.cuh"
@@ -109,6 +112,62 @@ int fail(corr_plan* h, int code, const char* fmt, ...) {
 
 int fail_cuda(corr_plan* h, cudaError_t e, const char* what) {
     return fail(h, CORR_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+EncodeTiledFn get_encode_fn() {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    const cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+    if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess) return nullptr;
+    return reinterpret_cast<EncodeTiledFn>(fn);
+}
+
+// Tensor-core F-engine (fengine_tc.cuh): per-device twiddle table [cos_hi | cos_lo | -sin_hi | -sin_lo], each
+// [128 channels][128 folded samples] fp16, and its tensor map; built on first use.
+struct FengTcState {
+    bool tried = false, ok = false;
+    void* d_tw = nullptr;
+    EncodeTiledFn encode = nullptr;
+    int sm_count = 0;
+};
+std::mutex g_feng_mutex;
+FengTcState g_feng[64];
+
+FengTcState* fengine_tc_state() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+    std::lock_guard<std::mutex> lock(g_feng_mutex);
+    FengTcState& st = g_feng[dev];
+    if (st.tried) return st.ok ? &st : nullptr;
+    st.tried = true;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess || prop.major != 10 || prop.minor != 0) return nullptr;
+    st.sm_count = prop.multiProcessorCount;
+    st.encode = get_encode_fn();
+    if (!st.encode) return nullptr;
+    // hi = fp16(w), lo = fp16(w - hi): w = hi + lo to ~3e-8 absolute (lo may be subnormal)
+    std::vector<__half> tw(4 * fengtc::kChan * fengtc::kFold);
+    const double two_pi = 6.283185307179586476925286766559;
+    for (int k = 0; k < fengtc::kChan; ++k)
+        for (int n = 0; n < fengtc::kFold; ++n) {
+            const int kn = (k * n) % fengtc::kFft;                       // exact angle reduction in integers
+            const double c = std::cos(two_pi * kn / fengtc::kFft), sn = -std::sin(two_pi * kn / fengtc::kFft);
+            const double w[2] = {c, sn};
+            for (int part = 0; part < 2; ++part) {
+                const __half hi = __float2half_rn(static_cast<float>(w[part]));
+                const __half lo = __float2half_rn(static_cast<float>(w[part] - static_cast<double>(__half2float(hi))));
+                tw[((2 * part + 0) * fengtc::kChan + k) * fengtc::kFold + n] = hi;
+                tw[((2 * part + 1) * fengtc::kChan + k) * fengtc::kFold + n] = lo;
+            }
+        }
+    if (cudaMalloc(&st.d_tw, tw.size() * sizeof(__half)) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    if (cudaMemcpy(st.d_tw, tw.data(), tw.size() * sizeof(__half), cudaMemcpyHostToDevice) != cudaSuccess) return nullptr;
+    if (cudaFuncSetAttribute(fengtc::fengine_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, fengtc::kSmemBytes) != cudaSuccess) {
+        cudaGetLastError();
+        return nullptr;
+    }
+    st.ok = true;
+    return &st;
 }
 
 bool valid_geometry(int N, int P, int dtype) {
@@ -491,16 +550,12 @@ static corr_handle create_plan(int n_station, int n_station_b, int n_pol, int n_
         return nullptr;
     }
     if (h->tma_ok) {
-        void* fn = nullptr;
-        cudaDriverEntryPointQueryResult qres;
-        e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
-        if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn) {
-            fail(nullptr, CORR_ECUDA, "corr_create: cuTensorMapEncodeTiled entry point unavailable (%s)",
-                 cudaGetErrorString(e));
+        h->encode = get_encode_fn();
+        if (!h->encode) {
+            fail(nullptr, CORR_ECUDA, "corr_create: cuTensorMapEncodeTiled entry point unavailable");
             corr_destroy(h);
             return nullptr;
         }
-        h->encode = reinterpret_cast<EncodeTiledFn>(fn);
         e = cudaFuncSetAttribute(xtc::xengine_direct_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, xtc::kSmemBytes);
         if (e == cudaSuccess)
             e = cudaFuncSetAttribute(xtc::xengine_direct_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, xtc::kSmemBytes);
@@ -607,12 +662,45 @@ int corr_set_kernel(corr_handle h, int kernel) {
 }
 int corr_last_launch_count(corr_handle h) { return h ? h->last_launches : CORR_EINVAL; }
 
-static int run_fengine(const void* in, void* out, int n_stream, long long n_spectra, bool int8_out, float scale, void* stream) {
+// tensor-core path: fp16 output, whole tiles of 64 streams, 16-byte aligned output rows
+static bool fengine_tc_applies(const void* out, int n_stream, bool int8_out) {
+    return !int8_out && n_stream % fengtc::kTileStreams == 0 && (reinterpret_cast<uintptr_t>(out) & 15) == 0;
+}
+
+static int run_fengine_tc(FengTcState* st, const void* in, void* out, int n_stream, long long n_spectra, cudaStream_t stream) {
+    CUtensorMap map_raw;       // in viewed as [n_stream][n_spectra][256] bytes, box = 64 streams x 1 spectrum x 256 samples
+    cuuint64_t dims[3] = {fengtc::kFft, static_cast<cuuint64_t>(n_spectra), static_cast<cuuint64_t>(n_stream)};
+    cuuint64_t strides[2] = {fengtc::kFft, static_cast<cuuint64_t>(n_spectra) * fengtc::kFft};
+    cuuint32_t box[3] = {fengtc::kFft, 1, fengtc::kTileStreams};
+    cuuint32_t estr[3] = {1, 1, 1};
+    const CUresult r = st->encode(&map_raw, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(in), dims, strides, box, estr,
+                                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(nullptr, CORR_ECUDA, "corr_fengine: cuTensorMapEncodeTiled failed with CUresult %d", static_cast<int>(r));
+    fengtc::Params prm;
+    prm.out = out;
+    prm.tw = static_cast<const uint4*>(st->d_tw);
+    prm.n_stream = n_stream;
+    prm.n_spectra = n_spectra;
+    prm.n_tiles = n_spectra * (n_stream / fengtc::kTileStreams);
+    const long long grid = prm.n_tiles < st->sm_count ? prm.n_tiles : st->sm_count;
+    fengtc::fengine_tc_kernel<<<static_cast<unsigned>(grid), fengtc::kThreads, fengtc::kSmemBytes, stream>>>(map_raw, prm);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(nullptr, e, "fengine_tc_kernel launch");
+    return CORR_OK;
+}
+
+static int run_fengine(const void* in, void* out, int n_stream, long long n_spectra, bool int8_out, float scale, void* stream,
+                       bool allow_tc = true) {
     g_create_error[0] = 0;
     if (!in || !out || n_stream < 1 || n_spectra < 1 || n_spectra > 0x7fffffffLL || (int8_out && !(scale > 0.0f)))
         return fail(nullptr, CORR_EINVAL, "corr_fengine: invalid arguments (n_stream=%d, n_spectra=%lld)", n_stream, n_spectra);
     if ((reinterpret_cast<uintptr_t>(in) & 15) || (reinterpret_cast<uintptr_t>(out) & (int8_out ? 1 : 3)))
         return fail(nullptr, CORR_EINVAL, "corr_fengine: `in` must be 16-byte and `out` element aligned");
+    if (allow_tc && fengine_tc_applies(out, n_stream, int8_out)) {
+        FengTcState* st = fengine_tc_state();
+        if (st) return run_fengine_tc(st, in, out, n_stream, n_spectra, static_cast<cudaStream_t>(stream));
+    }
     feng::Params prm;
     prm.in = static_cast<const int8_t*>(in);
     prm.out = out;
@@ -636,6 +724,14 @@ int corr_fengine(const void* in, void* out, int n_stream, long long n_spectra, v
 
 int corr_fengine_ci8(const void* in, void* out, int n_stream, long long n_spectra, float scale, void* stream) {
     return run_fengine(in, out, n_stream, n_spectra, true, scale, stream);
+}
+
+int corr_fengine_simt(const void* in, void* out, int n_stream, long long n_spectra, void* stream) {
+    return run_fengine(in, out, n_stream, n_spectra, false, 1.0f, stream, false);
+}
+
+int corr_fengine_uses_tensor_cores(int n_stream, const void* out) {
+    return fengine_tc_applies(out, n_stream, false) ? 1 : 0;
 }
 
 int corr_corner_turn(corr_handle h, const void* in, void* ws, void* stream) {

@@ -21,9 +21,9 @@ def corr():
     return binding
 
 
-def check(corr, s):
+def check(corr, s, simt=False):
     from oracle import fengine as fo
-    got = corr.fengine(torch.from_numpy(s).cuda()).cpu().numpy().astype(np.float64)       # [A, 128, M, 2]
+    got = corr.fengine(torch.from_numpy(s).cuda(), simt=simt).cpu().numpy().astype(np.float64)       # [A, 128, M, 2]
     want = fo.fengine(s)
     A, K, M = want.shape
     assert got.shape == (A, K, M, 2)
@@ -38,7 +38,51 @@ def check(corr, s):
 @pytest.mark.parametrize("M,A", [(1, 1), (2, 3), (7, 2), (32, 4), (33, 5), (64, 16), (100, 9), (512, 8)])
 def test_fengine_random_full_range(corr, M, A):
     rng = np.random.default_rng(9000 + M)
-    check(corr, rng.integers(-128, 128, size=(M, A * 256), dtype=np.int8))
+    s = rng.integers(-128, 128, size=(M, A * 256), dtype=np.int8)
+    assert corr.fengine_uses_tensor_cores(M) == (M % 64 == 0)
+    check(corr, s)
+    check(corr, s, simt=True)                            # the CUDA-core kernel on the same input
+
+
+@pytest.mark.parametrize("M,A", [(64, 1), (64, 149), (128, 33), (192, 7), (320, 2), (512, 300), (1024, 37)])
+def test_fengine_tensor_core_path(corr, M, A):
+    """The tcgen05 kernel (stream counts that are multiples of 64): more tiles than SMs, a single tile, odd tile counts;
+    full-range int8 including -128; the same bound as the CUDA-core kernel, and the two kernels agree to one fp16 ulp
+    plus both fp32 round-off allowances."""
+    rng = np.random.default_rng(9100 + M + A)
+    s = rng.integers(-128, 128, size=(M, A * 256), dtype=np.int8)
+    assert corr.fengine_uses_tensor_cores(M)
+    check(corr, s)
+    sd = torch.from_numpy(s).cuda()
+    tc, cc = corr.fengine(sd).float(), corr.fengine(sd, simt=True).float()
+    big = torch.maximum(tc.abs(), cc.abs()).cpu().numpy()
+    ulp = np.spacing(big.astype(np.float16)).astype(np.float64)
+    l1 = np.abs(s.reshape(M, A, 256).astype(np.float64)).sum(axis=2).T[:, None, :, None]          # [A, 1, M, 1]
+    assert ((tc - cc).abs().cpu().numpy() <= ulp + 4e-6 * l1).all()
+
+
+def test_fengine_tensor_core_exact_cases(corr):
+    """64 streams of hand-checkable inputs through the tcgen05 kernel: impulses at n = 0, 1, 128 (the sample that bypasses
+    the folded sums), 200; DC; extreme DC; the Nyquist tone (dropped bin); a full-scale tone on a bin centre."""
+    n = np.arange(512)
+    s = np.zeros((64, 512), np.int8)
+    s[0, 0] = 7; s[0, 256 + 5] = 9
+    s[1, :] = -3
+    s[2, :] = np.array([100, 50, -100, -50])[n % 4]
+    s[3, :] = 127; s[4, :] = -128
+    s[5, :] = np.where(n % 2 == 0, 127, -128)
+    s[6, 128] = 11; s[6, 256 + 1] = -5
+    s[7, :] = np.rint(127 * np.cos(2 * np.pi * 37 * n / 256)).astype(np.int8)
+    s[8:] = np.random.default_rng(3).integers(-128, 128, size=(56, 512), dtype=np.int8)
+    assert corr.fengine_uses_tensor_cores(64)
+    got = corr.fengine(torch.from_numpy(s).cuda()).cpu().numpy().astype(np.float64)
+    assert (got[0, :, 0, 0] == 7).all() and (got[0, :, 0, 1] == 0).all()
+    assert got[0, 0, 1, 0] == -768 and np.abs(got[:, 1:, 1]).max() <= 1e-3
+    assert got[1, 64, 2, 0] == 12800 and got[1, 64, 2, 1] == -6400
+    assert got[0, 0, 3, 0] == 127 * 256 and got[0, 0, 4, 0] == -128 * 256
+    assert got[0, 0, 5, 0] == -128 and np.abs(got[:, 1:, 5]).max() <= 0.05
+    assert (got[0, :, 6, 0] == 11 * np.where(np.arange(128) % 2 == 0, 1, -1)).all() and (got[0, :, 6, 1] == 0).all()
+    check(corr, s)
 
 
 def test_fengine_exact_cases(corr):

@@ -103,5 +103,5 @@ def test_cross_and_dumps_repeated(corr, oracle):
         first = h.xengine_dumps(x, 8)
         for d in range(8):
             assert (first[d].cpu().numpy().astype(np.int64) == oracle.xengine(x[d * 32:(d + 1) * 32].cpu().numpy())).all()
-        for it in range(60):
+        for it in range(400):                                 # 1-stage tiles: the fastest tile turnover the feed sees
             assert torch.equal(h.xengine_dumps(x, 8), first)
