@@ -51,8 +51,12 @@ FALLBACK_HBM_GBS = 6650.0
 # committed `ncu --set full` captures of the SAME kernel and geometry -- not measured by this run, and emitted only when
 # the kernel that ran is the one that was captured: workload -> (kernel, bytes, capture file)
 NCU_TRAFFIC = {
-    "cfg4": ("pair", (3.198e9 + 3 * 4.275e9) / 4, "profiles/r1c_final_ncu_pair_feed.md"),
-    "cfg3": ("pair", 4.651e9, "profiles/r1c_final_ncu_pair_feed.md"),
+    "cfg4": ("pair", (3.197e9 + 3 * 4.275e9) / 4, "profiles/r2_ncu_final.md"),      # accumulate = 0 once, = 1 three times
+    "cfg3": ("pair", 4.870e9, "profiles/r2_ncu_final.md"),
+    "cfg2": ("pair", 0.3165e9, "profiles/r2_ncu_final.md"),
+    "cfg5_n128": ("pair", 1.326e9, "profiles/r2_ncu_final.md"),
+    "cfg5_n1024": ("pair", 3.168e9, "profiles/r2_ncu_final.md"),
+    "cross_n256": ("pair", 3.190e9, "profiles/r2_ncu_final.md"),
     "cfg5_n64": ("pair", 1.200e9, "profiles/r1c_final_ncu_pair_feed.md"),
     "cfg5_n32": ("single", 1.139e9, "profiles/r1c_final_ncu_pair_feed.md"),
 }
@@ -404,7 +408,10 @@ def time_corner_turn(cfg, pk, K, W, planes=1):
                        "l2": "input + workspace (%.0f MiB) larger than L2" % (nbytes / 2 ** 20)},
             "gpu_launches": K,
             "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s", "frac": gbs / pk["hbm"],
-                         "traffic": None, "kernel": "cturn::corner_turn_kernel", "kernel_ms": ms,
+                         "traffic": 4.246e9 if (cfg["name"] == "cfg4" and planes == 1) else None,
+                         "traffic_source": "profiles/r2_ncu_final.md (ncu capture of this kernel and geometry; NOT measured by this run)"
+                         if (cfg["name"] == "cfg4" and planes == 1) else None,
+                         "kernel": "cturn::corner_turn_kernel", "kernel_ms": ms,
                          "algorithmic_bytes_per_launch": nbytes}}
 
 
@@ -426,15 +433,18 @@ def time_fengine(pk, K, W, M=512, A=8192):
     nbytes = s.numel() + out.numel() * 2
     gbs = nbytes / (ms * 1e-3) / 1e9
     return {"metric": "fengine_gbs", "value": gbs, "unit": "GB/s", "n_gpus": 1, "steps": K, "warmup": W,
-            "ms_per_step": ms, "higher_is_better": True, "dtype": "f32", "data": "synthetic",
+            "ms_per_step": ms, "higher_is_better": True, "dtype": "f16 x f16 -> f32 (twiddles hi + lo)", "data": "synthetic",
             "config": {"workload": "F-engine: %d streams x %d spectra of 256 real int8 samples (sigma 20) -> 128 complex fp16 "
                                    "channels in the X-engine layout" % (M, A),
                        "l2": "input + output (%.0f MiB) larger than L2" % (nbytes / 2 ** 20),
                        "gsamples_per_s": s.numel() / (ms * 1e-3) / 1e9},
             "gpu_launches": K,
             "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s", "frac": gbs / pk["hbm"],
-                         "traffic": None, "kernel": "feng::fengine_kernel", "kernel_ms": ms,
-                         "algorithmic_bytes_per_launch": nbytes}}
+                         "traffic": 3.165e9 if (M, A) == (512, 8192) else None,
+                         "traffic_source": "profiles/r2_ncu_final.md (ncu capture of this kernel and geometry; NOT measured by this run)"
+                         if (M, A) == (512, 8192) else None,
+                         "kernel": "fengtc::fengine_tc_kernel" if binding.fengine_uses_tensor_cores(M, out) else "feng::fengine_kernel",
+                         "kernel_ms": ms, "algorithmic_bytes_per_launch": nbytes}}
 
 
 def run_piece(args):
@@ -513,6 +523,7 @@ def short_run(name, pk, K=10, W=3, sha=True):
         kernel_ms = sum(ms) / len(ms)
         rec = {"workload": describe(cfg), "kernel": r.h.kernel, "steps": K, "ms_per_call": kernel_ms,
                "value": cfg["ops_per_call"] / (kernel_ms * 1e-3) / 1e12, "unit": UNIT,
+               "best_ms_per_call": min(ms), "best_value": cfg["ops_per_call"] / (min(ms) * 1e-3) / 1e12,
                "visibilities_per_s": cfg["C"] * cfg["n_baseline"] * cfg["P"] ** 2 / (kernel_ms * 1e-3),
                "l2": "flushed between steps (cold)" if r.flush is not None else "inputs larger than L2",
                "roofline": roofline_record(cfg, r.h.kernel, kernel_ms, pk, sustained=False)}
