@@ -11,18 +11,21 @@
 // so the result carries only the accumulation round-off: well inside the fp32 bound the parity test allows
 // (0.5 ulp of the fp16 output + 2e-6 sum|s|).  Per real sample: 256 tensor MACs instead of ~29 CUDA-core instructions.
 //
-// One CTA (cta_group::1, 320 threads, persistent over tiles of 64 streams x 1 spectrum):
-//   warp 0      TMA: the raw int8 tile [64 streams][256 samples] of every tile into a 2-deep ring
+// One CTA (cta_group::1, 576 threads, persistent over tiles of 64 streams x 1 spectrum):
+//   warp 0      TMA: the raw int8 tile [64 streams][256 samples] of every tile into a 4-deep ring
 //   warp 1      tcgen05.mma issuer: per tile 32 MMAs (M 128, N 64, K 16): {cos, sin} x {hi, lo} x 8 k-steps into two
 //               64-column fp32 accumulators in TMEM (double buffered across tiles).  The A operand -- the four twiddle
 //               matrices -- lives in TENSOR MEMORY for the whole kernel (256 columns, written once by warps 2-5 with
 //               tcgen05.st), so an MMA reads only its 2 KB of B from shared memory (with A in shared memory the MMAs
 //               were shared-memory-bandwidth bound at 2.3x their tensor time, and the 128 KB left no room to double
 //               buffer B)
-//   warps 2-5   fold + convert: raw int8 -> e, o as fp16 in the K-major SWIZZLE_128B layout the MMA reads (bytes are
+//   warps 2-9   fold + convert: raw int8 -> e, o as fp16 in the K-major SWIZZLE_128B layout the MMA reads (bytes are
 //               turned into halves with the 0x6400 | byte trick, no integer-to-float conversion instruction), 2-deep
-//   warps 6-9   epilogue: TMEM -> (+ (-1)^k s[128]) -> fp16 (re, im) -> shared-memory transpose -> 128-byte rows of 32
-//               streams per channel, written with 16-byte coalesced stores straight into the X-engine's input layout
+//   warps 10-17 epilogue (two warps per TMEM lane quarter, 32 streams each): TMEM -> (+ (-1)^k s[128]) -> fp16 (re, im)
+//               -> shared-memory transpose -> 128-byte rows of 32 streams per channel, written with 16-byte coalesced
+//               stores straight into the X-engine's input layout
+// (Round 2, first version: four fold and four epilogue warps, 2-deep raw ring: every role ~80 % busy in a chain of 2-deep
+// hand-overs, 2820 clk per tile, 4.56 TB/s.  Eight + eight warps halve the per-tile time of both roles.)
 #pragma once
 #include <cuda_fp16.h>
 #include "ptx.cuh"
@@ -33,23 +36,28 @@ constexpr int kFft = 256;
 constexpr int kChan = 128;                    // channels kept = MMA M
 constexpr int kFold = 128;                    // folded samples = GEMM K
 constexpr int kTileStreams = 64;              // streams per tile = MMA N
-constexpr int kThreads = 320;
+constexpr int kFoldWarps = 8, kEpiWarps = 8;
+constexpr int kThreads = 64 + 32 * (kFoldWarps + kEpiWarps);
+constexpr int kRawRing = 4;                   // raw int8 tiles in flight per CTA (covers the DRAM latency)
 constexpr int kMatCols = kFold / 2;           // one fp16 twiddle matrix in TMEM: 128 lanes x 64 columns (2 halves each)
 constexpr int kRawBytes = kTileStreams * kFft;              // 16 KB
 constexpr int kOpBytes = kTileStreams * kFold * 2;          // e or o as fp16: 16 KB (two chunks of 8 KB)
 constexpr int kStageRow = 128 + 16;                          // epilogue staging row (32 half2 + pad), bytes
 constexpr int kStageWarpBytes = 32 * kStageRow;
-constexpr int kS128Ring = 4;
+// s[128] of a tile travels from the fold warps to the epilogue through this ring.  fold(t) may start once MMA(t - 2) has
+// been committed, i.e. once every epilogue warp has RELEASED the accumulator of tile t - 4 -- at which point tile t - 5 is
+// finished in every epilogue warp, but tile t - 4 may still be reading its s[128]: the ring must hold >= 5 tiles
+constexpr int kS128Ring = 8;
 // tensor memory map (columns): two accumulator sets {cos 64, sin 64}, then cos_hi, cos_lo, sin_hi, sin_lo
 constexpr int kTmemAcc = 0, kTmemA = 256, kTmemCols = 512;
 // shared memory map (offsets from the 1024-byte aligned base)
 constexpr int kOffE = 0;                                     // 2 x {e, o}: slot s at s * 2 * kOpBytes
 constexpr int kOffO = kOpBytes;
-constexpr int kOffRaw = 4 * kOpBytes;                        // 2 x 16 KB
-constexpr int kOffStage = kOffRaw + 2 * kRawBytes;
-constexpr int kOffS128 = kOffStage + 4 * kStageWarpBytes;
+constexpr int kOffRaw = 4 * kOpBytes;                        // kRawRing x 16 KB
+constexpr int kOffStage = kOffRaw + kRawRing * kRawBytes;
+constexpr int kOffS128 = kOffStage + kEpiWarps * kStageWarpBytes;
 constexpr int kOffBar = kOffS128 + kS128Ring * kTileStreams * 4;
-constexpr int kSmemBytes = kOffBar + 128 + 1024 /*alignment slack*/;
+constexpr int kSmemBytes = kOffBar + 192 + 1024 /*alignment slack*/;
 static_assert(kSmemBytes <= 227 * 1024, "shared memory");
 
 struct Params {
@@ -99,9 +107,10 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t bar = base + kOffBar;
-    // barriers: a_full, raw_full[2], raw_empty[2], b_full[2], b_empty[2], acc_full[2], acc_empty[2], then the TMEM base word
-    const uint32_t a_full = bar, raw_full0 = bar + 8, raw_empty0 = bar + 24, b_full0 = bar + 40, b_empty0 = bar + 56;
-    const uint32_t acc_full0 = bar + 72, acc_empty0 = bar + 88, tmem_slot = bar + 104;
+    // barriers: a_full, raw_full[4], raw_empty[4], b_full[2], b_empty[2], acc_full[2], acc_empty[2], then the TMEM base word
+    const uint32_t a_full = bar, raw_full0 = bar + 8, raw_empty0 = raw_full0 + 8 * kRawRing, b_full0 = raw_empty0 + 8 * kRawRing;
+    const uint32_t b_empty0 = b_full0 + 16, acc_full0 = b_empty0 + 16, acc_empty0 = acc_full0 + 16, tmem_slot = acc_empty0 + 16;
+    static_assert(8 + 16 * kRawRing + 64 + 4 <= 192, "barrier region");
     uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - ptx::smem_u32(smem_raw)));
 
     const int warp = threadIdx.x >> 5;
@@ -109,14 +118,16 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
 
     if (threadIdx.x == 0) {
         ptx::prefetch_tensormap(&tmap_raw);
-        ptx::mbar_init(a_full, 4);                          // one arrive per fold warp once its twiddle rows are in TMEM
-        for (int k = 0; k < 2; ++k) {
+        ptx::mbar_init(a_full, 4);                          // one arrive per uploading warp once its twiddle rows are in TMEM
+        for (int k = 0; k < kRawRing; ++k) {
             ptx::mbar_init(raw_full0 + 8 * k, 1);
-            ptx::mbar_init(raw_empty0 + 8 * k, 4);          // one arrive per fold warp
-            ptx::mbar_init(b_full0 + 8 * k, 4);
+            ptx::mbar_init(raw_empty0 + 8 * k, kFoldWarps); // one arrive per fold warp
+        }
+        for (int k = 0; k < 2; ++k) {
+            ptx::mbar_init(b_full0 + 8 * k, kFoldWarps);
             ptx::mbar_init(b_empty0 + 8 * k, 1);
             ptx::mbar_init(acc_full0 + 8 * k, 1);
-            ptx::mbar_init(acc_empty0 + 8 * k, 4);          // one arrive per epilogue warp
+            ptx::mbar_init(acc_empty0 + 8 * k, kEpiWarps);  // one arrive per epilogue warp
         }
         ptx::fence_mbar_init();
     }
@@ -144,12 +155,13 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
                 ptx::mbar_arrive_expect_tx(raw_full0 + 8 * slot, kRawBytes);
                 // the sample axis is cut into [spectrum][256] (rank 3), so a box never needs a coordinate beyond 2^31
                 ptx::tma_load_3d(base + kOffRaw + slot * kRawBytes, &tmap_raw, raw_full0 + 8 * slot, 0, static_cast<int>(a), m0);
-                if (++slot == 2) { slot = 0; phase ^= 1u; }
+                if (++slot == kRawRing) { slot = 0; phase ^= 1u; }
             }
         }
     } else if (warp == 1) {
-        // ===================== MMA issuer =====================
-        if (lane == 0) {
+        // ===================== MMA issuer (whole warp in uniform control flow, one elected lane issues) =====================
+        {
+            const uint32_t tb = ptx::uniform(tmem_base);
             ptx::mbar_wait(a_full, 0);
             ptx::tc_fence_after();
             uint32_t phase = 0;                              // B slot, accumulator set and their phases advance together
@@ -158,31 +170,34 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
                 ptx::mbar_wait(b_full0 + 8 * slot, phase);
                 ptx::mbar_wait(acc_empty0 + 8 * slot, phase ^ 1u);
                 ptx::tc_fence_after();
+                if (ptx::elect_one()) {
 #pragma unroll
-                for (int part = 0; part < 2; ++part) {       // 0: cos x e -> Re, 1: sin x o -> Im
-                    const uint32_t d_tmem = tmem_base + kTmemAcc + slot * 128 + part * 64;
-                    const uint32_t sb = base + slot * 2 * kOpBytes + (part ? kOffO : kOffE);
+                    for (int part = 0; part < 2; ++part) {       // 0: cos x e -> Re, 1: sin x o -> Im
+                        const uint32_t d_tmem = tb + kTmemAcc + slot * 128 + part * 64;
+                        const uint32_t sb = base + slot * 2 * kOpBytes + (part ? kOffO : kOffE);
 #pragma unroll
-                    for (int hl = 0; hl < 2; ++hl) {
-                        const uint32_t a_tmem = tmem_base + kTmemA + (2 * part + hl) * kMatCols;
+                        for (int hl = 0; hl < 2; ++hl) {
+                            const uint32_t a_tmem = tb + kTmemA + (2 * part + hl) * kMatCols;
 #pragma unroll
-                        for (int ks = 0; ks < kFold / 16; ++ks) {
-                            // B: K-major SWIZZLE_128B: a k-step is 32 bytes inside the 128-byte row, the second 64-sample
-                            // chunk is 64 rows * 128 bytes further; SBO = 8 rows * 128 B.  A: 8 TMEM columns per k-step
-                            const uint32_t b_off = (ks >> 2) * (kOpBytes / 2) + (ks & 3) * 32;
-                            const uint64_t bdesc = ptx::smem_desc_sw128(sb + b_off, 16, 1024);
-                            ptx::mma_f16_ts(d_tmem, a_tmem + 8 * ks, bdesc, kIdesc, (hl | ks) ? 1u : 0u);
+                            for (int ks = 0; ks < kFold / 16; ++ks) {
+                                // B: K-major SWIZZLE_128B: a k-step is 32 bytes inside the 128-byte row, the second 64-sample
+                                // chunk is 64 rows * 128 bytes further; SBO = 8 rows * 128 B.  A: 8 TMEM columns per k-step
+                                const uint32_t b_off = (ks >> 2) * (kOpBytes / 2) + (ks & 3) * 32;
+                                const uint64_t bdesc = ptx::smem_desc_sw128(sb + b_off, 16, 1024);
+                                ptx::mma_f16_ts(d_tmem, a_tmem + 8 * ks, bdesc, kIdesc, (hl | ks) ? 1u : 0u);
+                            }
                         }
                     }
+                    ptx::mma_commit(b_empty0 + 8 * slot);        // e / o may be overwritten once these MMAs have read them
+                    ptx::mma_commit(acc_full0 + 8 * slot);
                 }
-                ptx::mma_commit(b_empty0 + 8 * slot);        // e / o may be overwritten once these MMAs have read them
-                ptx::mma_commit(acc_full0 + 8 * slot);
+                __syncwarp();
                 if (++slot == 2) { slot = 0; phase ^= 1u; }
             }
         }
-    } else if (warp < 6) {
+    } else if (warp < 2 + kFoldWarps) {
         // ===================== fold + convert: raw int8 -> e, o (fp16, K-major SWIZZLE_128B) =====================
-        {   // the twiddle matrices into tensor memory, once: row (channel) 32 (warp % 4) + lane of every matrix
+        if (warp < 6) {   // the twiddle matrices into tensor memory, once: row (channel) 32 (warp % 4) + lane of every matrix
             const int krow = (warp & 3) * 32 + lane;
 #pragma unroll 1
             for (int m = 0; m < 4; ++m) {
@@ -203,20 +218,20 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(a_full);
         }
-        const int ct = threadIdx.x - 64;                    // 0 .. 127
+        const int ct = threadIdx.x - 64;                    // 0 .. 255
         const int j = ct & 7;                                // samples n = 16 j .. 16 j + 15 of the stream
-        int slot = 0;
-        uint32_t phase = 0;                                  // raw slot, B slot and their phases advance together
+        int slot = 0, rslot = 0;
+        uint32_t phase = 0, rphase = 0;                      // B slot / raw slot and their phases
         long long it_tile = 0;
         for (long long t = first; t < prm.n_tiles; t += step, ++it_tile) {
-            ptx::mbar_wait(raw_full0 + 8 * slot, phase);
+            ptx::mbar_wait(raw_full0 + 8 * rslot, rphase);
             ptx::mbar_wait(b_empty0 + 8 * slot, phase ^ 1u); // the MMAs of two tiles ago have read this e / o slot
-            const uint32_t raw = base + kOffRaw + slot * kRawBytes;
+            const uint32_t raw = base + kOffRaw + rslot * kRawBytes;
             const uint32_t opb = base + slot * 2 * kOpBytes;
             const uint32_t s128 = base + kOffS128 + static_cast<uint32_t>(it_tile & (kS128Ring - 1)) * (kTileStreams * 4);
 #pragma unroll
-            for (int rep = 0; rep < 4; ++rep) {
-                const int r = (ct >> 3) + 16 * rep;          // stream within the tile
+            for (int rep = 0; rep < kTileStreams / (4 * kFoldWarps); ++rep) {
+                const int r = (ct >> 3) + 4 * kFoldWarps * rep;   // stream within the tile
                 const uint32_t row = raw + r * kFft;
                 const uint4 f = lds_v4(row + 16 * j);                          // s[16 j + 0 .. 15]
                 const uint4 b = lds_v4(row + 240 - 16 * j);                    // s[240 - 16 j + 0 .. 15]
@@ -252,16 +267,18 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
             __syncwarp();
             if (lane == 0) {
                 ptx::mbar_arrive(b_full0 + 8 * slot);
-                ptx::mbar_arrive(raw_empty0 + 8 * slot);
+                ptx::mbar_arrive(raw_empty0 + 8 * rslot);
             }
             if (++slot == 2) { slot = 0; phase ^= 1u; }
+            if (++rslot == kRawRing) { rslot = 0; rphase ^= 1u; }
         }
     } else {
         // ===================== epilogue =====================
         const int quarter = warp & 3;                        // TMEM lanes [32 quarter, +32) = channels
         const int k = quarter * 32 + lane;                   // this thread's channel
         const float sgn = (k & 1) ? -1.0f : 1.0f;
-        const uint32_t stage = base + kOffStage + (warp - 6) * kStageWarpBytes;
+        const int hh = (warp - 2 - kFoldWarps) >> 2;        // this warp's 32 streams of the tile
+        const uint32_t stage = base + kOffStage + (warp - 2 - kFoldWarps) * kStageWarpBytes;
         __half2* out = static_cast<__half2*>(prm.out);
         uint32_t acc_phase = 0;
         int acc = 0;
@@ -273,17 +290,14 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
             ptx::mbar_wait(acc_full0 + 8 * acc, acc_phase);
             ptx::tc_fence_after();
             const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + kTmemAcc + acc * 128;
-#pragma unroll
-            for (int hh = 0; hh < 2; ++hh) {                 // 32 streams at a time
+            {
                 uint32_t re[32], im[32];
                 ptx::tmem_ld_32x32(taddr + 32 * hh, re);
                 ptx::tmem_ld_32x32(taddr + 64 + 32 * hh, im);
                 ptx::tmem_ld_wait();
-                if (hh == 1) {                               // both halves are in registers: the accumulator is free
-                    ptx::tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) ptx::mbar_arrive(acc_empty0 + 8 * acc);
-                }
+                ptx::tc_fence_before();                      // this warp's part is in registers
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(acc_empty0 + 8 * acc);
                 uint32_t h[32];
 #pragma unroll
                 for (int c4 = 0; c4 < 8; ++c4) {
@@ -297,7 +311,7 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
                     }
                 }
                 // transpose through shared memory: row = channel (this lane), 32 streams x 4 bytes
-                __syncwarp();                                // the previous half has been read out of the staging rows
+                __syncwarp();                                // the previous tile has been read out of the staging rows
 #pragma unroll
                 for (int c4 = 0; c4 < 8; ++c4)
                     sts_v4(stage + lane * kStageRow + 16 * c4, h[4 * c4], h[4 * c4 + 1], h[4 * c4 + 2], h[4 * c4 + 3]);

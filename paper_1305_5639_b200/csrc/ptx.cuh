@@ -49,6 +49,19 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     }
 }
 
+// One lane of a CONVERGED warp (deterministic for a given member mask).  Single-thread instructions (tcgen05.mma,
+// tcgen05.commit, TMA) are issued as `if (elect_one()) {...}` inside warp-uniform control flow: the compiler then keeps
+// their descriptor / address operands in uniform registers and emits the instructions back to back.  Under a divergent
+// `if (lane == 0)` it cannot prove the operands uniform and wraps EVERY such instruction in an elect / R2UR / branch loop
+// (~90 clk per tcgen05.mma: the F-engine's 32-clk MMAs were issue-bound at 2.8x their tensor time).
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
+// a value every lane holds identically, made provably warp-uniform for the compiler (loads from memory are not)
+__device__ __forceinline__ uint32_t uniform(uint32_t v) { return __shfl_sync(0xffffffffu, v, 0); }
+
 // ---- TMA --------------------------------------------------------------------------------
 __device__ __forceinline__ void prefetch_tensormap(const CUtensorMap* map) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(map)) : "memory");
