@@ -144,17 +144,20 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
     const long long first = blockIdx.x, step = gridDim.x;
 
     if (warp == 0) {
-        // ===================== TMA producer =====================
-        if (lane == 0) {
+        // ===================== TMA producer (one elected lane of the converged warp) =====================
+        {
             int slot = 0;
             uint32_t phase = 0;
             for (long long t = first; t < prm.n_tiles; t += step) {
                 const long long a = t / n_sb;
                 const int m0 = static_cast<int>(t - a * n_sb) * kTileStreams;
                 ptx::mbar_wait(raw_empty0 + 8 * slot, phase ^ 1u);
-                ptx::mbar_arrive_expect_tx(raw_full0 + 8 * slot, kRawBytes);
-                // the sample axis is cut into [spectrum][256] (rank 3), so a box never needs a coordinate beyond 2^31
-                ptx::tma_load_3d(base + kOffRaw + slot * kRawBytes, &tmap_raw, raw_full0 + 8 * slot, 0, static_cast<int>(a), m0);
+                if (ptx::elect_one()) {
+                    ptx::mbar_arrive_expect_tx(raw_full0 + 8 * slot, kRawBytes);
+                    // the sample axis is cut into [spectrum][256] (rank 3), so a box never needs a coordinate beyond 2^31
+                    ptx::tma_load_3d(base + kOffRaw + slot * kRawBytes, &tmap_raw, raw_full0 + 8 * slot, 0, static_cast<int>(a), m0);
+                }
+                __syncwarp();
                 if (++slot == kRawRing) { slot = 0; phase ^= 1u; }
             }
         }

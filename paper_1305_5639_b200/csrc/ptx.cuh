@@ -53,7 +53,9 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 // tcgen05.commit, TMA) are issued as `if (elect_one()) {...}` inside warp-uniform control flow: the compiler then keeps
 // their descriptor / address operands in uniform registers and emits the instructions back to back.  Under a divergent
 // `if (lane == 0)` it cannot prove the operands uniform and wraps EVERY such instruction in an elect / R2UR / branch loop
-// (~90 clk per tcgen05.mma: the F-engine's 32-clk MMAs were issue-bound at 2.8x their tensor time).
+// (~90 clk per tcgen05.mma: the F-engine's 32-clk MMAs were issue-bound at 2.8x their tensor time).  The barrier waits
+// of such a warp are polled by ALL its lanes: letting only the elected lane poll and parking the others at __syncwarp
+// was measured 7 - 10 % slower on configs 2 / 4 / 5 (the wake-up -> warp barrier -> elect chain sits on the critical path).
 __device__ __forceinline__ bool elect_one() {
     uint32_t pred;
     asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));

@@ -12,9 +12,9 @@
 // the multicast saves L2 reads, not bytes delivered to each SM, and couples the two pipelines -- and removed.)
 //
 // Roles per CTA (320 threads, one CTA per SM, persistent; the tiles come from the dynamic TileFeed below):
-//   warp 0      TMA producer (one lane): its 128 A rows and its 128 B columns of every pipeline stage; completion
+//   warp 0      TMA producer (one elected lane of the converged warp): its 128 A rows and its 128 B columns of every pipeline stage; completion
 //               bytes of both CTAs are counted on the pair LEADER's `full` barrier
-//   warp 1      TMEM allocator (both CTAs) + tcgen05.mma.cta_group::2 issuer (one lane of the leader CTA);
+//   warp 1      TMEM allocator (both CTAs) + tcgen05.mma.cta_group::2 issuer (one elected lane of the leader CTA's warp);
 //               tcgen05.commit multicasts the `empty` and `tmem full` arrivals to both CTAs;
 //               in cluster rank 1 (no MMAs to issue) the same lane is the tile-feed writer
 //   warps 2..9  epilogue of this CTA's 128 TMEM lanes (drain_accumulator in xengine_tc.cuh); they release the
@@ -90,6 +90,10 @@ struct TileFeed {
         advance();
         return g;
     }
+    // a whole (converged) warp whose control flow must stay provably warp-uniform (TMA producer, MMA issuer)
+    __device__ __forceinline__ long long next_uniform(int lane) {
+        return ptx::uniform(static_cast<uint32_t>(next_warp(lane)));
+    }
     // the writer (one thread of cluster rank 1; `free0_local` is its own barrier): same slot/phase bookkeeping
     __device__ __forceinline__ void publish(uint32_t g, uint32_t free0_local) {
         ptx::mbar_wait(free0_local + 8u * slot, phase ^ 1u);         // every consumer of the cluster has read the old value
@@ -142,9 +146,11 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const __grid_co
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
-    const int half = static_cast<int>(ptx::cluster_ctarank());      // 0 = pair leader (issues the MMAs)
-    const long long cluster_id = ptx::cluster_id_x();
-    const long long n_clusters = ptx::cluster_count_x();
+    // (special registers read through asm: made provably warp-uniform so that the single-thread instruction streams below
+    // keep their operands in uniform registers, see ptx::elect_one)
+    const int half = static_cast<int>(ptx::uniform(ptx::cluster_ctarank()));      // 0 = pair leader (issues the MMAs)
+    const long long cluster_id = ptx::uniform(ptx::cluster_id_x());
+    const long long n_clusters = ptx::uniform(ptx::cluster_count_x());
 
     if (threadIdx.x == 0) {
         ptx::prefetch_tensormap(&tmap_in);
@@ -180,56 +186,61 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const __grid_co
     const int M2b = rect ? 2 * prm.M_b : M2;                   // G columns per channel
 
     if (warp == 0) {
-        // ===================== TMA producer =====================
-        if (lane == 0) {
+        // ===================== TMA producer (whole warp in uniform control flow, one elected lane issues) =====================
+        {
             int stage = 0;
             uint32_t phase = 0;
             TileFeed feed(feed_full0, feed_free0, feed_slot0);
-            for (long long g = cluster_id; g < pp.n_tiles; g = feed.next()) {
+            for (long long g = cluster_id; g < pp.n_tiles; g = feed.next_uniform(lane)) {
                 const int cd = static_cast<int>(g / pp.tiles_per_chan);             // integration * C + channel
-                const PairTile td = pp.tiles[g - static_cast<long long>(cd) * pp.tiles_per_chan];
+                const PairTile* tdp = pp.tiles + (g - static_cast<long long>(cd) * pp.tiles_per_chan);
+                const int row0 = static_cast<int>(ptx::uniform(tdp->row0)), col0 = static_cast<int>(ptx::uniform(tdp->col0));
                 const int dump = cd / prm.n_chan, c = prm.chan0 + (cd - dump * prm.n_chan);
-                const int w_a = c * M2 + td.row0 + 128 * half;      // this CTA's A rows in the [n_dump][T][C*2M] view
-                const int w_b = c * M2b + td.col0 + 128 * half;     // this CTA's half of the B columns
+                const int w_a = c * M2 + row0 + 128 * half;         // this CTA's A rows in the [n_dump][T][C*2M] view
+                const int w_b = c * M2b + col0 + 128 * half;        // this CTA's half of the B columns
                 // diagonal tile: this CTA's half of the B columns IS its 128 A rows -> one load serves both operands
-                const bool diag = !rect && td.row0 == td.col0;
+                const bool diag = !rect && row0 == col0;
                 for (int kb = 0; kb < num_kb; ++kb) {
                     ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
                     const uint32_t sa = smem_base + stage * kPairStageBytes;
                     const uint32_t sb = sa + kOpChunks * kChunkBytes;
-                    if (half == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), diag ? kPairStageBytes : 2u * kPairStageBytes);
-#pragma unroll
-                    for (int ch = 0; ch < kOpChunks; ++ch)
-#pragma unroll
-                        for (int b = 0; b < kPairBoxes; ++b)
-                            ptx::tma_load_3d_pair(sa + ch * kChunkBytes + b * kBoxBytes, &tmap_in, full_bar(stage),
-                                                  w_a + ch * kChunkElems, kb * kStageK + b * kBoxRows, dump);
-                    if (!diag) {
+                    if (ptx::elect_one()) {
+                        if (half == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), diag ? kPairStageBytes : 2u * kPairStageBytes);
 #pragma unroll
                         for (int ch = 0; ch < kOpChunks; ++ch)
 #pragma unroll
                             for (int b = 0; b < kPairBoxes; ++b)
-                                ptx::tma_load_3d_pair(sb + ch * kChunkBytes + b * kBoxBytes, &tmap_b, full_bar(stage),
-                                                      w_b + ch * kChunkElems, kb * kStageK + b * kBoxRows, dump);
+                                ptx::tma_load_3d_pair(sa + ch * kChunkBytes + b * kBoxBytes, &tmap_in, full_bar(stage),
+                                                      w_a + ch * kChunkElems, kb * kStageK + b * kBoxRows, dump);
+                        if (!diag) {
+#pragma unroll
+                            for (int ch = 0; ch < kOpChunks; ++ch)
+#pragma unroll
+                                for (int b = 0; b < kPairBoxes; ++b)
+                                    ptx::tma_load_3d_pair(sb + ch * kChunkBytes + b * kBoxBytes, &tmap_b, full_bar(stage),
+                                                          w_b + ch * kChunkElems, kb * kStageK + b * kBoxRows, dump);
+                        }
                     }
+                    __syncwarp();
                     if (++stage == kPairStages) { stage = 0; phase ^= 1u; }
                 }
             }
         }
     } else if (warp == 1) {
-        // ===================== MMA issuer (pair leader only) =====================
-        if (lane == 0 && half == 0) {
+        // ===================== MMA issuer (pair leader only; whole warp in uniform control flow, one elected lane issues) ==
+        if (half == 0) {
+            const uint32_t tb = ptx::uniform(tmem_base);
             int stage = 0;
             uint32_t phase = 0;
             int acc = 0;
             uint32_t acc_phase = 0;
             TileFeed feed(feed_full0, feed_free0, feed_slot0);
-            for (long long g = cluster_id; g < pp.n_tiles; g = feed.next()) {
-                const PairTile td = pp.tiles[g % pp.tiles_per_chan];
-                const bool diag = !rect && td.row0 == td.col0;      // B operand = the A buffer
+            for (long long g = cluster_id; g < pp.n_tiles; g = feed.next_uniform(lane)) {
+                const PairTile* tdp = pp.tiles + g % pp.tiles_per_chan;
+                const bool diag = !rect && ptx::uniform(tdp->row0) == ptx::uniform(tdp->col0);      // B operand = the A buffer
                 for (int kb0 = 0; kb0 < num_kb; kb0 += kb_per_chunk) {
                     const int kb1 = kb0 + kb_per_chunk < num_kb ? kb0 + kb_per_chunk : num_kb;
-                    const uint32_t d_tmem = tmem_base + acc * kTileCols;
+                    const uint32_t d_tmem = tb + acc * kTileCols;
                     ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1u);     // both CTAs' epilogues have drained it
                     ptx::tc_fence_after();
                     for (int kb = kb0; kb < kb1; ++kb) {
@@ -237,22 +248,25 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const __grid_co
                         ptx::tc_fence_after();
                         const uint32_t sa = smem_base + stage * kPairStageBytes;
                         const uint32_t sb = diag ? sa : sa + kOpChunks * kChunkBytes;
+                        if (ptx::elect_one()) {
 #pragma unroll
-                        for (int k = 0; k < kKSteps; ++k) {
-                            const uint64_t adesc = ptx::smem_desc_sw128(sa + k * kKStepBytes, kChunkBytes, 1024);
-                            const uint64_t bdesc = ptx::smem_desc_sw128(sb + k * kKStepBytes, kChunkBytes, 1024);
-                            const uint32_t accum = (kb != kb0 || k != 0) ? 1u : 0u;
-                            if constexpr (C::kFloat) ptx::mma_f16_pair(d_tmem, adesc, bdesc, kIdesc, accum);
-                            else ptx::mma_i8_pair(d_tmem, adesc, bdesc, kIdesc, accum);
+                            for (int k = 0; k < kKSteps; ++k) {
+                                const uint64_t adesc = ptx::smem_desc_sw128(sa + k * kKStepBytes, kChunkBytes, 1024);
+                                const uint64_t bdesc = ptx::smem_desc_sw128(sb + k * kKStepBytes, kChunkBytes, 1024);
+                                const uint32_t accum = (kb != kb0 || k != 0) ? 1u : 0u;
+                                if constexpr (C::kFloat) ptx::mma_f16_pair(d_tmem, adesc, bdesc, kIdesc, accum);
+                                else ptx::mma_i8_pair(d_tmem, adesc, bdesc, kIdesc, accum);
+                            }
+                            ptx::mma_commit_pair_mc(empty_bar(stage), kPairMask);  // slot free in both CTAs
+                            if (kb + 1 == kb1) ptx::mma_commit_pair_mc(tfull_bar(acc), kPairMask);   // accumulator complete in both CTAs
                         }
-                        ptx::mma_commit_pair_mc(empty_bar(stage), kPairMask);  // slot free in both CTAs
+                        __syncwarp();
                         if (++stage == kPairStages) { stage = 0; phase ^= 1u; }
                     }
-                    ptx::mma_commit_pair_mc(tfull_bar(acc), kPairMask);        // accumulator complete in both CTAs
                     if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
                 }
             }
-        } else if (lane == 0 && half == 1) {
+        } else if (lane == 0) {
             // ===================== tile-feed writer (this CTA issues no MMAs) =====================
             TileFeed feed(feed_full0, feed_free0, feed_slot0);
             for (;;) {

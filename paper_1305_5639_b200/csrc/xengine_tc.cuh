@@ -15,8 +15,8 @@
 // one shuffle between adjacent TMEM lanes and streams the packed triangle to HBM.
 //
 // Warp roles (320 threads, 1 CTA / SM, persistent over a static round-robin of tiles):
-//   warp 0      TMA producer  (one lane)
-//   warp 1      TMEM allocator + tcgen05.mma issuer (one lane)
+//   warp 0      TMA producer  (one elected lane of the converged warp, see ptx::elect_one)
+//   warp 1      TMEM allocator + tcgen05.mma issuer (one elected lane)
 //   warps 2..9  epilogue: tcgen05.ld -> combine -> shared-memory staging in packed-baseline order ->
 //               bulk async store (or bulk reduce-add when accumulating) of whole station-row segments.
 //               Warp w owns TMEM lanes 32 (w % 4) .. +31 and the column half (w - 2) / 4 of the tile.
@@ -401,76 +401,87 @@ xengine_direct_kernel(const __grid_constant__ CUtensorMap tmap_in, const Params 
     const int M2 = 2 * prm.M;
 
     if (warp == 0) {
-        // ===================== TMA producer =====================
-        if (lane == 0) {
+        // ===================== TMA producer (whole warp in uniform control flow, one elected lane issues) =====================
+        {
             int stage = 0;
             uint32_t phase = 0;
             for (long long tile = blockIdx.x; tile < prm.n_tiles; tile += gridDim.x) {
                 const int c = static_cast<int>(tile / prm.tiles_per_chan);
-                const TileDesc td = prm.tiles[tile - static_cast<long long>(c) * prm.tiles_per_chan];
-                const int w_row = (prm.chan0 + c) * M2 + td.row0;        // element coordinate in the [T][C*2M] view
-                const int w_col = (prm.chan0 + c) * M2 + td.col0;
-                const int nb = (td.ncols + kChunkElems - 1) / kChunkElems;
+                const TileDesc* tdp = prm.tiles + (tile - static_cast<long long>(c) * prm.tiles_per_chan);
+                const int row0 = static_cast<int>(ptx::uniform(tdp->row0)), col0 = static_cast<int>(ptx::uniform(tdp->col0));
+                const int ncols = static_cast<int>(ptx::uniform(tdp->ncols));
+                const int w_row = (prm.chan0 + c) * M2 + row0;           // element coordinate in the [T][C*2M] view
+                const int w_col = (prm.chan0 + c) * M2 + col0;
+                const int nb = (ncols + kChunkElems - 1) / kChunkElems;
                 // tile on the diagonal: the 128 A rows are among the loaded B columns -> A is not loaded at all
-                const bool a_in_b = td.row0 >= td.col0 && td.row0 + kTileRows <= td.col0 + nb * kChunkElems;
+                const bool a_in_b = row0 >= col0 && row0 + kTileRows <= col0 + nb * kChunkElems;
                 const uint32_t tx = static_cast<uint32_t>(((a_in_b ? 0 : kAChunks) + nb) * kChunkBytes);
                 for (int kb = 0; kb < num_kb; ++kb) {
                     ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
                     const uint32_t sb = smem_base + stage * kStageBytes;
                     const uint32_t sa = sb + prm.b_chunks * kChunkBytes;
-                    ptx::mbar_arrive_expect_tx(full_bar(stage), tx);
+                    if (ptx::elect_one()) {
+                        ptx::mbar_arrive_expect_tx(full_bar(stage), tx);
 #pragma unroll
-                    for (int a = 0; a < kAChunks; ++a)
-                        if (!a_in_b)
-                            ptx::tma_load_3d(sa + a * kChunkBytes, &tmap_in, full_bar(stage),
-                                             w_row + a * kChunkElems, kb * C::kKStage, 0);
+                        for (int a = 0; a < kAChunks; ++a)
+                            if (!a_in_b)
+                                ptx::tma_load_3d(sa + a * kChunkBytes, &tmap_in, full_bar(stage),
+                                                 w_row + a * kChunkElems, kb * C::kKStage, 0);
 #pragma unroll
-                    for (int b = 0; b < kBChunksMax; ++b)
-                        if (b < nb)
-                            ptx::tma_load_3d(sb + b * kChunkBytes, &tmap_in, full_bar(stage),
-                                             w_col + b * kChunkElems, kb * C::kKStage, 0);
+                        for (int b = 0; b < kBChunksMax; ++b)
+                            if (b < nb)
+                                ptx::tma_load_3d(sb + b * kChunkBytes, &tmap_in, full_bar(stage),
+                                                 w_col + b * kChunkElems, kb * C::kKStage, 0);
+                    }
+                    __syncwarp();
                     if (++stage == kNumStages) { stage = 0; phase ^= 1u; }
                 }
             }
         }
     } else if (warp == 1) {
-        // ===================== MMA issuer =====================
-        if (lane == 0) {
+        // ===================== MMA issuer (whole warp in uniform control flow, one elected lane issues) =====================
+        {
+            const uint32_t tb = ptx::uniform(tmem_base);
             int stage = 0;
             uint32_t phase = 0;
             int acc = 0;
             uint32_t acc_phase = 0;
             for (long long tile = blockIdx.x; tile < prm.n_tiles; tile += gridDim.x) {
                 const int c = static_cast<int>(tile / prm.tiles_per_chan);
-                const TileDesc td = prm.tiles[tile - static_cast<long long>(c) * prm.tiles_per_chan];
-                const uint32_t idesc = C::kIdesc | (static_cast<uint32_t>(td.ncols >> 3) << 17);
-                const int nb = (td.ncols + kChunkElems - 1) / kChunkElems;
-                const bool a_in_b = td.row0 >= td.col0 && td.row0 + kTileRows <= td.col0 + nb * kChunkElems;
+                const TileDesc* tdp = prm.tiles + (tile - static_cast<long long>(c) * prm.tiles_per_chan);
+                const int row0 = static_cast<int>(ptx::uniform(tdp->row0)), col0 = static_cast<int>(ptx::uniform(tdp->col0));
+                const int ncols = static_cast<int>(ptx::uniform(tdp->ncols));
+                const uint32_t idesc = C::kIdesc | (static_cast<uint32_t>(ncols >> 3) << 17);
+                const int nb = (ncols + kChunkElems - 1) / kChunkElems;
+                const bool a_in_b = row0 >= col0 && row0 + kTileRows <= col0 + nb * kChunkElems;
                 // A operand = the B chunks holding rows row0 .. row0 + 127 when the tile lies on the diagonal
-                const uint32_t a_off = (a_in_b ? (td.row0 - td.col0) / kChunkElems : prm.b_chunks) * kChunkBytes;
+                const uint32_t a_off = (a_in_b ? (row0 - col0) / kChunkElems : prm.b_chunks) * kChunkBytes;
                 for (int kb0 = 0; kb0 < num_kb; kb0 += kb_per_chunk) {
                     const int kb1 = kb0 + kb_per_chunk < num_kb ? kb0 + kb_per_chunk : num_kb;
-                    const uint32_t d_tmem = tmem_base + acc * kTileCols;
+                    const uint32_t d_tmem = tb + acc * kTileCols;
                     ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1u);     // epilogue has drained this accumulator
                     ptx::tc_fence_after();
                     for (int kb = kb0; kb < kb1; ++kb) {
                         ptx::mbar_wait(full_bar(stage), phase);          // TMA bytes have landed
                         ptx::tc_fence_after();
                         const uint32_t sb = smem_base + stage * kStageBytes;
+                        if (ptx::elect_one()) {
 #pragma unroll
-                        for (int k = 0; k < kKSteps; ++k) {
-                            // MN-major SWIZZLE_128B: LBO = distance between 128-byte-wide chunks (one TMA box),
-                            // SBO = distance between 8-row groups along K (8 * 128 B).
-                            const uint64_t adesc = ptx::smem_desc_sw128(sb + a_off + k * kKStepBytes, kChunkBytes, 1024);
-                            const uint64_t bdesc = ptx::smem_desc_sw128(sb + k * kKStepBytes, kChunkBytes, 1024);
-                            const uint32_t accum = (kb != kb0 || k != 0) ? 1u : 0u;
-                            if constexpr (C::kFloat) ptx::mma_f16(d_tmem, adesc, bdesc, idesc, accum);
-                            else ptx::mma_i8(d_tmem, adesc, bdesc, idesc, accum);
+                            for (int k = 0; k < kKSteps; ++k) {
+                                // MN-major SWIZZLE_128B: LBO = distance between 128-byte-wide chunks (one TMA box),
+                                // SBO = distance between 8-row groups along K (8 * 128 B).
+                                const uint64_t adesc = ptx::smem_desc_sw128(sb + a_off + k * kKStepBytes, kChunkBytes, 1024);
+                                const uint64_t bdesc = ptx::smem_desc_sw128(sb + k * kKStepBytes, kChunkBytes, 1024);
+                                const uint32_t accum = (kb != kb0 || k != 0) ? 1u : 0u;
+                                if constexpr (C::kFloat) ptx::mma_f16(d_tmem, adesc, bdesc, idesc, accum);
+                                else ptx::mma_i8(d_tmem, adesc, bdesc, idesc, accum);
+                            }
+                            ptx::mma_commit(empty_bar(stage));               // frees the smem slot when the MMAs retire
+                            if (kb + 1 == kb1) ptx::mma_commit(tfull_bar(acc));   // accumulator complete -> epilogue
                         }
-                        ptx::mma_commit(empty_bar(stage));               // frees the smem slot when the MMAs retire
+                        __syncwarp();
                         if (++stage == kNumStages) { stage = 0; phase ^= 1u; }
                     }
-                    ptx::mma_commit(tfull_bar(acc));                     // accumulator complete -> epilogue
                     if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
                 }
             }
