@@ -26,15 +26,18 @@ namespace xtc {
 
 constexpr int kPairRows = 256;                 // G rows per pair tile
 constexpr int kPairBoxes = 1;                  // TMA boxes stacked along time per 128-byte chunk of a pipeline stage
-// Three stages of 64 KB: one 32 KB TMA box per operand chunk and 8 MMAs per stage.  Measured against six stages of 32 KB
-// (16 KB boxes, 4 MMAs per stage): 8 - 15 % fewer SM cycles per call on configs 3 / 4 / 5 (profiles/r2_*): the per-box
-// and per-stage costs (TMA issue, barrier round trips, commits) halve, and three stages still cover the L2 latency.
-constexpr int kPairStageBytes = 64 * 1024;     // per CTA and stage: A 128 components + B 128 components, kPairStageK samples
-template <int kElt> constexpr int kPairStageK = kPairStageBytes / (2 * 128 * kElt);    // 256 (ci8) / 128 (cf16) samples
+// Six stages of 32 KB: one 16 KB TMA box per operand chunk and 4 MMAs per stage.  History: round 1 had 6 x 32 KB; while the
+// MMAs were issued from a divergent `if (lane == 0)` (an elect / R2UR loop of ~90 clk around every instruction) four MMAs
+// plus the stage's barrier traffic did not fit into the 512 clk they execute in, and three stages of 64 KB (8 MMAs) were
+// 8 - 15 % fewer cycles.  With the issue in uniform control flow (ptx::elect_one) that cost is gone and the finer ring wins:
+// 160 instead of 128 KB of operands in flight per CTA while a stage is consumed (the load latency of ~2000 clk is the
+// ring's whole period), measured +5 % cross-only, +3 % N = 128, +2 - 4 % fp16, +1 % config 4 / N = 1024.  (12 x 16 KB: -10 %.)
+constexpr int kPairStageBytes = 32 * 1024;     // per CTA and stage: A 128 components + B 128 components, kPairStageK samples
+template <int kElt> constexpr int kPairStageK = kPairStageBytes / (2 * 128 * kElt);    // 128 (ci8) / 64 (cf16) samples
 constexpr int kPairEpiBufs = 1;                // staging buffers per epilogue warp (a second one costs two pipeline stages)
 constexpr int kPairEpiWarpBytes = kPairEpiBufs * kEpiBufBytes;
 constexpr int kPairEpiBytes = kNumEpiWarps * kPairEpiWarpBytes;
-constexpr int kPairStages = 3;
+constexpr int kPairStages = 6;
 // the dynamic shared memory window of a kernel without static shared memory starts 1024-byte aligned (checked
 // in the kernel), so no alignment slack is reserved
 constexpr int kPairSmemBytes = kPairStages * kPairStageBytes + kPairEpiBytes + 256 /*barriers*/;
