@@ -122,8 +122,8 @@ EncodeTiledFn get_encode_fn() {
     return reinterpret_cast<EncodeTiledFn>(fn);
 }
 
-// Tensor-core F-engine (fengine_tc.cuh): per-device twiddle table [cos_hi | cos_lo | -sin_hi | -sin_lo], each
-// [128 channels][128 folded samples] fp16, and its tensor map; built on first use.
+// Tensor-core F-engine (fengine_tc.cuh): per-device twiddle table [cos_hi | cos_lo | -sin_hi | -sin_lo | nyquist], each
+// [128 channels][128 folded samples] fp16 (nyquist: (-1)^k in sample slot 0, zero elsewhere); built on first use.
 struct FengTcState {
     bool tried = false, ok = false;
     void* d_tw = nullptr;
@@ -146,7 +146,7 @@ FengTcState* fengine_tc_state() {
     st.encode = get_encode_fn();
     if (!st.encode) return nullptr;
     // hi = fp16(w), lo = fp16(w - hi): w = hi + lo to ~3e-8 absolute (lo may be subnormal)
-    std::vector<__half> tw(4 * fengtc::kChan * fengtc::kFold);
+    std::vector<__half> tw(fengtc::kNumMats * fengtc::kChan * fengtc::kFold, __float2half_rn(0.0f));
     const double two_pi = 6.283185307179586476925286766559;
     for (int k = 0; k < fengtc::kChan; ++k)
         for (int n = 0; n < fengtc::kFold; ++n) {
@@ -160,6 +160,7 @@ FengTcState* fengine_tc_state() {
                 tw[((2 * part + 1) * fengtc::kChan + k) * fengtc::kFold + n] = lo;
             }
         }
+    for (int k = 0; k < fengtc::kChan; ++k) tw[(4 * fengtc::kChan + k) * fengtc::kFold] = __float2half_rn((k & 1) ? -1.0f : 1.0f);
     if (cudaMalloc(&st.d_tw, tw.size() * sizeof(__half)) != cudaSuccess) { cudaGetLastError(); return nullptr; }
     if (cudaMemcpy(st.d_tw, tw.data(), tw.size() * sizeof(__half), cudaMemcpyHostToDevice) != cudaSuccess) return nullptr;
     if (cudaFuncSetAttribute(fengtc::fengine_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, fengtc::kSmemBytes) != cudaSuccess) {
@@ -668,13 +669,13 @@ static bool fengine_tc_applies(const void* out, int n_stream, bool int8_out) {
 }
 
 static int run_fengine_tc(FengTcState* st, const void* in, void* out, int n_stream, long long n_spectra, cudaStream_t stream) {
-    CUtensorMap map_raw;       // in viewed as [n_stream][n_spectra][256] bytes, box = 64 streams x 1 spectrum x 256 samples
+    CUtensorMap map_raw;       // in viewed as [n_stream][n_spectra][256] bytes, box = 64 streams x 1 spectrum x 128 samples
     cuuint64_t dims[3] = {fengtc::kFft, static_cast<cuuint64_t>(n_spectra), static_cast<cuuint64_t>(n_stream)};
     cuuint64_t strides[2] = {fengtc::kFft, static_cast<cuuint64_t>(n_spectra) * fengtc::kFft};
-    cuuint32_t box[3] = {fengtc::kFft, 1, fengtc::kTileStreams};
+    cuuint32_t box[3] = {fengtc::kFft / 2, 1, fengtc::kTileStreams};
     cuuint32_t estr[3] = {1, 1, 1};
     const CUresult r = st->encode(&map_raw, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(in), dims, strides, box, estr,
-                                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(nullptr, CORR_ECUDA, "corr_fengine: cuTensorMapEncodeTiled failed with CUresult %d", static_cast<int>(r));
     fengtc::Params prm;
@@ -682,7 +683,8 @@ static int run_fengine_tc(FengTcState* st, const void* in, void* out, int n_stre
     prm.tw = static_cast<const uint4*>(st->d_tw);
     prm.n_stream = n_stream;
     prm.n_spectra = n_spectra;
-    prm.n_tiles = n_spectra * (n_stream / fengtc::kTileStreams);
+    prm.n_half = n_spectra * (n_stream / fengtc::kTileStreams);
+    prm.n_tiles = (prm.n_half + 1) / 2;
     const long long grid = prm.n_tiles < st->sm_count ? prm.n_tiles : st->sm_count;
     fengtc::fengine_tc_kernel<<<static_cast<unsigned>(grid), fengtc::kThreads, fengtc::kSmemBytes, stream>>>(map_raw, prm);
     const cudaError_t e = cudaGetLastError();

@@ -61,6 +61,21 @@ __device__ __forceinline__ bool elect_one() {
     asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
     return pred != 0;
 }
+// Blocking wait of a whole converged warp that goes on to elect_one().  The poll result is put through a warp vote, so
+// the loop's branch is uniform IN HARDWARE, not only in the compiler's analysis: ptxas treats the predicate of
+// mbarrier.try_wait as warp-uniform when its operands are (it drops the reconvergence points and even __syncwarp() after
+// such a loop), but the lanes of one try_wait can come back with different answers when the phase flips while they are
+// suspended in it.  Lanes that then leave the loop in different iterations never reconverge, elect.sync elects one leader
+// per fragment and every TMA load / MMA / commit behind it is issued twice (seen as a sporadic launch failure of the
+// F-engine under full DRAM load, 1 launch in 15).
+__device__ __forceinline__ void mbar_wait_uniform(uint32_t bar, uint32_t parity) {
+    if (__all_sync(0xffffffffu, mbar_try_wait(bar, parity))) return;
+    const long long t0 = clock64();
+    uint32_t spins = 0;
+    while (!__all_sync(0xffffffffu, mbar_try_wait(bar, parity))) {
+        if ((++spins & 0x3ffu) == 0 && clock64() - t0 > (1ll << 33)) __trap();
+    }
+}
 // a value every lane holds identically, made provably warp-uniform for the compiler (loads from memory are not)
 __device__ __forceinline__ uint32_t uniform(uint32_t v) { return __shfl_sync(0xffffffffu, v, 0); }
 
@@ -199,6 +214,12 @@ __device__ __forceinline__ void tmem_st_32x32(uint32_t taddr, const uint32_t (&v
           "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31])
         : "memory");
 }
+// registers -> TMEM: this warp's 32 lanes x 8 consecutive 32-bit columns
+__device__ __forceinline__ void tmem_st_32x8(uint32_t taddr, const uint32_t (&v)[8]) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr), "r"(v[0]), "r"(v[1]),
+                 "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7])
+                 : "memory");
+}
 __device__ __forceinline__ void tmem_st_wait() {
     asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
@@ -283,6 +304,15 @@ __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity)
     const long long t0 = clock64();
     uint32_t spins = 0;
     while (!mbar_try_wait_cluster(bar, parity)) {
+        if ((++spins & 0x3ffu) == 0 && clock64() - t0 > (1ll << 33)) __trap();
+    }
+}
+// the same for a whole converged warp that stays in uniform control flow (see mbar_wait_uniform)
+__device__ __forceinline__ void mbar_wait_cluster_uniform(uint32_t bar, uint32_t parity) {
+    if (__all_sync(0xffffffffu, mbar_try_wait_cluster(bar, parity))) return;
+    const long long t0 = clock64();
+    uint32_t spins = 0;
+    while (!__all_sync(0xffffffffu, mbar_try_wait_cluster(bar, parity))) {
         if ((++spins & 0x3ffu) == 0 && clock64() - t0 > (1ll << 33)) __trap();
     }
 }

@@ -95,7 +95,12 @@ struct TileFeed {
     }
     // a whole (converged) warp whose control flow must stay provably warp-uniform (TMA producer, MMA issuer)
     __device__ __forceinline__ long long next_uniform(int lane) {
-        return ptx::uniform(static_cast<uint32_t>(next_warp(lane)));
+        ptx::mbar_wait_cluster_uniform(full0 + 8u * slot, phase);
+        const uint32_t g = ptx::ld_shared_u32(slot0 + 4u * slot);
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive_cluster_after(free0_writer + 8u * slot, g);
+        advance();
+        return ptx::uniform(g);
     }
     // the writer (one thread of cluster rank 1; `free0_local` is its own barrier): same slot/phase bookkeeping
     __device__ __forceinline__ void publish(uint32_t g, uint32_t free0_local) {
@@ -204,7 +209,7 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const __grid_co
                 // diagonal tile: this CTA's half of the B columns IS its 128 A rows -> one load serves both operands
                 const bool diag = !rect && row0 == col0;
                 for (int kb = 0; kb < num_kb; ++kb) {
-                    ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
+                    ptx::mbar_wait_uniform(empty_bar(stage), phase ^ 1u);
                     const uint32_t sa = smem_base + stage * kPairStageBytes;
                     const uint32_t sb = sa + kOpChunks * kChunkBytes;
                     if (ptx::elect_one()) {
@@ -244,10 +249,10 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const __grid_co
                 for (int kb0 = 0; kb0 < num_kb; kb0 += kb_per_chunk) {
                     const int kb1 = kb0 + kb_per_chunk < num_kb ? kb0 + kb_per_chunk : num_kb;
                     const uint32_t d_tmem = tb + acc * kTileCols;
-                    ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1u);     // both CTAs' epilogues have drained it
+                    ptx::mbar_wait_uniform(tempty_bar(acc), acc_phase ^ 1u);     // both CTAs' epilogues have drained it
                     ptx::tc_fence_after();
                     for (int kb = kb0; kb < kb1; ++kb) {
-                        ptx::mbar_wait(full_bar(stage), phase);          // both CTAs' operand bytes have landed
+                        ptx::mbar_wait_uniform(full_bar(stage), phase);          // both CTAs' operand bytes have landed
                         ptx::tc_fence_after();
                         const uint32_t sa = smem_base + stage * kPairStageBytes;
                         const uint32_t sb = diag ? sa : sa + kOpChunks * kChunkBytes;

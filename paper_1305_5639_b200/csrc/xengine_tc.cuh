@@ -417,7 +417,7 @@ xengine_direct_kernel(const __grid_constant__ CUtensorMap tmap_in, const Params 
                 const bool a_in_b = row0 >= col0 && row0 + kTileRows <= col0 + nb * kChunkElems;
                 const uint32_t tx = static_cast<uint32_t>(((a_in_b ? 0 : kAChunks) + nb) * kChunkBytes);
                 for (int kb = 0; kb < num_kb; ++kb) {
-                    ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
+                    ptx::mbar_wait_uniform(empty_bar(stage), phase ^ 1u);
                     const uint32_t sb = smem_base + stage * kStageBytes;
                     const uint32_t sa = sb + prm.b_chunks * kChunkBytes;
                     if (ptx::elect_one()) {
@@ -459,10 +459,10 @@ xengine_direct_kernel(const __grid_constant__ CUtensorMap tmap_in, const Params 
                 for (int kb0 = 0; kb0 < num_kb; kb0 += kb_per_chunk) {
                     const int kb1 = kb0 + kb_per_chunk < num_kb ? kb0 + kb_per_chunk : num_kb;
                     const uint32_t d_tmem = tb + acc * kTileCols;
-                    ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1u);     // epilogue has drained this accumulator
+                    ptx::mbar_wait_uniform(tempty_bar(acc), acc_phase ^ 1u);     // epilogue has drained this accumulator
                     ptx::tc_fence_after();
                     for (int kb = kb0; kb < kb1; ++kb) {
-                        ptx::mbar_wait(full_bar(stage), phase);          // TMA bytes have landed
+                        ptx::mbar_wait_uniform(full_bar(stage), phase);          // TMA bytes have landed
                         ptx::tc_fence_after();
                         const uint32_t sb = smem_base + stage * kStageBytes;
                         if (ptx::elect_one()) {

@@ -105,3 +105,29 @@ def test_cross_and_dumps_repeated(corr, oracle):
             assert (first[d].cpu().numpy().astype(np.int64) == oracle.xengine(x[d * 32:(d + 1) * 32].cpu().numpy())).all()
         for it in range(400):                                 # 1-stage tiles: the fastest tile turnover the feed sees
             assert torch.equal(h.xengine_dumps(x, 8), first)
+
+
+def test_fengine_tensor_core_long_queues_under_dram_load(corr):
+    """The tensor-core F-engine with hundreds of tiles per CTA, input and output far larger than L2, launched repeatedly:
+    TMA loads then complete out of order and the hand-overs of the raw ring, the A buffers in tensor memory and the two
+    accumulators see every interleaving.  (Round 2: waiting on a ring slot before the A buffer let a fast fold warp meet
+    the slot's barrier one phase behind -- 1 launch in 15 of this geometry failed, none of the small parity cases.)
+    Every launch must reproduce the first bit for bit, and the first must agree with the CUDA-core kernel."""
+    M, A = 512, 4096
+    g = torch.Generator(device="cuda")
+    g.manual_seed(8500)
+    s = torch.clamp(torch.round(torch.randn((M, A * 256), generator=g, device="cuda") * 20.0), -127, 127).to(torch.int8)
+    assert corr.fengine_uses_tensor_cores(M)
+    first = corr.fengine(s)
+    torch.cuda.synchronize()
+    ref = corr.fengine(s, simt=True)
+    # the two kernels round the same exact value through different fp32 sums: one fp16 ulp of the largest magnitude apart
+    d = (first.float() - ref.float()).abs().max().item()
+    assert d <= 2.0 * float(torch.finfo(torch.float16).eps) * ref.float().abs().max().item() + 1e-3
+    del ref
+    out = torch.empty_like(first)
+    for it in range(120):
+        corr.fengine(s, out)
+        if it % 20 == 19:
+            torch.cuda.synchronize()
+            assert torch.equal(out, first)
