@@ -51,12 +51,12 @@ FALLBACK_HBM_GBS = 6650.0
 # committed `ncu --set full` captures of the SAME kernel and geometry -- not measured by this run, and emitted only when
 # the kernel that ran is the one that was captured: workload -> (kernel, bytes, capture file)
 NCU_TRAFFIC = {
-    "cfg4": ("pair", (3.197e9 + 3 * 4.275e9) / 4, "profiles/r2_ncu_final.md"),      # accumulate = 0 once, = 1 three times
-    "cfg3": ("pair", 4.870e9, "profiles/r2_ncu_final.md"),
-    "cfg2": ("pair", 0.3165e9, "profiles/r2_ncu_final.md"),
-    "cfg5_n128": ("pair", 1.326e9, "profiles/r2_ncu_final.md"),
-    "cfg5_n1024": ("pair", 3.168e9, "profiles/r2_ncu_final.md"),
-    "cross_n256": ("pair", 3.190e9, "profiles/r2_ncu_final.md"),
+    "cfg4": ("pair", (3.198e9 + 3 * 4.275e9) / 4, "profiles/r2b_ncu_final.md"),     # accumulate = 0 once, = 1 three times
+    "cfg3": ("pair", 4.756e9, "profiles/r2b_ncu_final.md"),
+    "cfg2": ("pair", 0.3152e9, "profiles/r2b_ncu_final.md"),
+    "cfg5_n128": ("pair", 1.325e9, "profiles/r2b_ncu_final.md"),
+    "cfg5_n1024": ("pair", 3.168e9, "profiles/r2b_ncu_final.md"),
+    "cross_n256": ("pair", 3.190e9, "profiles/r2b_ncu_final.md"),
     "cfg5_n64": ("pair", 1.200e9, "profiles/r1c_final_ncu_pair_feed.md"),
     "cfg5_n32": ("single", 1.139e9, "profiles/r1c_final_ncu_pair_feed.md"),
 }
@@ -440,8 +440,8 @@ def time_fengine(pk, K, W, M=512, A=8192):
                        "gsamples_per_s": s.numel() / (ms * 1e-3) / 1e9},
             "gpu_launches": K,
             "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s", "frac": gbs / pk["hbm"],
-                         "traffic": 3.165e9 if (M, A) == (512, 8192) else None,
-                         "traffic_source": "profiles/r2_ncu_final.md (ncu capture of this kernel and geometry; NOT measured by this run)"
+                         "traffic": 3.169e9 if (M, A) == (512, 8192) else None,
+                         "traffic_source": "profiles/r2b_ncu_final.md (ncu capture of this kernel and geometry; NOT measured by this run)"
                          if (M, A) == (512, 8192) else None,
                          "kernel": "fengtc::fengine_tc_kernel" if binding.fengine_uses_tensor_cores(M, out) else "feng::fengine_kernel",
                          "kernel_ms": ms, "algorithmic_bytes_per_launch": nbytes}}

@@ -106,6 +106,10 @@ __device__ __forceinline__ uint32_t pack_half2(float lo, float hi) {
     asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
     return d;
 }
+// streaming store of one output word: written once, not read by this kernel: no L1 allocation, first in line for L2 eviction
+__device__ __forceinline__ void stg_stream(uint32_t* p, uint32_t v, uint64_t policy) {
+    asm volatile("st.global.L1::no_allocate.L2::cache_hint.b32 [%0], %1, %2;" ::"l"(p), "r"(v), "l"(policy) : "memory");
+}
 // a half tile in the raw ring (two SWIZZLE_128B boxes of [64 rows][128 bytes]): 16-byte unit u of row r of box b
 __device__ __forceinline__ uint32_t raw_unit(uint32_t slot_base, int b, int r, int u) {
     return slot_base + b * (kRawBytes / 2) + r * 128 + ((u ^ (r & 7)) << 4);
@@ -300,6 +304,7 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
         const int r = (quarter & 1) * 32 + lane;
         const uint32_t lane_addr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16);
         uint32_t* out = static_cast<uint32_t*>(prm.out);
+        const uint64_t policy = ptx::policy_evict_first();
         uint32_t it = 0;
         for (long long t = first; t < prm.n_tiles; t += step, ++it) {
             const long long hidx = 2 * t + h;
@@ -341,8 +346,8 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
                         const uint32_t ii = pack_half2(__uint_as_float(v[2 * c]), __uint_as_float(v[2 * c + 1]));
                         const uint32_t re2 = rr[16 * part + c];
                         // (re, im) half2 words of channels 2c and 2c + 1: one 128-byte line per channel and warp
-                        dst[static_cast<long long>(32 * part + 2 * c) * prm.n_stream] = __byte_perm(re2, ii, 0x5410);
-                        dst[static_cast<long long>(32 * part + 2 * c + 1) * prm.n_stream] = __byte_perm(re2, ii, 0x7632);
+                        stg_stream(dst + static_cast<long long>(32 * part + 2 * c) * prm.n_stream, __byte_perm(re2, ii, 0x5410), policy);
+                        stg_stream(dst + static_cast<long long>(32 * part + 2 * c + 1) * prm.n_stream, __byte_perm(re2, ii, 0x7632), policy);
                     }
                 }
             }
