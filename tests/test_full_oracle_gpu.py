@@ -7,7 +7,7 @@ Opt-in, because it is ~2.5e12 complex MACs on the host cores (about 5 - 8 minute
     CORR_FULL_ORACLE=cfg2,cfg5_n64 python -m pytest tests/test_full_oracle_gpu.py -m gpu -q
 
 int8 configs: bit-exact.  fp16 config: max over all visibilities of |dV| / sqrt(V_ii V_jj) <= 2e-5.
-The last recorded run is profiles/r2_full_oracle_parity.md.
+The last recorded run is profiles/r2b_full_oracle_parity.md.
 """
 import os
 import time
