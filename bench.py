@@ -73,7 +73,7 @@ def parse_args():
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
     ap.add_argument("--kernel", default="auto", choices=["auto", "single", "pair", "simt"],
                     help="force a kernel variant (default: the library's own choice)")
-    ap.add_argument("--piece", default="xengine", choices=["xengine", "corner_turn", "fengine"],
+    ap.add_argument("--piece", default="xengine", choices=["xengine", "corner_turn", "fengine", "fengine_ci8"],
                     help="corner_turn: time the standalone corner-turn kernel (SURVEY 8(a) a1) on the workload's input; "
                          "fengine: time corr_fengine (SURVEY 8(f) rank 2) on 512 streams x 8192 spectra of 256 real int8 samples")
     ap.add_argument("--shard", default="none", choices=["none", "channels"],
@@ -415,35 +415,37 @@ def time_corner_turn(cfg, pk, K, W, planes=1):
                          "algorithmic_bytes_per_launch": nbytes}}
 
 
-def time_fengine(pk, K, W, M=512, A=8192):
-    """corr_fengine alone: HBM-bound (1 byte read + 2 bytes written per real sample)."""
+def time_fengine(pk, K, W, M=512, A=8192, ci8=False):
+    """corr_fengine alone: HBM-bound (1 byte read + 2 bytes written per real sample; corr_fengine_ci8: 1 + 1)."""
     import torch
     from paper_1305_5639_b200 import binding
     g = torch.Generator(device="cuda"); g.manual_seed(1700)
     s = torch.clamp(torch.round(torch.randn((M, A * 256), generator=g, device="cuda") * 20.0), -127, 127).to(torch.int8)
-    out = binding.fengine(s)
+    scale = 1.0 / 20 if ci8 else None                # sigma ~ 16 codes per component, the int8 X-engine's input range
+    out = binding.fengine(s, scale=scale)
     for _ in range(W):
-        binding.fengine(s, out)
+        binding.fengine(s, out, scale=scale)
     torch.cuda.synchronize()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
     for a, b in ev:
-        a.record(); binding.fengine(s, out); b.record()
+        a.record(); binding.fengine(s, out, scale=scale); b.record()
     torch.cuda.synchronize()
     ms = sum(a.elapsed_time(b) for a, b in ev) / K
-    nbytes = s.numel() + out.numel() * 2
+    nbytes = s.numel() + out.numel() * out.element_size()
     gbs = nbytes / (ms * 1e-3) / 1e9
     return {"metric": "fengine_gbs", "value": gbs, "unit": "GB/s", "n_gpus": 1, "steps": K, "warmup": W,
             "ms_per_step": ms, "higher_is_better": True, "dtype": "f16 x f16 -> f32 (twiddles hi + lo)", "data": "synthetic",
-            "config": {"workload": "F-engine: %d streams x %d spectra of 256 real int8 samples (sigma 20) -> 128 complex fp16 "
-                                   "channels in the X-engine layout" % (M, A),
+            "config": {"workload": "F-engine: %d streams x %d spectra of 256 real int8 samples (sigma 20) -> 128 complex %s "
+                                   "channels in the X-engine layout" % (M, A, "int8 (requantised, scale 1/20)" if ci8 else "fp16"),
                        "l2": "input + output (%.0f MiB) larger than L2" % (nbytes / 2 ** 20),
                        "gsamples_per_s": s.numel() / (ms * 1e-3) / 1e9},
             "gpu_launches": K,
             "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s", "frac": gbs / pk["hbm"],
-                         "traffic": 3.169e9 if (M, A) == (512, 8192) else None,
+                         "traffic": 3.169e9 if (M, A) == (512, 8192) and not ci8 else None,
                          "traffic_source": "profiles/r2b_ncu_final.md (ncu capture of this kernel and geometry; NOT measured by this run)"
-                         if (M, A) == (512, 8192) else None,
-                         "kernel": "fengtc::fengine_tc_kernel" if binding.fengine_uses_tensor_cores(M, out) else "feng::fengine_kernel",
+                         if (M, A) == (512, 8192) and not ci8 else None,
+                         "kernel": ("fengtc::fengine_tc_kernel<%s>" % ("true" if ci8 else "false"))
+                         if binding.fengine_uses_tensor_cores(M, out) else "feng::fengine_kernel",
                          "kernel_ms": ms, "algorithmic_bytes_per_launch": nbytes}}
 
 
@@ -453,7 +455,7 @@ def run_piece(args):
         raise RuntimeError("bench.py needs a CUDA device")
     torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
     K, W = args.steps, max(args.warmup, 3)
-    rec = time_corner_turn(workload(args.workload), peaks(), K, W, args.planes) if args.piece == "corner_turn" else time_fengine(peaks(), K, W)
+    rec = time_corner_turn(workload(args.workload), peaks(), K, W, args.planes) if args.piece == "corner_turn" else time_fengine(peaks(), K, W, ci8=args.piece == "fengine_ci8")
     print(json.dumps(rec), flush=True)
 
 

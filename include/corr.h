@@ -179,7 +179,8 @@ int corr_fengine_uses_tensor_cores(int n_stream, const void* out);
  * (CORR_CI8): out[n_spectra][128][n_stream] (re, im) int8 pairs, code = clip(rint(S * scale), -127, 127) per component
  * (rint = round to nearest, ties to even, applied to the fp32 product; -128 is never produced).  `scale` > 0 is the
  * caller's requantisation gain (e.g. 1 / (sigma_in * 16) * target sigma); `out` needs 2-byte alignment.  Everything
- * else as corr_fengine.
+ * else as corr_fengine, the kernel choice included: a multiple of 64 streams and a 16-byte aligned `out` run on the
+ * tensor cores (the rounding decision is taken on that kernel's fp32 sums), other geometries on the CUDA-core kernel.
  */
 int corr_fengine_ci8(const void* in, void* out, int n_stream, long long n_spectra, float scale, void* stream);
 

@@ -163,7 +163,8 @@ FengTcState* fengine_tc_state() {
     for (int k = 0; k < fengtc::kChan; ++k) tw[(4 * fengtc::kChan + k) * fengtc::kFold] = __float2half_rn((k & 1) ? -1.0f : 1.0f);
     if (cudaMalloc(&st.d_tw, tw.size() * sizeof(__half)) != cudaSuccess) { cudaGetLastError(); return nullptr; }
     if (cudaMemcpy(st.d_tw, tw.data(), tw.size() * sizeof(__half), cudaMemcpyHostToDevice) != cudaSuccess) return nullptr;
-    if (cudaFuncSetAttribute(fengtc::fengine_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, fengtc::kSmemBytes) != cudaSuccess) {
+    if (cudaFuncSetAttribute(fengtc::fengine_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fengtc::kSmemBytes) != cudaSuccess ||
+        cudaFuncSetAttribute(fengtc::fengine_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fengtc::kSmemBytes) != cudaSuccess) {
         cudaGetLastError();
         return nullptr;
     }
@@ -663,12 +664,13 @@ int corr_set_kernel(corr_handle h, int kernel) {
 }
 int corr_last_launch_count(corr_handle h) { return h ? h->last_launches : CORR_EINVAL; }
 
-// tensor-core path: fp16 output, whole tiles of 64 streams, 16-byte aligned output rows
-static bool fengine_tc_applies(const void* out, int n_stream, bool int8_out) {
-    return !int8_out && n_stream % fengtc::kTileStreams == 0 && (reinterpret_cast<uintptr_t>(out) & 15) == 0;
+// tensor-core path (fp16 output and requantised int8 output): whole tiles of 64 streams, 16-byte aligned output rows
+static bool fengine_tc_applies(const void* out, int n_stream) {
+    return n_stream % fengtc::kTileStreams == 0 && (reinterpret_cast<uintptr_t>(out) & 15) == 0;
 }
 
-static int run_fengine_tc(FengTcState* st, const void* in, void* out, int n_stream, long long n_spectra, cudaStream_t stream) {
+static int run_fengine_tc(FengTcState* st, const void* in, void* out, int n_stream, long long n_spectra, bool int8_out, float scale,
+                          cudaStream_t stream) {
     CUtensorMap map_raw;       // in viewed as [n_stream][n_spectra][256] bytes, box = 64 streams x 1 spectrum x 128 samples
     cuuint64_t dims[3] = {fengtc::kFft, static_cast<cuuint64_t>(n_spectra), static_cast<cuuint64_t>(n_stream)};
     cuuint64_t strides[2] = {fengtc::kFft, static_cast<cuuint64_t>(n_spectra) * fengtc::kFft};
@@ -680,13 +682,15 @@ static int run_fengine_tc(FengTcState* st, const void* in, void* out, int n_stre
     if (r != CUDA_SUCCESS) return fail(nullptr, CORR_ECUDA, "corr_fengine: cuTensorMapEncodeTiled failed with CUresult %d", static_cast<int>(r));
     fengtc::Params prm;
     prm.out = out;
+    prm.scale = scale;
     prm.tw = static_cast<const uint4*>(st->d_tw);
     prm.n_stream = n_stream;
     prm.n_spectra = n_spectra;
     prm.n_half = n_spectra * (n_stream / fengtc::kTileStreams);
     prm.n_tiles = (prm.n_half + 1) / 2;
     const long long grid = prm.n_tiles < st->sm_count ? prm.n_tiles : st->sm_count;
-    fengtc::fengine_tc_kernel<<<static_cast<unsigned>(grid), fengtc::kThreads, fengtc::kSmemBytes, stream>>>(map_raw, prm);
+    if (int8_out) fengtc::fengine_tc_kernel<true><<<static_cast<unsigned>(grid), fengtc::kThreads, fengtc::kSmemBytes, stream>>>(map_raw, prm);
+    else fengtc::fengine_tc_kernel<false><<<static_cast<unsigned>(grid), fengtc::kThreads, fengtc::kSmemBytes, stream>>>(map_raw, prm);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail_cuda(nullptr, e, "fengine_tc_kernel launch");
     return CORR_OK;
@@ -699,9 +703,9 @@ static int run_fengine(const void* in, void* out, int n_stream, long long n_spec
         return fail(nullptr, CORR_EINVAL, "corr_fengine: invalid arguments (n_stream=%d, n_spectra=%lld)", n_stream, n_spectra);
     if ((reinterpret_cast<uintptr_t>(in) & 15) || (reinterpret_cast<uintptr_t>(out) & (int8_out ? 1 : 3)))
         return fail(nullptr, CORR_EINVAL, "corr_fengine: `in` must be 16-byte and `out` element aligned");
-    if (allow_tc && fengine_tc_applies(out, n_stream, int8_out)) {
+    if (allow_tc && fengine_tc_applies(out, n_stream)) {
         FengTcState* st = fengine_tc_state();
-        if (st) return run_fengine_tc(st, in, out, n_stream, n_spectra, static_cast<cudaStream_t>(stream));
+        if (st) return run_fengine_tc(st, in, out, n_stream, n_spectra, int8_out, scale, static_cast<cudaStream_t>(stream));
     }
     feng::Params prm;
     prm.in = static_cast<const int8_t*>(in);
@@ -733,7 +737,7 @@ int corr_fengine_simt(const void* in, void* out, int n_stream, long long n_spect
 }
 
 int corr_fengine_uses_tensor_cores(int n_stream, const void* out) {
-    return fengine_tc_applies(out, n_stream, false) ? 1 : 0;
+    return fengine_tc_applies(out, n_stream) ? 1 : 0;
 }
 
 int corr_corner_turn(corr_handle h, const void* in, void* ws, void* stream) {

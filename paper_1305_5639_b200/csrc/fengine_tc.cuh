@@ -31,9 +31,12 @@
 //               integer-to-float conversion instruction) -> tcgen05.st into the A buffer (double buffered);
 //               thread = one stream row, two warps per TMEM lane quarter split the sample groups
 //   warps 10-17 epilogue: two warps per lane quarter, 64 channels each: Re -> packed halves in registers, then Im ->
-//               (re, im) half2 words -> one coalesced 128-byte store per channel and warp
+//               (re, im) half2 words -> one coalesced 128-byte store per channel and warp.  kInt8 (corr_fengine_ci8):
+//               requantised (re, im) int8 codes instead; the two warps of a half tile trade halves through an exchange
+//               buffer so that the stores are still full 128-byte lines (4-deep raw ring, the fifth slot is the buffers)
 #pragma once
 #include <cuda_fp16.h>
+#include <type_traits>
 #include "ptx.cuh"
 
 namespace fengtc {
@@ -45,7 +48,12 @@ constexpr int kTileStreams = 64;              // streams of one half tile (n_str
 constexpr int kFoldWarps = 8, kEpiWarps = 8;
 constexpr int kThreads = 64 + 32 * (kFoldWarps + kEpiWarps);
 constexpr int kRawBytes = kTileStreams * kFft;               // one half tile: 16 KB (two boxes of 64 rows x 128 B)
-constexpr int kRawRing = 5;                                  // half tiles in flight per CTA
+constexpr int kRawRing = 5;                                  // half tiles in flight per CTA (fp16 output)
+// int8 output: 4 half tiles, the fifth slot is the epilogue's exchange buffer: a warp's 32 streams are only 64 bytes of an
+// int8 output row, and the write path is bound by the number of line requests, not by bytes (measured: 64-byte stores
+// took as long as the fp16 kernel's 128-byte stores), so the two warps of a half tile assemble full 128-byte lines
+constexpr int kRawRingI8 = 4;
+constexpr int kXchgBytes = 32 * 128;                         // per warp pair: 32 channels x 64 streams x (re, im) int8
 constexpr int kMatBytes = kChan * kFold * 2;                 // one fp16 twiddle matrix: 32 KB (two K chunks of 16 KB)
 constexpr int kNumMats = 5;                                  // cos_hi, cos_lo, -sin_hi, -sin_lo, Nyquist sign (first K chunk only)
 // tensor memory map (columns): Re accumulator, Im accumulator, two A buffers {e: 64 columns, o: 64 columns}
@@ -59,7 +67,8 @@ constexpr int kSmemBytes = kOffBar + 256 + 1024 /*alignment slack*/;
 static_assert(kSmemBytes <= 227 * 1024, "shared memory");
 
 struct Params {
-    void* out;               // [n_spectra][128][n_stream] __half2 (re, im)
+    void* out;               // [n_spectra][128][n_stream] __half2 (re, im); kInt8: char2 codes clip(rint(S * scale), +-127)
+    float scale;             // kInt8 only
     const uint4* tw;         // DEVICE: twiddles [cos_hi | cos_lo | -sin_hi | -sin_lo | nyquist][128 channels][128 samples] fp16
     int n_stream;            // multiple of 64
     long long n_spectra;
@@ -110,17 +119,39 @@ __device__ __forceinline__ uint32_t pack_half2(float lo, float hi) {
 __device__ __forceinline__ void stg_stream(uint32_t* p, uint32_t v, uint64_t policy) {
     asm volatile("st.global.L1::no_allocate.L2::cache_hint.b32 [%0], %1, %2;" ::"l"(p), "r"(v), "l"(policy) : "memory");
 }
+// two accumulator values -> one packed pair: fp16 output: half2 word; int8 output (corr_fengine_ci8): the codes
+// clip(rint(v * scale), -127, 127) (rint: ties to even; -128 is never produced) in bytes 0 and 1
+template <bool kInt8> __device__ __forceinline__ uint32_t pack_pair(float lo, float hi, float scale) {
+    if constexpr (kInt8) {
+        // No float-to-int instruction (a quarter-rate pipe: 128 of them per thread and tile made this epilogue the slowest
+        // stage of the kernel): clamp the fp32 product, then add 1.5 * 2^23 -- the add rounds to nearest even at unit
+        // spacing and leaves the two's-complement code in the low byte.  Same result as clip(rint(v * scale), +-127).
+        const float a = fminf(fmaxf(lo * scale, -127.0f), 127.0f) + 12582912.0f;
+        const float b = fminf(fmaxf(hi * scale, -127.0f), 127.0f) + 12582912.0f;
+        return __byte_perm(__float_as_uint(a), __float_as_uint(b), 0x0040);     // bytes 0, 1: the two codes
+    } else {
+        return pack_half2(lo, hi);
+    }
+}
+__device__ __forceinline__ void sts_u16(uint32_t addr, uint32_t v) {
+    asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"(static_cast<uint16_t>(v)) : "memory");
+}
+// named barrier of one warp pair (64 threads); ids 1 .. 4
+__device__ __forceinline__ void pair_sync(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
 // a half tile in the raw ring (two SWIZZLE_128B boxes of [64 rows][128 bytes]): 16-byte unit u of row r of box b
 __device__ __forceinline__ uint32_t raw_unit(uint32_t slot_base, int b, int r, int u) {
     return slot_base + b * (kRawBytes / 2) + r * 128 + ((u ^ (r & 7)) << 4);
 }
 
+template <bool kInt8>
 __global__ void __launch_bounds__(kThreads, 1)
 fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t bar = base + kOffBar;
     // barriers: raw_full[5], raw_empty[5], a_full[2], a_empty[2], re_full, re_empty, im_full, im_empty, then the TMEM base word
+    constexpr int kRing = kInt8 ? kRawRingI8 : kRawRing;
+    static_assert(!kInt8 || 4 * kXchgBytes <= (kRawRing - kRawRingI8) * kRawBytes, "exchange buffers");
     const uint32_t raw_full0 = bar, raw_empty0 = raw_full0 + 8 * kRawRing, a_full0 = raw_empty0 + 8 * kRawRing, a_empty0 = a_full0 + 16;
     const uint32_t re_full = a_empty0 + 16, re_empty = re_full + 8, im_full = re_empty + 8, im_empty = im_full + 8;
     const uint32_t tmem_slot = im_empty + 8;
@@ -132,7 +163,7 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
 
     if (threadIdx.x == 0) {
         ptx::prefetch_tensormap(&tmap_raw);
-        for (int k = 0; k < kRawRing; ++k) {
+        for (int k = 0; k < kRing; ++k) {
             ptx::mbar_init(raw_full0 + 8 * k, 1);
             ptx::mbar_init(raw_empty0 + 8 * k, kFoldWarps / 2);   // the four fold warps of the half tile's two lane quarters
         }
@@ -178,8 +209,8 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
                 if (hidx >= prm.n_half) continue;            // odd number of half tiles: the last tile has one
                 const long long a = hidx / n_sb;
                 const int m0 = static_cast<int>(hidx - a * n_sb) * kTileStreams;
-                const int slot = static_cast<int>(pos % kRawRing);
-                const uint32_t phase = static_cast<uint32_t>(pos / kRawRing) & 1u;
+                const int slot = static_cast<int>(pos % kRing);
+                const uint32_t phase = static_cast<uint32_t>(pos / kRing) & 1u;
                 ptx::mbar_wait_uniform(raw_empty0 + 8 * slot, phase ^ 1u);
                 if (ptx::elect_one()) {
                     ptx::mbar_arrive_expect_tx(raw_full0 + 8 * slot, kRawBytes);
@@ -244,7 +275,7 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
             const uint32_t buf = it & 1u;
             const bool valid = 2 * t + h < prm.n_half;
             const long long pos = 2 * static_cast<long long>(it) + h;
-            const int slot = static_cast<int>(pos % kRawRing);
+            const int slot = static_cast<int>(pos % kRing);
             // ORDER MATTERS.  The A buffer first: once the MMAs of tile it - 2 have been committed, every fold warp has finished
             // tile it - 2, so every load up to that tile has landed.  Only then is the parity wait on the raw slot sound: the
             // ring is 5 deep and a tile takes 2 slots, so the previous user of this slot is the OTHER half's warps (tile it - 2
@@ -253,7 +284,7 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
             // samples, an extra arrival on raw_empty, and eventually a corrupted barrier (seen as 1 failed launch in 15).
             ptx::mbar_wait(a_empty0 + 8 * buf, ((it >> 1) & 1u) ^ 1u);   // the MMAs of two tiles ago have read this A buffer
             ptx::tc_fence_after();
-            if (valid) ptx::mbar_wait(raw_full0 + 8 * slot, static_cast<uint32_t>(pos / kRawRing) & 1u);
+            if (valid) ptx::mbar_wait(raw_full0 + 8 * slot, static_cast<uint32_t>(pos / kRing) & 1u);
             if (valid) {
                 const uint32_t raw = base + kOffRaw + slot * kRawBytes;
                 const uint32_t a_tmem = lane_addr + kTmemA + buf * kTmemABuf;
@@ -303,16 +334,20 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
         const int h = quarter >> 1;
         const int r = (quarter & 1) * 32 + lane;
         const uint32_t lane_addr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16);
-        uint32_t* out = static_cast<uint32_t*>(prm.out);
+        using OutT = typename std::conditional<kInt8, uint16_t, uint32_t>::type;     // one (re, im) pair of one stream
+        OutT* out = static_cast<OutT*>(prm.out);
         const uint64_t policy = ptx::policy_evict_first();
+        const int pair_id = 2 * h + chalf;                   // the two warps (quarters 2h, 2h + 1) of a half tile and channel half
+        const uint32_t xchg = base + kOffRaw + kRawRingI8 * kRawBytes + pair_id * kXchgBytes;     // (kInt8 only)
         uint32_t it = 0;
         for (long long t = first; t < prm.n_tiles; t += step, ++it) {
             const long long hidx = 2 * t + h;
             const bool valid = hidx < prm.n_half;
             const long long a = hidx / n_sb;
             const int m0 = static_cast<int>(hidx - a * n_sb) * kTileStreams;
-            uint32_t* dst = out + (a * kChan + 64 * chalf) * prm.n_stream + m0 + r;     // channel 64 chalf of this stream
-            uint32_t rr[32];                                 // Re of this thread's 64 channels as packed halves
+            OutT* dst = out + (a * kChan + 64 * chalf) * prm.n_stream + m0 + r;         // channel 64 chalf of this stream
+            OutT* dst_line = out + (a * kChan + 64 * chalf) * prm.n_stream + m0;        // ... of the half tile's first stream
+            uint32_t rr[32];                                 // Re of this thread's 64 channels as packed pairs
             ptx::mbar_wait(re_full, it & 1u);
             ptx::tc_fence_after();
 #pragma unroll
@@ -326,7 +361,8 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
                     if (lane == 0) ptx::mbar_arrive(re_empty);
                 }
 #pragma unroll
-                for (int c = 0; c < 16; ++c) rr[16 * part + c] = pack_half2(__uint_as_float(v[2 * c]), __uint_as_float(v[2 * c + 1]));
+                for (int c = 0; c < 16; ++c)
+                    rr[16 * part + c] = pack_pair<kInt8>(__uint_as_float(v[2 * c]), __uint_as_float(v[2 * c + 1]), prm.scale);
             }
             ptx::mbar_wait(im_full, it & 1u);
             ptx::tc_fence_after();
@@ -341,13 +377,36 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
                     if (lane == 0) ptx::mbar_arrive(im_empty);
                 }
                 if (valid) {
+                    if constexpr (kInt8) {
+                        // this warp's 32 channels x 32 streams of codes into the pair's exchange buffer [channel][64 streams x 2 B]
 #pragma unroll
-                    for (int c = 0; c < 16; ++c) {
-                        const uint32_t ii = pack_half2(__uint_as_float(v[2 * c]), __uint_as_float(v[2 * c + 1]));
-                        const uint32_t re2 = rr[16 * part + c];
-                        // (re, im) half2 words of channels 2c and 2c + 1: one 128-byte line per channel and warp
-                        stg_stream(dst + static_cast<long long>(32 * part + 2 * c) * prm.n_stream, __byte_perm(re2, ii, 0x5410), policy);
-                        stg_stream(dst + static_cast<long long>(32 * part + 2 * c + 1) * prm.n_stream, __byte_perm(re2, ii, 0x7632), policy);
+                        for (int c = 0; c < 16; ++c) {
+                            const uint32_t ii = pack_pair<kInt8>(__uint_as_float(v[2 * c]), __uint_as_float(v[2 * c + 1]), prm.scale);
+                            const uint32_t re2 = rr[16 * part + c];
+                            sts_u16(xchg + (2 * c) * 128 + (quarter & 1) * 64 + lane * 2, __byte_perm(re2, ii, 0x0040));
+                            sts_u16(xchg + (2 * c + 1) * 128 + (quarter & 1) * 64 + lane * 2, __byte_perm(re2, ii, 0x0051));
+                        }
+                        pair_sync(1 + pair_id);              // both halves of the 32 rows are in the buffer
+                        // each warp ships 16 of the 32 rows as full 128-byte lines (lane = streams 2 lane, 2 lane + 1)
+#pragma unroll
+                        for (int k = 0; k < 16; ++k) {
+                            const int ch = (quarter & 1) * 16 + k;
+                            const uint32_t word = lds_u32(xchg + ch * 128 + lane * 4);
+                            stg_stream(reinterpret_cast<uint32_t*>(dst_line + static_cast<long long>(32 * part + ch) * prm.n_stream) + lane, word, policy);
+                        }
+                        pair_sync(1 + pair_id);              // the buffer may be overwritten
+                    } else {
+#pragma unroll
+                        for (int c = 0; c < 16; ++c) {
+                            const uint32_t ii = pack_pair<kInt8>(__uint_as_float(v[2 * c]), __uint_as_float(v[2 * c + 1]), prm.scale);
+                            const uint32_t re2 = rr[16 * part + c];
+                            OutT* d0 = dst + static_cast<long long>(32 * part + 2 * c) * prm.n_stream;
+                            // (re, im) half2 words of channels 2c and 2c + 1: one 128-byte line per channel and warp
+                            // (lane pairs trading words for 8-byte stores of two lines per instruction: no gain, the
+                            // write path is bound by lines, not by instructions)
+                            stg_stream(d0, __byte_perm(re2, ii, 0x5410), policy);
+                            stg_stream(d0 + prm.n_stream, __byte_perm(re2, ii, 0x7632), policy);
+                        }
                     }
                 }
             }

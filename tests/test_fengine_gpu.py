@@ -137,7 +137,9 @@ def test_fengine_argument_errors(corr):
 # ---- requantised int8 output (corr_fengine_ci8): the code is decided by rint of an fp32 product on the GPU and of an
 # fp64 product in the oracle, so the two must agree EXACTLY except where the scaled value lies within the fp32 round-off
 # bound of a rounding tie, and there they may differ by one code (quantised decisions) ----
-@pytest.mark.parametrize("M,A,scale", [(2, 3, 1.0 / 64), (33, 4, 1.0 / 40), (64, 8, 0.05), (100, 5, 1.0 / 300)])
+# (stream counts that are a multiple of 64 run on the tensor-core kernel, the others on the CUDA-core kernel)
+@pytest.mark.parametrize("M,A,scale", [(2, 3, 1.0 / 64), (33, 4, 1.0 / 40), (64, 8, 0.05), (100, 5, 1.0 / 300),
+                                       (128, 33, 1.0 / 40), (192, 7, 1.0 / 25), (512, 40, 1.0 / 64)])
 def test_fengine_ci8_codes(corr, M, A, scale):
     from oracle import fengine as fo
     rng = np.random.default_rng(9100 + M)
