@@ -730,7 +730,8 @@ def run_native(args):
                 others.append(short_run(name, pk, sha=not args.no_sha))
             except Exception as e:                                    # a failed side run must not lose the headline
                 others.append({"workload": name, "error": repr(e)})
-        for fn in (lambda: dumps_run(pk), lambda: time_corner_turn(workload("cfg4"), pk, 10, 3), lambda: time_fengine(pk, 10, 3)):
+        for fn in (lambda: dumps_run(pk), lambda: time_corner_turn(workload("cfg4"), pk, 10, 3), lambda: time_fengine(pk, 10, 3),
+                   lambda: time_fengine(pk, 10, 3, ci8=True)):
             try:
                 others.append(fn())
             except Exception as e:
