@@ -566,3 +566,30 @@ def test_dumps_argument_errors(corr):
         assert L.corr_xengine_dumps(h._h, None, out.data_ptr(), 4, None) == corr.CORR_EINVAL
         assert L.corr_xengine_dumps(g._h, x.data_ptr(), out.data_ptr(), 4, None) == corr.CORR_EINVAL     # cross plan
         assert L.corr_xengine_dumps(None, x.data_ptr(), out.data_ptr(), 4, None) == corr.CORR_EINVAL
+
+
+@pytest.mark.parametrize("kernel,N,P,C,T", [("single", 16, 2, 64, 256), ("pair", 136, 2, 21, 260)])
+def test_cuda_graph_capture_of_an_accumulate_sequence(corr, oracle, kernel, N, P, C, T):
+    """corr.h: a sequence of corr_xengine calls (store, accumulate, accumulate) captured with stream capture and replayed
+    reproduces the oracle's integration bit for bit on every replay (the tile-feed counter memset is part of the graph)."""
+    xs = [inputs.gauss_ci8(T, C, N, P, 30.0, seed=9900 + k).cuda() for k in range(3)]
+    want = None
+    for x in xs:
+        want = oracle.xengine(x.cpu().numpy(), accumulate_into=want)
+    with corr.Correlator(N, P, C, T, "ci8") as h:
+        h.set_kernel(kernel)
+        out = h.empty_output()
+        for k, x in enumerate(xs):                                   # once outside the capture
+            h.xengine(x, out, accumulate=k > 0)
+        torch.cuda.synchronize()
+        s = torch.cuda.Stream()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(s):
+            with torch.cuda.graph(g, stream=s):
+                for k, x in enumerate(xs):
+                    h.xengine(x, out, accumulate=k > 0, stream=s)
+        for rep in range(3):
+            out.fill_(-7)                                            # every replay starts from garbage and must overwrite it
+            g.replay()
+            torch.cuda.synchronize()
+            assert (out.cpu().numpy().astype(np.int64) == want).all()
