@@ -441,9 +441,9 @@ def time_fengine(pk, K, W, M=512, A=8192, ci8=False):
                        "gsamples_per_s": s.numel() / (ms * 1e-3) / 1e9},
             "gpu_launches": K,
             "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s", "frac": gbs / pk["hbm"],
-                         "traffic": 3.169e9 if (M, A) == (512, 8192) and not ci8 else None,
+                         "traffic": (2.094e9 if ci8 else 3.163e9) if (M, A) == (512, 8192) else None,
                          "traffic_source": "profiles/r2b_ncu_final.md (ncu capture of this kernel and geometry; NOT measured by this run)"
-                         if (M, A) == (512, 8192) and not ci8 else None,
+                         if (M, A) == (512, 8192) else None,
                          "kernel": ("fengtc::fengine_tc_kernel<%s>" % ("true" if ci8 else "false"))
                          if binding.fengine_uses_tensor_cores(M, out) else "feng::fengine_kernel",
                          "kernel_ms": ms, "algorithmic_bytes_per_launch": nbytes}}
