@@ -189,6 +189,58 @@ int corr_fengine_uses_tensor_cores(int n_stream, const void* out);
  */
 int corr_fengine_ci8(const void* in, void* out, int n_stream, long long n_spectra, float scale, void* stream);
 
+/*
+ * corr_xengine_static -- corr_xengine for callers that are not allowed to allocate device memory.
+ *
+ * Who needs it.  corr_create calls cudaMalloc (tile tables, the tile-feed counters), and corr_fengine / corr_xengine_host
+ * allocate on first use.  Some users of a correlator library cannot make such a call at the point where they need a
+ * result: a real-time capture process that has handed all of the GPU's memory to its own ring buffers at start-up and
+ * must never see an allocation fail (or stall: cudaMalloc and cudaFree synchronise the whole device, which drops
+ * samples on every other stream); a plug-in running inside a host application whose memory policy forbids driver
+ * allocations after initialisation; a tool that attaches to a GPU which another tenant has already filled.  For them
+ * this ONE entry point computes exactly what corr_create + corr_xengine compute (Eq. 2; lower
+ * triangle with autocorrelations) and calls no cudaMalloc, cudaFree or other allocating CUDA routine, and
+ * no malloc / new of its own, on any call.  There is no handle: the geometry is passed with every call.
+ *
+ * How.  It runs the CTA-pair tcgen05 kernel (CORR_KERNEL_PAIR).  The two things that kernel keeps in global memory
+ * besides `in` and `out` -- the per-channel tile table and the 4-byte tile-feed counter -- live in a fixed array
+ * compiled into the library, corr_static_scratch_bytes() = 16896 bytes.  Every GPU on which the process uses
+ * libcorr.so holds that array from the moment the library's code is loaded onto it until the process exits, whether or
+ * not this function is ever called.  The caller still owns and passes `in` and `out`.
+ *
+ *   n_station, n_pol, n_chan, n_time, dtype   as corr_create, with two limits of this entry point:
+ *              n_station * n_pol <= CORR_STATIC_MAX_STREAMS (8192): the built-in tile table has room for the
+ *              2080 tiles per channel of that size and no more; a larger problem is rejected with CORR_EINVAL and a
+ *              message that names the limit (use corr_create / corr_xengine for it).
+ *              n_station * n_pol * sample bytes must be a multiple of 16 (TMA addressing), else CORR_EUNSUPPORTED:
+ *              the CUDA-core fallback of corr_xengine is not offered here.
+ *   in, out, accumulate, stream               exactly as corr_xengine (DEVICE pointers, 16-byte aligned, same layouts
+ *              and sizes: T*C*N*P*(2 or 4) bytes in, C*B*P*P*8 bytes out; asynchronous on `stream`).
+ * Returns CORR_OK or a negative code; the message is corr_last_error(NULL).  All argument checks come before the
+ * first CUDA call, so a rejected call touches no device.
+ *
+ * First call on a device.  The first successful call with a given device current does a one-time, host-side set-up
+ * for that device (it looks up the array's device address, raises the kernel's shared-memory limit, queries how many
+ * CTA pairs fit); it allocates nothing either, but it talks to the driver, so make that first call during start-up,
+ * and before any stream capture is begun on that device.  Later calls only encode one tensor map on the host and
+ * enqueue two kernels on `stream` (a small one that prepares the array, then the X-engine).
+ *
+ * Shared state -- read this.  Every call on a device uses the SAME array, and the array keeps what the last call left
+ * in it; each call therefore re-initialises it (counter cleared, tile table rewritten) on its own stream before its
+ * kernel starts.  Consequences: calls issued on ONE stream are safe back to back, with any mix of geometries; two
+ * calls that can be in flight on the GPU at the same time (different streams without an event between them, or
+ * several host threads of one process each calling it) race on the array and produce wrong visibilities without
+ * any error.  Order them with events or use handles (each corr_create handle has its own scratch).  The host side is
+ * thread-safe.
+ *
+ * CORR_CI8 overflow: a single call with n_time > 65535 returns CORR_EOVERFLOW; with accumulate != 0 there is no handle
+ * to count the samples integrated so far, so keeping the running total within 65535 samples is the caller's job.
+ */
+#define CORR_STATIC_MAX_STREAMS 8192
+int corr_xengine_static(int n_station, int n_pol, int n_chan, int n_time, int dtype, const void* in, void* out,
+                        int accumulate, void* stream);
+size_t corr_static_scratch_bytes(void);      /* size of the built-in scratch array, per GPU (16896) */
+
 /* corr_destroy -- frees the handle and everything it owns.  NULL is a no-op. */
 void corr_destroy(corr_handle h);
 

@@ -46,6 +46,8 @@ SYMBOLS = {
     "corr_workspace_time": (_i, [_vp]),
     "corr_tile_schedule": (_i, [_i, _i, _i, _i, ctypes.POINTER(_i), _i]),
     "corr_last_launch_count": (_i, [_vp]),
+    "corr_xengine_static": (_i, [_i, _i, _i, _i, _i, _vp, _vp, _i, _vp]),
+    "corr_static_scratch_bytes": (_sz, []),
 }
 
 _lib = None
@@ -134,6 +136,45 @@ def _fengine_ci8(samples, scale, out, stream):
         raise ValueError("out must be a contiguous int8 tensor [n_spectra, 128, n_stream, 2]")
     L = lib()
     rc = L.corr_fengine_ci8(samples.data_ptr(), out.data_ptr(), n_stream, n_spec, scale, _stream_ptr(stream))
+    if rc != CORR_OK:
+        raise CorrError(rc, L.corr_last_error(None).decode())
+    return out
+
+
+STATIC_MAX_STREAMS = 8192       # CORR_STATIC_MAX_STREAMS
+
+
+def xengine_static(x, out=None, accumulate=False, stream=None, dtype=None):
+    """corr_xengine_static: the X-engine for callers that may not allocate device memory.
+
+    Same result as ``Correlator(...).xengine(x, out, accumulate)`` on the pair kernel, but with no handle and no
+    cudaMalloc anywhere in the library: the kernel's tile table and tile-feed counter sit in a 16.5 KB array built into
+    libcorr.so.  It exists for users such as a real-time capture process that gave all GPU memory to its ring buffers at
+    start-up, or a plug-in whose host forbids driver allocations after initialisation.  Limits: ``N * P <= 8192`` and a
+    16-byte multiple per channel row.  All calls on a GPU share that one array, so calls that may overlap on the GPU
+    (different streams with no event between them) corrupt each other; calls on one stream are safe back to back.
+
+    ``x``: CUDA ``[T, C, N, P, 2]`` int8 (ci8) or float16 (cf16).  ``out``: the caller's ``[C, B, P, P, 2]`` int32 /
+    float32 tensor.  (``out=None`` lets torch allocate one for convenience; a caller that really cannot allocate passes
+    its own.)  The first call on a device does a one-time host-side set-up; make it before any stream capture.
+    """
+    import torch
+    if dtype is None:
+        dtype = "ci8" if x.dtype == torch.int8 else "cf16"
+    want_in = torch.int8 if dtype == "ci8" else torch.float16
+    want_out = torch.int32 if dtype == "ci8" else torch.float32
+    if x.dtype != want_in or x.dim() != 5 or x.shape[4] != 2 or not x.is_contiguous() or x.device.type != "cuda":
+        raise ValueError("input must be a contiguous CUDA %s tensor [T, C, N, P, 2]" % want_in)
+    T, C, N, P, _ = (int(v) for v in x.shape)
+    shape = (C, N * (N + 1) // 2, P, P, 2)
+    if out is None:
+        if accumulate:
+            raise ValueError("accumulate=True needs the running `out`")
+        out = torch.empty(shape, dtype=want_out, device=x.device)
+    if out.dtype != want_out or tuple(out.shape) != shape or not out.is_contiguous() or out.device.type != "cuda":
+        raise ValueError("output must be a contiguous CUDA %s tensor of shape %s" % (want_out, shape))
+    L = lib()
+    rc = L.corr_xengine_static(N, P, C, T, DTYPES[dtype], x.data_ptr(), out.data_ptr(), int(bool(accumulate)), _stream_ptr(stream))
     if rc != CORR_OK:
         raise CorrError(rc, L.corr_last_error(None).decode())
     return out

@@ -889,3 +889,201 @@ int corr_xengine_host(corr_handle h, const void* in_host, void* out_host, int ac
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// corr_xengine_static: the CTA-pair X-engine for callers that must not allocate device memory (include/corr.h).
+//
+// The pair kernel needs two pieces of global memory besides the caller's input and output: the per-channel tile table
+// it walks and the 4-byte tile-feed counter its clusters claim work from.  A handle gets both from cudaMalloc in
+// corr_create.  Here they live in ONE file-scope device array that is part of the library image, so no call on this path
+// ever asks the driver for memory: every GPU that loads libcorr.so carries these kStaticScratchBytes (16.5 KB) until the
+// process exits, used or not.
+//
+// g_static_scratch is a DEVICE symbol.  In host code its name is only a host-side shadow of the symbol, not a device
+// address: handing `g_static_scratch` itself to a kernel would make the kernel fault (or, on systems where the GPU can
+// reach host memory, quietly work on the wrong memory).  The device address is looked up once per device with
+// cudaGetSymbolAddress (static_state below) and only that pointer is passed to kernels.  Device code in this file
+// (static_prepare_kernel) may name the array directly.
+namespace {
+
+constexpr int kStaticMaxBlocks = CORR_STATIC_MAX_STREAMS * 2 / xtc::kPairRows;            // 64 row blocks of 256 components
+constexpr int kStaticMaxTiles = kStaticMaxBlocks * (kStaticMaxBlocks + 1) / 2;            // 2080 pair tiles per channel
+constexpr int kStaticCounterWords = 64;      // word 0 is the tile-feed counter; the rest pads the table to a 256-byte boundary
+constexpr int kStaticWords = kStaticCounterWords + 2 * kStaticMaxTiles;
+constexpr size_t kStaticScratchBytes = sizeof(unsigned int) * kStaticWords;
+static_assert(sizeof(xtc::PairTile) == 2 * sizeof(unsigned int), "tile table entry");
+
+static __device__ __align__(256) unsigned int g_static_scratch[kStaticWords];
+
+// Prepares the shared scratch for one launch, on the launch's own stream: the array still holds whatever the previous
+// call left there (a counter that has run past its tile count, a table for another station count), so the counter is
+// cleared and the table rewritten every time.  Same order as build_pair_tiles: column-block major, row block >= column block.
+__global__ void static_prepare_kernel(int n_blocks) {
+    if (blockIdx.x == 0 && threadIdx.x == 0) g_static_scratch[0] = 0u;
+    xtc::PairTile* tiles = reinterpret_cast<xtc::PairTile*>(g_static_scratch + kStaticCounterWords);
+    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n_blocks * n_blocks; k += gridDim.x * blockDim.x) {
+        const int cb = k / n_blocks, rb = k - cb * n_blocks;
+        if (rb < cb) continue;
+        const int idx = cb * n_blocks - cb * (cb - 1) / 2 + (rb - cb);
+        tiles[idx] = xtc::PairTile{rb * xtc::kPairRows, cb * xtc::kPairRows};
+    }
+}
+
+struct StaticState {
+    bool ready = false;
+    unsigned int* scratch = nullptr;        // DEVICE address of g_static_scratch on this device
+    EncodeTiledFn encode = nullptr;
+    int sm_count = 0;
+    int max_clusters[2] = {0, 0};           // co-resident CTA pairs of the ci8 / cf16 pair kernel
+};
+std::mutex g_static_mutex;
+StaticState g_static[64];
+
+// One-time set-up for the CURRENT device (looked up again on every call, done once).  Nothing here allocates device
+// memory: it resolves the scratch array's device address, raises the pair kernels' shared-memory limit and asks how many
+// CTA pairs fit on the GPU.  `ready` is set only after everything succeeded, so a transient failure is retried by the next call.
+int static_state(StaticState** out) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(nullptr, CORR_EUNSUPPORTED, "corr_xengine_static: no usable CUDA device (%s)", cudaGetErrorString(e));
+    if (dev < 0 || dev >= 64) return fail(nullptr, CORR_EUNSUPPORTED, "corr_xengine_static: device ordinal %d out of range", dev);
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticState& st = g_static[dev];
+    if (!st.ready) {
+        int major = 0, minor = 0, sms = 0;
+        e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return fail(nullptr, CORR_EUNSUPPORTED, "corr_xengine_static: device query: %s", cudaGetErrorString(e));
+        if (major != 10 || minor != 0)
+            return fail(nullptr, CORR_EUNSUPPORTED, "corr_xengine_static: device %d is sm_%d%d; this library is built for sm_100a only",
+                        dev, major, minor);
+        unsigned int* ptr = nullptr;
+        e = cudaGetSymbolAddress(reinterpret_cast<void**>(&ptr), g_static_scratch);
+        if (e != cudaSuccess || !ptr) {
+            cudaGetLastError();
+            return fail(nullptr, CORR_ECUDA, "corr_xengine_static: cudaGetSymbolAddress(scratch): %s", cudaGetErrorString(e));
+        }
+        EncodeTiledFn enc = get_encode_fn();
+        if (!enc) return fail(nullptr, CORR_ECUDA, "corr_xengine_static: cuTensorMapEncodeTiled entry point unavailable");
+        int clusters[2] = {0, 0};
+        for (int k = 0; k < 2; ++k) {
+            const void* fn_ptr = k == 0 ? (const void*)xtc::xengine_pair_kernel<1> : (const void*)xtc::xengine_pair_kernel<2>;
+            e = cudaFuncSetAttribute(fn_ptr, cudaFuncAttributeMaxDynamicSharedMemorySize, xtc::kPairSmemBytes);
+            if (e != cudaSuccess) {
+                cudaGetLastError();
+                return fail(nullptr, CORR_ECUDA, "corr_xengine_static: cudaFuncSetAttribute(smem): %s", cudaGetErrorString(e));
+            }
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3(static_cast<unsigned>(sms / 2 * 2));
+            cfg.blockDim = dim3(xtc::kNumThreads);
+            cfg.dynamicSmemBytes = xtc::kPairSmemBytes;
+            cudaLaunchAttribute at[1];
+            at[0].id = cudaLaunchAttributeClusterDimension;
+            at[0].val.clusterDim.x = 2;
+            at[0].val.clusterDim.y = 1;
+            at[0].val.clusterDim.z = 1;
+            cfg.attrs = at;
+            cfg.numAttrs = 1;
+            e = cudaOccupancyMaxActiveClusters(&clusters[k], fn_ptr, &cfg);
+            if (e != cudaSuccess || clusters[k] <= 0) {
+                cudaGetLastError();
+                return fail(nullptr, CORR_EUNSUPPORTED, "corr_xengine_static: no co-resident CTA pairs for the pair kernel on device %d", dev);
+            }
+        }
+        st.scratch = ptr;
+        st.encode = enc;
+        st.sm_count = sms;
+        st.max_clusters[0] = clusters[0];
+        st.max_clusters[1] = clusters[1];
+        st.ready = true;
+    }
+    *out = &st;
+    return CORR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t corr_static_scratch_bytes(void) { return kStaticScratchBytes; }
+
+int corr_xengine_static(int n_station, int n_pol, int n_chan, int n_time, int dtype, const void* in, void* out, int accumulate,
+                        void* stream) {
+    g_create_error[0] = 0;
+    // ---- arguments first: nothing below this block is reached (and no CUDA call is made) for a rejected geometry ----
+    if (!valid_geometry(n_station, n_pol, dtype) || n_chan < 1 || n_time < 1)
+        return fail(nullptr, CORR_EINVAL, "corr_xengine_static: invalid geometry N=%d P=%d C=%d T=%d dtype=%d", n_station, n_pol,
+                    n_chan, n_time, dtype);
+    const long long M = static_cast<long long>(n_station) * n_pol;
+    if (M > CORR_STATIC_MAX_STREAMS)
+        return fail(nullptr, CORR_EINVAL,
+                    "corr_xengine_static: n_station * n_pol = %lld exceeds CORR_STATIC_MAX_STREAMS = %d, the largest tile table "
+                    "the library's built-in scratch array holds (%d tiles per channel); use corr_create / corr_xengine",
+                    M, CORR_STATIC_MAX_STREAMS, kStaticMaxTiles);
+    const int sample_bytes = dtype == CORR_CI8 ? 2 : 4;
+    if (static_cast<long long>(n_chan) * 2 * M > (1ll << 31) - 1024 || n_time > (1 << 24))
+        return fail(nullptr, CORR_EINVAL, "corr_xengine_static: geometry too large (C*2*N*P=%lld, T=%d)",
+                    static_cast<long long>(n_chan) * 2 * M, n_time);
+    if ((M * sample_bytes) % 16 != 0)
+        return fail(nullptr, CORR_EUNSUPPORTED,
+                    "corr_xengine_static: per-channel row of %lld B is not a multiple of 16 (TMA cannot address it); use corr_create",
+                    M * sample_bytes);
+    if (dtype == CORR_CI8 && n_time > kMaxIntegrationCi8)
+        return fail(nullptr, CORR_EOVERFLOW, "corr_xengine_static: integrating %d samples would overflow int32 (limit %lld)", n_time,
+                    kMaxIntegrationCi8);
+    if (!in || !out) return fail(nullptr, CORR_EINVAL, "corr_xengine_static: NULL pointer");
+    if ((reinterpret_cast<uintptr_t>(in) & 15) || (reinterpret_cast<uintptr_t>(out) & 15))
+        return fail(nullptr, CORR_EINVAL, "corr_xengine_static: `in` and `out` must be 16-byte aligned");
+    const int n_blocks = static_cast<int>((2 * M + xtc::kPairRows - 1) / xtc::kPairRows);
+    const int tiles_per_chan = n_blocks * (n_blocks + 1) / 2;
+    const long long n_tiles = static_cast<long long>(tiles_per_chan) * n_chan;
+    if (n_blocks > kStaticMaxBlocks || tiles_per_chan > kStaticMaxTiles)        // (implied by the stream limit; kept as the array's own guard)
+        return fail(nullptr, CORR_EINVAL, "corr_xengine_static: %d tiles per channel exceed the scratch array's %d", tiles_per_chan,
+                    kStaticMaxTiles);
+    if (n_tiles > (1ll << 31) - 4096)
+        return fail(nullptr, CORR_EINVAL, "corr_xengine_static: %lld tiles exceed the tile feed's range", n_tiles);
+
+    StaticState* st = nullptr;
+    int rc = static_state(&st);
+    if (rc != CORR_OK) return rc;
+
+    // a plan on the stack, never a heap or device allocation: only the fields fill_params / get_map read
+    corr_plan plan{};
+    plan.N = n_station;
+    plan.P = n_pol;
+    plan.C = plan.C_total = n_chan;
+    plan.T = n_time;
+    plan.dtype = dtype;
+    plan.M = static_cast<int>(M);
+    plan.B = static_cast<long long>(n_station) * (n_station + 1) / 2;
+    plan.sample_bytes = sample_bytes;
+    plan.encode = st->encode;
+    const View v{n_time, n_chan, n_chan, 0, n_chan, 0};
+    const int box_rows = (dtype == CORR_CI8 ? xtc::kPairStageK<1> : xtc::kPairStageK<2>) / xtc::kPairBoxes;
+    const CUtensorMap* map = nullptr;
+    rc = get_map(&plan, in, plan.M, n_chan, n_time, 1, box_rows, &map);        // host-side encode into plan.map_val[]
+    if (rc != CORR_OK) {
+        fail(nullptr, rc, "corr_xengine_static: %s", plan.err);
+        return rc;
+    }
+    xtc::PairParams pp;
+    fill_params(&plan, v, out, accumulate, 1, pp.base);
+    pp.sched_counter = st->scratch;                                                        // DEVICE addresses inside the
+    pp.tiles = reinterpret_cast<const xtc::PairTile*>(st->scratch + kStaticCounterWords);  // static scratch array
+    pp.tiles_per_chan = tiles_per_chan;
+    pp.n_tiles = n_tiles;
+    const int max_clusters = st->max_clusters[dtype == CORR_CI8 ? 0 : 1];
+    const unsigned clusters = static_cast<unsigned>(n_tiles < max_clusters ? n_tiles : max_clusters);
+
+    cudaStream_t cs = static_cast<cudaStream_t>(stream);
+    const int cells = n_blocks * n_blocks;
+    static_prepare_kernel<<<(cells + 255) / 256, 256, 0, cs>>>(n_blocks);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(nullptr, e, "corr_xengine_static: scratch preparation launch");
+    e = dtype == CORR_CI8 ? launch_pair_kernel<1>(*map, *map, pp, clusters, cs) : launch_pair_kernel<2>(*map, *map, pp, clusters, cs);
+    if (e != cudaSuccess) return fail_cuda(nullptr, e, "corr_xengine_static: xengine_pair_kernel launch");
+    return CORR_OK;
+}
+
+}  // extern "C"
