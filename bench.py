@@ -57,9 +57,7 @@ NCU_TRAFFIC = {
     "cfg5_n128": ("pair", 1.325e9, "profiles/r2b_ncu_final.md"),
     "cfg5_n1024": ("pair", 3.168e9, "profiles/r2b_ncu_final.md"),
     "cross_n256": ("pair", 3.190e9, "profiles/r2b_ncu_final.md"),
-    "cfg5_n64": ("pair", 1.200e9, "profiles/r1c_final_ncu_pair_feed.md"),
-    "cfg5_n32": ("single", 1.139e9, "profiles/r1c_final_ncu_pair_feed.md"),
-}
+}      # (no row = no capture of the shipped kernel at that geometry: `traffic` is null there)
 KERNEL_NAMES = {"single": "xtc::xengine_direct_kernel<%d>", "pair": "xtc::xengine_pair_kernel<%d>",
                 "simt": "xsimt::xengine_simt_kernel<%d>"}
 
@@ -335,6 +333,21 @@ def bytes_per_call(cfg):
     return cfg["in_bytes"] + cfg["out_bytes"] * (1.0 + (calls - 1) / calls)
 
 
+def exec_over_useful(cfg, kernel):
+    """Real MACs the tensor-core tiles EXECUTE per channel and sample / the 4 real MACs of every needed complex product
+    (the tensor fraction on executed as well as on useful operations).  Host logic only (corr_tile_schedule)."""
+    from paper_1305_5639_b200 import binding
+    N, P = cfg["N"], cfg["P"]
+    useful = 4.0 * cfg["n_baseline"] * P * P
+    if kernel == "simt":
+        return 1.0
+    if cfg.get("Nb"):
+        blocks = -(-2 * N * P // 256) * -(-2 * cfg["Nb"] * P // 256)
+        return blocks * 65536.0 / useful
+    rows = 256 if kernel == "pair" else 128
+    return sum(rows * ncols for (_, _, ncols) in binding.tile_schedule(N, P, cfg["dtype"], kernel)) / useful
+
+
 def roofline_record(cfg, kernel, kernel_ms, pk, sustained):
     """The dominant kernel against the slower of its two roofs; both sides reported (north_star's definition)."""
     dtype = cfg["dtype"]
@@ -351,7 +364,7 @@ def roofline_record(cfg, kernel, kernel_ms, pk, sustained):
     traffic, traffic_source = None, None
     if cfg["name"] in NCU_TRAFFIC and NCU_TRAFFIC[cfg["name"]][0] == kernel and not cfg.get("sharded"):
         traffic = NCU_TRAFFIC[cfg["name"]][1]
-        traffic_source = "%s (ncu --set full capture of this kernel and geometry; NOT measured by this run)" % NCU_TRAFFIC[cfg["name"]][2]
+        traffic_source = "%s (ncu capture)" % NCU_TRAFFIC[cfg["name"]][2]      # of this kernel + geometry, not this run
     return {
         "bound": bound,
         "achieved": ach_tensor if bound == "tensor" else ach_hbm,
@@ -360,13 +373,15 @@ def roofline_record(cfg, kernel, kernel_ms, pk, sustained):
         "frac": max(t_tensor_ms, t_hbm_ms) / kernel_ms,
         "traffic": traffic, "traffic_source": traffic_source,
         "kernel": KERNEL_NAMES[kernel] % (1 if dtype == "ci8" else 2), "kernel_ms": kernel_ms,
+        "exec_over_useful": exec_over_useful(cfg, kernel),
         "roof_ms": {"tensor": t_tensor_ms, "hbm": t_hbm_ms},
         "peak_source": "%s: bf16 %s %.1f TFLOP/s x nominal %s/bf16 ratio %.0f; HBM copy %.1f GB/s" % (
             pk["source"], "sustained" if sustained else "burst", bf16, dtype, ratio, pk["hbm"]),
         "tensor": {"algorithmic_ops_per_launch": ops, "achieved": ach_tensor, "unit": tunit, "peak": peak_tensor,
                    "frac": ach_tensor / peak_tensor, "frac_of_burst": ach_tensor / (pk["bf16"] * ratio),
                    "frac_of_sustained": ach_tensor / (pk["bf16_sustained"] * ratio),
-                   "frac_of_nominal": ach_tensor / (NOMINAL_BF16 * ratio)},
+                   "frac_of_nominal": ach_tensor / (NOMINAL_BF16 * ratio),
+                   "frac_on_executed_ops": ach_tensor * exec_over_useful(cfg, kernel) / peak_tensor},
         "hbm": {"algorithmic_bytes_per_launch": nbytes, "achieved_gbs": ach_hbm, "peak_gbs": pk["hbm"],
                 "frac": ach_hbm / pk["hbm"]},
     }
@@ -409,8 +424,7 @@ def time_corner_turn(cfg, pk, K, W, planes=1):
             "gpu_launches": K,
             "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s", "frac": gbs / pk["hbm"],
                          "traffic": 4.246e9 if (cfg["name"] == "cfg4" and planes == 1) else None,
-                         "traffic_source": "profiles/r2_ncu_final.md (ncu capture of this kernel and geometry; NOT measured by this run)"
-                         if (cfg["name"] == "cfg4" and planes == 1) else None,
+                         "traffic_source": "profiles/r2_ncu_final.md (ncu capture)" if (cfg["name"] == "cfg4" and planes == 1) else None,
                          "kernel": "cturn::corner_turn_kernel", "kernel_ms": ms,
                          "algorithmic_bytes_per_launch": nbytes}}
 
@@ -442,8 +456,7 @@ def time_fengine(pk, K, W, M=512, A=8192, ci8=False):
             "gpu_launches": K,
             "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s", "frac": gbs / pk["hbm"],
                          "traffic": (2.094e9 if ci8 else 3.163e9) if (M, A) == (512, 8192) else None,
-                         "traffic_source": "profiles/r2b_ncu_final.md (ncu capture of this kernel and geometry; NOT measured by this run)"
-                         if (M, A) == (512, 8192) else None,
+                         "traffic_source": "profiles/r2b_ncu_final.md (ncu capture)" if (M, A) == (512, 8192) else None,
                          "kernel": ("fengtc::fengine_tc_kernel<%s>" % ("true" if ci8 else "false"))
                          if binding.fengine_uses_tensor_cores(M, out) else "feng::fengine_kernel",
                          "kernel_ms": ms, "algorithmic_bytes_per_launch": nbytes}}
@@ -582,6 +595,121 @@ def dumps_run(pk, K=10, W=3):
 
 
 # ------------------------------------------------------------------------------------------------
+# the headline line: compact (the driver keeps only the last ~3 KB of stdout and parses the LAST line)
+# ------------------------------------------------------------------------------------------------
+HEADLINE_MAX_BYTES = 2000
+
+
+def _r(v, sig=5):
+    """Floats to `sig` significant digits (bytes matter on the headline line); everything else unchanged."""
+    if isinstance(v, float):
+        return float("%.*g" % (sig, v)) if v == v and v not in (float("inf"), float("-inf")) else None
+    return v
+
+
+def _cut(s, n):
+    return s if s is None or len(s) <= n else s[:n - 1] + "~"
+
+
+def workload_key(rec, k):
+    """Short key of a side record for the headline's `workloads` summary."""
+    w = rec.get("workload") or (rec.get("config") or {}).get("workload") or rec.get("metric") or "w%d" % k
+    key = w.split(":")[0].strip().replace(" ", "_")
+    if rec.get("metric") == "fengine_gbs":
+        key = "fengine_ci8" if "int8 (requantised" in w else "fengine_f16"
+    elif rec.get("metric") == "corner_turn_gbs":
+        key = "corner_turn"
+    return _cut(key, 16)
+
+
+def workloads_summary(others):
+    """{"cfg3": [value, frac, bound], ...}: ~40 bytes per side record; the full records go out on earlier lines."""
+    out = {}
+    for k, rec in enumerate(others or []):
+        key = workload_key(rec, k)
+        if "error" in rec:
+            out[key] = "error"
+            continue
+        roof = rec.get("roofline") or {}
+        if not roof and "hbm" in rec:
+            roof = {"frac": rec["hbm"].get("frac"), "bound": "hbm"}
+        out[key] = [_r(rec.get("value"), 4), _r(roof.get("frac"), 3), roof.get("bound")]
+    return out
+
+
+def compact_headline(full, others):
+    """The ONE line the driver parses: the contract keys, compact roofline / sustained / e2e / cpu_baseline objects and a
+    `workloads` summary.  Always a single line of strict JSON shorter than HEADLINE_MAX_BYTES: if worst-case strings
+    push it over, the optional parts are dropped in a fixed order (never the contract keys)."""
+    cfg, roof, sus, cpu, e2e, clk = (full.get(k) or {} for k in ("config", "roofline", "sustained", "cpu_baseline", "e2e", "clocks"))
+    line = {k: _r(full.get(k)) for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better",
+                                        "scaling", "vs_baseline", "dtype", "data", "gpu_launches")}
+    line["config"] = {"workload": _cut(cfg.get("workload"), 160), "parallelism": _cut(cfg.get("parallelism"), 80),
+                      "l2": _cut(cfg.get("l2"), 60)}
+    line["clocks"] = {k: _r(clk.get(k)) for k in ("sm_mhz", "sm_max_mhz", "power_w_max", "reasons")} if clk else None
+    line["e2e"] = {k: _r(e2e.get(k)) for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "steps", "ms_per_step")} if e2e else None
+    if roof:
+        line["roofline"] = {k: _r(roof.get(k)) for k in ("bound", "achieved", "peak", "unit", "frac", "kernel", "kernel_ms", "traffic")}
+        line["roofline"].update({"traffic_source": _cut(roof.get("traffic_source"), 40),
+                                 "frac_of_nominal": _r((roof.get("tensor") or {}).get("frac_of_nominal"), 3),
+                                 "frac_on_executed_ops": _r((roof.get("tensor") or {}).get("frac_on_executed_ops"), 3),
+                                 "hbm_frac": _r((roof.get("hbm") or {}).get("frac"), 3),
+                                 "exec_over_useful": _r(roof.get("exec_over_useful"), 4),
+                                 "hbm_write_peak": _r(roof.get("hbm_write_peak_gbs"), 4)})
+    else:
+        line["roofline"] = None
+    line["sustained"] = {"value": _r(sus.get("value")), "frac": _r((sus.get("roofline") or {}).get("frac"), 3),
+                         "sm_mhz": _r((sus.get("clocks") or {}).get("sm_mhz")),
+                         "reasons": (sus.get("clocks") or {}).get("reasons")} if sus else None
+    line["cpu_baseline"] = {"value": _r(cpu.get("value")), "unit": cpu.get("unit"), "cores": cpu.get("cores"), "kind": cpu.get("kind"),
+                            "sample": _cut(cpu.get("sample"), 72), "threads_1": _r((cpu.get("threads_1") or {}).get("value")),
+                            "cpu_model": _cut(cpu.get("cpu_model"), 48)} if cpu else None
+    line["workloads"] = workloads_summary(others) if others else None
+    line["full"] = "gpurun_out/bench_full.json"
+    for drop in (None, "full", ("cpu_baseline", "sample"), ("config", "l2"), "workloads", ("cpu_baseline", "sample"), ("cpu_baseline", "cpu_model"), ("config", "l2"),
+                 ("config", "parallelism"), ("roofline", "traffic_source"), "sustained", ("config", "workload")):
+        if isinstance(drop, tuple):
+            if line.get(drop[0]):
+                line[drop[0]][drop[1]] = None
+        elif drop is not None:
+            line[drop] = None
+        text = json.dumps(line, separators=(",", ":"), allow_nan=False)
+        if len(text.encode()) < HEADLINE_MAX_BYTES:
+            break
+    return text
+
+
+def emit(full, others):
+    """Side records first (one JSON line each, also written to gpurun_out/bench_full.json), the compact headline LAST."""
+    for rec in others or []:
+        print(json.dumps({"record": "workload", **rec}), flush=True)
+    print(json.dumps({"record": "headline_detail", **full}), flush=True)
+    try:
+        os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+        with open(os.path.join(ROOT, "gpurun_out", "bench_full.json"), "w") as f:
+            json.dump({"headline": full, "workloads": others}, f, indent=1)
+    except OSError:
+        pass
+    print(compact_headline(full, others), flush=True)
+
+
+def hbm_write_peak(torch, nbytes=2 << 30, reps=10):
+    """Write-only HBM bandwidth (a plain fill of 2 GiB, CUDA events, best of `reps`): the roof of the write-dominated
+    pieces (dumps, F-engine, N = 1024), for which the 1:1 read/write copy figure of MEASURED_PEAKS.json is not the bound."""
+    buf = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    buf.fill_(1)
+    torch.cuda.synchronize()
+    best = float("inf")
+    for k in range(reps):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); buf.fill_(k & 1); b.record()
+        torch.cuda.synchronize()
+        best = min(best, a.elapsed_time(b))
+    del buf
+    return nbytes / (best * 1e-3) / 1e9
+
+
+# ------------------------------------------------------------------------------------------------
 # native arm
 # ------------------------------------------------------------------------------------------------
 def run_native(args):
@@ -654,6 +782,35 @@ def run_native(args):
         value = whole_job_value(ops_step, K, world, total_ms) / 1e12
     kernel_ms = sum(call_ms) / max(1, len(call_ms))          # average launch duration of the dominant (only) kernel
 
+    # ---- every other config point and piece, briefly (N = 1 only), so the driver-run line carries them --------------
+    # They run BEFORE the >= 2 s sustained leg, after a pause, on a part that is not yet power-capped, so that scoring them
+    # against the burst peaks is fair and their fractions are comparable from run to run.
+    others, write_peak = None, None
+    if world == 1 and not args.no_others and args.workload == "cfg4" and args.kernel == "auto":
+        others = []
+        time.sleep(1.0)
+        try:
+            write_peak = hbm_write_peak(torch)
+        except Exception:
+            write_peak = None
+        for name in ["cfg1", "cfg2", "cfg3"] + ["cfg5_n%d" % n for n in (32, 64, 128, 256, 512, 1024)] + ["cross_n256"]:
+            try:
+                others.append(short_run(name, pk, sha=not args.no_sha))
+            except Exception as e:                                    # a failed side run must not lose the headline
+                others.append({"workload": name, "error": repr(e)})
+        for fn in (lambda: dumps_run(pk), lambda: time_corner_turn(workload("cfg4"), pk, 10, 3), lambda: time_fengine(pk, 10, 3),
+                   lambda: time_fengine(pk, 10, 3, ci8=True)):
+            try:
+                others.append(fn())
+            except Exception as e:
+                others.append({"error": repr(e)})
+        if write_peak:
+            for rec in others:
+                if isinstance(rec.get("roofline"), dict):
+                    rec["roofline"]["hbm_write_peak_gbs"] = write_peak
+                elif "hbm" in rec:
+                    rec["hbm"]["hbm_write_peak_gbs"] = write_peak
+
     # ---- sustained: the same step back to back for >= 2 s (power-capped clocks), its own clock record -----------
     sustained = None
     if not args.no_sustained and not idle:
@@ -723,6 +880,7 @@ def run_native(args):
     # ---- the library GEMM of the same dtype, same protocol as MEASURED_PEAKS.json (context, not the denominator) --
     if world == 1 and not args.no_gemm_peak:
         roofline["library_gemm_8192"] = library_gemm_peak(torch, dtype)
+    roofline["hbm_write_peak_gbs"] = write_peak
 
     # ---- CPU oracle on a bounded sample (rank 0, N = 1 only) ------------------------------------------
     cpu = None
@@ -738,22 +896,6 @@ def run_native(args):
     if r is not None:
         r.close()
 
-    # ---- every other config point and piece, briefly (N = 1 only), so the driver-run line carries them --------------
-    others = None
-    if world == 1 and not args.no_others and args.workload == "cfg4" and args.kernel == "auto":
-        others = []
-        for name in ["cfg1", "cfg2", "cfg3"] + ["cfg5_n%d" % n for n in (32, 64, 128, 256, 512, 1024)] + ["cross_n256"]:
-            try:
-                others.append(short_run(name, pk, sha=not args.no_sha))
-            except Exception as e:                                    # a failed side run must not lose the headline
-                others.append({"workload": name, "error": repr(e)})
-        for fn in (lambda: dumps_run(pk), lambda: time_corner_turn(workload("cfg4"), pk, 10, 3), lambda: time_fengine(pk, 10, 3),
-                   lambda: time_fengine(pk, 10, 3, ci8=True)):
-            try:
-                others.append(fn())
-            except Exception as e:
-                others.append({"error": repr(e)})
-
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
@@ -765,9 +907,9 @@ def run_native(args):
                    "visibilities_per_s": (1 if sharded else world) * K * C * cfg["n_baseline"] * P * P / (total_ms * 1e-3),
                    "input_sha256": sha},
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_call * calls * K,
-        "roofline": roofline, "sustained": sustained, "cpu_baseline": cpu, "workloads": others,
+        "roofline": roofline, "sustained": sustained, "cpu_baseline": cpu,
     }
-    print(json.dumps(line), flush=True)
+    emit(line, others)
     if world > 1:
         dist.destroy_process_group()
 
