@@ -282,9 +282,9 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
             // or it - 3), and TMA loads complete out of order.  Waiting on the slot first, a fast warp could meet the barrier
             // one phase behind (the older load still in flight under DRAM load), which a parity wait reads as "done": stale
             // samples, an extra arrival on raw_empty, and eventually a corrupted barrier (seen as 1 failed launch in 15).
-            ptx::mbar_wait(a_empty0 + 8 * buf, ((it >> 1) & 1u) ^ 1u);   // the MMAs of two tiles ago have read this A buffer
+            ptx::mbar_wait_uniform(a_empty0 + 8 * buf, ((it >> 1) & 1u) ^ 1u);   // the MMAs of two tiles ago have read this A buffer
             ptx::tc_fence_after();
-            if (valid) ptx::mbar_wait(raw_full0 + 8 * slot, static_cast<uint32_t>(pos / kRing) & 1u);
+            if (valid) ptx::mbar_wait_uniform(raw_full0 + 8 * slot, static_cast<uint32_t>(pos / kRing) & 1u);
             if (valid) {
                 const uint32_t raw = base + kOffRaw + slot * kRawBytes;
                 const uint32_t a_tmem = lane_addr + kTmemA + buf * kTmemABuf;
@@ -348,7 +348,7 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
             OutT* dst = out + (a * kChan + 64 * chalf) * prm.n_stream + m0 + r;         // channel 64 chalf of this stream
             OutT* dst_line = out + (a * kChan + 64 * chalf) * prm.n_stream + m0;        // ... of the half tile's first stream
             uint32_t rr[32];                                 // Re of this thread's 64 channels as packed pairs
-            ptx::mbar_wait(re_full, it & 1u);
+            ptx::mbar_wait_uniform(re_full, it & 1u);
             ptx::tc_fence_after();
 #pragma unroll
             for (int part = 0; part < 2; ++part) {
@@ -364,7 +364,7 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
                 for (int c = 0; c < 16; ++c)
                     rr[16 * part + c] = pack_pair<kInt8>(__uint_as_float(v[2 * c]), __uint_as_float(v[2 * c + 1]), prm.scale);
             }
-            ptx::mbar_wait(im_full, it & 1u);
+            ptx::mbar_wait_uniform(im_full, it & 1u);
             ptx::tc_fence_after();
 #pragma unroll
             for (int part = 0; part < 2; ++part) {

@@ -68,6 +68,10 @@ __device__ __forceinline__ bool elect_one() {
 // suspended in it.  Lanes that then leave the loop in different iterations never reconverge, elect.sync elects one leader
 // per fragment and every TMA load / MMA / commit behind it is issued twice (seen as a sporadic launch failure of the
 // F-engine under full DRAM load, 1 launch in 15).
+// Round 3: EVERY whole-warp wait goes through the vote, not only the electing warps: the fold and epilogue warps follow
+// their waits with .sync.aligned tcgen05.st / tcgen05.ld, a __syncwarp() and a lane-0 arrive that hands the buffer back;
+// a warp split at the wait could release the buffer before its other lanes' tcgen05 accesses are done.  Plain mbar_wait
+// is left for single-thread waiters (the tile-feed writer) only.
 __device__ __forceinline__ void mbar_wait_uniform(uint32_t bar, uint32_t parity) {
     if (__all_sync(0xffffffffu, mbar_try_wait(bar, parity))) return;
     const long long t0 = clock64();

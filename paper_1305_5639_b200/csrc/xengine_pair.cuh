@@ -84,9 +84,10 @@ struct TileFeed {
         advance();
         return g;
     }
-    // a whole (converged) warp: every lane reads, lane 0 reports
+    // a whole (converged) warp: every lane reads, lane 0 reports (vote-based wait: the lanes leave the poll together, so the
+    // __syncwarp below and the .sync.aligned tcgen05.ld that follow find the warp converged; see ptx::mbar_wait_uniform)
     __device__ __forceinline__ long long next_warp(int lane) {
-        ptx::mbar_wait_cluster(full0 + 8u * slot, phase);
+        ptx::mbar_wait_cluster_uniform(full0 + 8u * slot, phase);
         const uint32_t g = ptx::ld_shared_u32(slot0 + 4u * slot);
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive_cluster_after(free0_writer + 8u * slot, g);
@@ -314,7 +315,7 @@ xengine_pair_kernel(const __grid_constant__ CUtensorMap tmap_in, const __grid_co
             const int h_end = need < h_begin + kTileCols / 2 ? need : h_begin + kTileCols / 2;
             drain_tile<C::kFloat, true, kPairEpiBufs>(prm, n_kchunks, c_out, u0, td.col0, h_begin, h_end, stage_smem, buf, lane,
                                                       [&](int, uint32_t& taddr, uint32_t& bar) {
-                ptx::mbar_wait(tfull_bar(acc), acc_phase);
+                ptx::mbar_wait_uniform(tfull_bar(acc), acc_phase);
                 ptx::tc_fence_after();
                 taddr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + acc * kTileCols;
                 bar = ptx::mapa(tempty_bar(acc), 0);

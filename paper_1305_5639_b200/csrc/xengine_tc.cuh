@@ -503,7 +503,7 @@ xengine_direct_kernel(const __grid_constant__ CUtensorMap tmap_in, const Params 
             const int h_end = td.ncols < h_begin + kTileCols / 2 ? td.ncols : h_begin + kTileCols / 2;
             drain_tile<C::kFloat, false, 2>(prm, n_kchunks, prm.chan0_out + c, u0, td.col0, h_begin, h_end, stage_smem, buf, lane,
                                             [&](int, uint32_t& taddr, uint32_t& bar) {
-                ptx::mbar_wait(tfull_bar(acc), acc_phase);
+                ptx::mbar_wait_uniform(tfull_bar(acc), acc_phase);
                 ptx::tc_fence_after();
                 taddr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + acc * kTileCols;
                 bar = tempty_bar(acc);
