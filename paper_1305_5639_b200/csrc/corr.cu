@@ -93,6 +93,7 @@ struct corr_plan {
     // corr_xengine_host: device staging (two input windows, the running output) and the copy pipeline
     void* d_in_stage[2];
     void* d_out_stage;
+    bool host_sum_valid;   // d_out_stage holds a complete integration (false after a failed corr_xengine_host call)
     cudaStream_t st_h2d, st_run, st_d2h;
     cudaEvent_t ev_h2d[2], ev_run[2];
 
@@ -123,7 +124,9 @@ EncodeTiledFn get_encode_fn() {
 }
 
 // Tensor-core F-engine (fengine_tc.cuh): per-device twiddle table [cos_hi | cos_lo | -sin_hi | -sin_lo | nyquist], each
-// [128 channels][128 folded samples] fp16 (nyquist: (-1)^k in sample slot 0, zero elsewhere); built on first use.
+// [128 channels][128 folded samples] fp16 (nyquist: (-1)^k in sample slot 0, zero elsewhere); built on first use and kept
+// (160 KB per device) until the process exits: freeing it from a static destructor would call into a CUDA runtime that may
+// already have shut down.
 struct FengTcState {
     bool tried = false, ok = false;
     void* d_tw = nullptr;
@@ -139,12 +142,14 @@ FengTcState* fengine_tc_state() {
     std::lock_guard<std::mutex> lock(g_feng_mutex);
     FengTcState& st = g_feng[dev];
     if (st.tried) return st.ok ? &st : nullptr;
-    st.tried = true;
+    // `tried` is set only on a DEFINITIVE answer (wrong architecture, no tensor-map encoder, or success): a transient
+    // failure of the allocation or the copy below is retried by the next call instead of disabling the kernel for good.
     cudaDeviceProp prop;
-    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess || prop.major != 10 || prop.minor != 0) return nullptr;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    if (prop.major != 10 || prop.minor != 0) { st.tried = true; return nullptr; }
     st.sm_count = prop.multiProcessorCount;
     st.encode = get_encode_fn();
-    if (!st.encode) return nullptr;
+    if (!st.encode) { st.tried = true; return nullptr; }
     // hi = fp16(w), lo = fp16(w - hi): w = hi + lo to ~3e-8 absolute (lo may be subnormal)
     std::vector<__half> tw(fengtc::kNumMats * fengtc::kChan * fengtc::kFold, __float2half_rn(0.0f));
     const double two_pi = 6.283185307179586476925286766559;
@@ -161,14 +166,17 @@ FengTcState* fengine_tc_state() {
             }
         }
     for (int k = 0; k < fengtc::kChan; ++k) tw[(4 * fengtc::kChan + k) * fengtc::kFold] = __float2half_rn((k & 1) ? -1.0f : 1.0f);
-    if (cudaMalloc(&st.d_tw, tw.size() * sizeof(__half)) != cudaSuccess) { cudaGetLastError(); return nullptr; }
-    if (cudaMemcpy(st.d_tw, tw.data(), tw.size() * sizeof(__half), cudaMemcpyHostToDevice) != cudaSuccess) return nullptr;
-    if (cudaFuncSetAttribute(fengtc::fengine_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fengtc::kSmemBytes) != cudaSuccess ||
+    void* d_tw = nullptr;
+    if (cudaMalloc(&d_tw, tw.size() * sizeof(__half)) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    if (cudaMemcpy(d_tw, tw.data(), tw.size() * sizeof(__half), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaFuncSetAttribute(fengtc::fengine_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fengtc::kSmemBytes) != cudaSuccess ||
         cudaFuncSetAttribute(fengtc::fengine_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fengtc::kSmemBytes) != cudaSuccess) {
         cudaGetLastError();
+        cudaFree(d_tw);
         return nullptr;
     }
-    st.ok = true;
+    st.d_tw = d_tw;
+    st.ok = st.tried = true;
     return &st;
 }
 
@@ -537,6 +545,7 @@ static corr_handle create_plan(int n_station, int n_station_b, int n_pol, int n_
     h->Tp = (n_time + 63) / 64 * 64;
     h->d_in_stage[0] = h->d_in_stage[1] = nullptr;
     h->d_out_stage = nullptr;
+    h->host_sum_valid = false;
     h->st_h2d = h->st_run = h->st_d2h = nullptr;
     h->ev_h2d[0] = h->ev_h2d[1] = h->ev_run[0] = h->ev_run[1] = nullptr;
     h->err[0] = 0;
@@ -737,7 +746,8 @@ int corr_fengine_simt(const void* in, void* out, int n_stream, long long n_spect
 }
 
 int corr_fengine_uses_tensor_cores(int n_stream, const void* out) {
-    return fengine_tc_applies(out, n_stream) ? 1 : 0;
+    // the same two conditions run_fengine applies, in the same order: geometry / alignment, then the device's state
+    return fengine_tc_applies(out, n_stream) && fengine_tc_state() != nullptr ? 1 : 0;
 }
 
 int corr_corner_turn(corr_handle h, const void* in, void* ws, void* stream) {
@@ -843,32 +853,45 @@ int corr_xengine_host(corr_handle h, const void* in_host, void* out_host, int ac
             e = cudaMalloc(&h->d_in_stage[k], static_cast<size_t>(h->T) * win_max * chan_in_bytes);
             if (e != cudaSuccess) return fail(h, CORR_ENOMEM, "corr_xengine_host: input staging: %s", cudaGetErrorString(e));
         }
+    if (accumulate && !h->host_sum_valid)
+        return fail(h, CORR_EINVAL, "corr_xengine_host: accumulate without a complete previous integration on this handle "
+                                    "(no earlier call, or the last one failed part-way)");
     if (!h->d_out_stage) {
-        if (accumulate) return fail(h, CORR_EINVAL, "corr_xengine_host: accumulate without a previous call");
         e = cudaMalloc(&h->d_out_stage, static_cast<size_t>(h->C) * chan_out_bytes);
         if (e != cudaSuccess) return fail(h, CORR_ENOMEM, "corr_xengine_host: output staging: %s", cudaGetErrorString(e));
     }
     h->last_launches = 0;
+    h->host_sum_valid = false;            // until every window of this call has gone through
     const uint8_t* src = static_cast<const uint8_t*>(in_host);
     uint8_t* dst = static_cast<uint8_t*>(out_host);
     const int base = h->C / n_win, extra = h->C % n_win;
+    // A failure part-way leaves copies queued that still read `in_host` / write `out_host`, and some windows of the running
+    // sum already updated: drain all three streams before returning (the caller may free its buffers right away) and leave
+    // the running sum marked invalid, so that a retry cannot double-count the windows that did go through.
+    auto bail = [&](int code) {
+        cudaStreamSynchronize(h->st_h2d);
+        cudaStreamSynchronize(h->st_run);
+        cudaStreamSynchronize(h->st_d2h);
+        cudaGetLastError();
+        return code;
+    };
     int c0 = 0;
     for (int w = 0; w < n_win; ++w) {
         const int wn = base + (w < extra ? 1 : 0);
         const int slot = w & 1;
         if (w >= 2) {                                     // the kernel of window w - 2 has finished reading this slot
             e = cudaStreamWaitEvent(h->st_h2d, h->ev_run[slot], 0);
-            if (e != cudaSuccess) return fail_cuda(h, e, "corr_xengine_host: wait for the staging slot");
+            if (e != cudaSuccess) return bail(fail_cuda(h, e, "corr_xengine_host: wait for the staging slot"));
         }
         e = cudaMemcpy2DAsync(h->d_in_stage[slot], wn * chan_in_bytes, src + static_cast<size_t>(h->chan0 + c0) * chan_in_bytes,
                               static_cast<size_t>(h->C_total) * chan_in_bytes, wn * chan_in_bytes, h->T, cudaMemcpyHostToDevice,
                               h->st_h2d);
         if (e == cudaSuccess) e = cudaEventRecord(h->ev_h2d[slot], h->st_h2d);
         if (e == cudaSuccess) e = cudaStreamWaitEvent(h->st_run, h->ev_h2d[slot], 0);
-        if (e != cudaSuccess) return fail_cuda(h, e, "corr_xengine_host: H2D copy");
+        if (e != cudaSuccess) return bail(fail_cuda(h, e, "corr_xengine_host: H2D copy"));
         const View v{h->T, wn, wn, 0, h->C, c0};
         const int rc = launch_xengine(h, v, h->d_in_stage[slot], nullptr, h->d_out_stage, accumulate, h->st_run);
-        if (rc != CORR_OK) return rc;
+        if (rc != CORR_OK) return bail(rc);
         e = cudaEventRecord(h->ev_run[slot], h->st_run);
         if (e == cudaSuccess && dst) {
             e = cudaStreamWaitEvent(h->st_d2h, h->ev_run[slot], 0);
@@ -877,13 +900,14 @@ int corr_xengine_host(corr_handle h, const void* in_host, void* out_host, int ac
                                     static_cast<uint8_t*>(h->d_out_stage) + static_cast<size_t>(c0) * chan_out_bytes,
                                     wn * chan_out_bytes, cudaMemcpyDeviceToHost, h->st_d2h);
         }
-        if (e != cudaSuccess) return fail_cuda(h, e, "corr_xengine_host: D2H copy");
+        if (e != cudaSuccess) return bail(fail_cuda(h, e, "corr_xengine_host: D2H copy"));
         c0 += wn;
     }
     e = cudaStreamSynchronize(h->st_run);
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->st_d2h);
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->st_h2d);
-    if (e != cudaSuccess) return fail_cuda(h, e, "corr_xengine_host: stream synchronize");
+    if (e != cudaSuccess) return bail(fail_cuda(h, e, "corr_xengine_host: stream synchronize"));
+    h->host_sum_valid = true;
     h->t_total = t_next;
     return CORR_OK;
 }

@@ -449,6 +449,22 @@ def test_host_path_pipeline(corr, oracle, N, P, C, T, dtype):
                 assert fp16_normalised_error(oh.numpy(), want, N, P) <= FP16_TOL
 
 
+def test_host_path_accumulate_needs_a_complete_integration(corr):
+    """corr_xengine_host keeps its running sum on the device: accumulate != 0 is refused until a call with
+    accumulate == 0 has gone through on this handle (the same flag is cleared when a call fails part-way)."""
+    x = inputs.gauss_ci8(64, 3, 16, 2, 30.0, seed=7990)
+    with corr.Correlator(16, 2, 3, 64, "ci8") as h:
+        oh = torch.empty(h.output_shape(), dtype=torch.int32)
+        with pytest.raises(corr.CorrError) as ei:
+            h.xengine_host(x, oh, accumulate=True)
+        assert ei.value.code == corr.CORR_EINVAL and "accumulate without" in str(ei.value)
+        h.xengine_host(x, oh)
+        h.xengine_host(x, oh, accumulate=True)
+        first = oh.clone()
+        h.xengine_host(x, oh)
+        assert torch.equal(2 * oh, first)
+
+
 # ---------------------------------------------------------------------------------------------
 # rectangular cross-only X-engine (corr_xengine_cross; PAPER.md:79) against oracle.xengine_cross
 # ---------------------------------------------------------------------------------------------
