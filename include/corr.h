@@ -105,7 +105,11 @@ corr_handle corr_create_window(int n_station, int n_pol, int n_chan_total, int c
  * memset of its tile-feed counter in front), so a sequence of calls can be captured with stream capture and replayed --
  * the way to run launch-bound geometries (config 1: 13 us per call eagerly, 4.8 us replayed).  Call once before
  * capturing (the first call on a handle encodes its tensor map on the host); the overflow accounting above is done at
- * CAPTURE time, replays do not advance it.
+ * CAPTURE time, replays do not advance it.  A captured pair-kernel launch has ONE of the handle's 256 tile-feed counters
+ * (and the memset that clears it) baked into the graph, while later launches on the handle keep walking the ring: once
+ * calls of this handle have been captured, do not run that graph concurrently with other launches of the SAME handle on
+ * another stream (after 256 further launches they would share the counter and tiles would be skipped or done twice).
+ * Replays and eager calls ordered on one stream, or concurrent work on DIFFERENT handles, are fine.
  */
 int corr_xengine(corr_handle h, const void* in, void* out, int accumulate, void* stream);
 
@@ -119,6 +123,9 @@ int corr_xengine(corr_handle h, const void* in, void* out, int accumulate, void*
  * `out_host` receives the updated integration; `out_host` may be NULL to leave the running sum on the device until a
  * later call asks for it.  Returns after all copies have completed.  PINNED host memory is needed for the copies to
  * overlap (pageable memory works but serialises).  CORR_EOVERFLOW as corr_xengine.
+ * On failure: the call returns only after everything it had queued has drained, so `in_host` / `out_host` may be freed
+ * or reused at once; the running sum on the device is then incomplete and is marked invalid -- the next call must start a
+ * new integration (accumulate == 0; accumulate != 0 returns CORR_EINVAL), and the contents of `out_host` are undefined.
  */
 int corr_xengine_host(corr_handle h, const void* in_host, void* out_host, int accumulate);
 
@@ -173,7 +180,9 @@ int corr_xengine_dumps(corr_handle h, const void* in, void* out, int n_dump, voi
  * fp32 accumulation: csrc/fengine_tc.cuh); every other geometry runs on the CUDA-core radix-16 x 16 FFT kernel
  * (csrc/fengine.cuh).  Both meet the same bound against the fp64 definition: 0.5 ulp of the fp16 output plus
  * 2e-6 sum_n |s[n]|.  corr_fengine_simt forces the CUDA-core kernel (cross-check); corr_fengine_uses_tensor_cores tells
- * which one corr_fengine would launch (1 / 0).
+ * which one corr_fengine would launch on the CURRENT device (1 / 0): it applies the same two tests as corr_fengine itself,
+ * the geometry / alignment rule above and the per-device set-up of the tensor-core kernel (0 on a device that is not
+ * sm_100, or where that set-up failed; calling it may perform the set-up, which allocates the 160 KB twiddle table).
  */
 int corr_fengine(const void* in, void* out, int n_stream, long long n_spectra, void* stream);
 int corr_fengine_simt(const void* in, void* out, int n_stream, long long n_spectra, void* stream);
@@ -182,7 +191,9 @@ int corr_fengine_uses_tensor_cores(int n_stream, const void* out);
 /*
  * corr_fengine_ci8 -- the same transform with REQUANTISED complex int8 output, the input format of the int8 X-engine
  * (CORR_CI8): out[n_spectra][128][n_stream] (re, im) int8 pairs, code = clip(rint(S * scale), -127, 127) per component
- * (rint = round to nearest, ties to even, applied to the fp32 product; -128 is never produced).  `scale` > 0 is the
+ * (rint = round to nearest, ties to even; -128 is never produced.  The tensor-core kernel rounds ONCE -- S * scale is
+ * formed and rounded to an integer by a single fused multiply-add on its fp32 sum S -- while the CUDA-core kernel rounds the
+ * fp32 product first and then to an integer; the two can differ by one code only within an fp32 rounding error of a tie).  `scale` > 0 is the
  * caller's requantisation gain (e.g. 1 / (sigma_in * 16) * target sigma); `out` needs 2-byte alignment.  Everything
  * else as corr_fengine, the kernel choice included: a multiple of 64 streams and a 16-byte aligned `out` run on the
  * tensor cores (the rounding decision is taken on that kernel's fp32 sums), other geometries on the CUDA-core kernel.

@@ -124,11 +124,15 @@ __device__ __forceinline__ void stg_stream(uint32_t* p, uint32_t v, uint64_t pol
 template <bool kInt8> __device__ __forceinline__ uint32_t pack_pair(float lo, float hi, float scale) {
     if constexpr (kInt8) {
         // No float-to-int instruction (a quarter-rate pipe: 128 of them per thread and tile made this epilogue the slowest
-        // stage of the kernel): clamp the fp32 product, then add 1.5 * 2^23 -- the add rounds to nearest even at unit
-        // spacing and leaves the two's-complement code in the low byte.  Same result as clip(rint(v * scale), +-127).
-        const float a = fminf(fmaxf(lo * scale, -127.0f), 127.0f) + 12582912.0f;
-        const float b = fminf(fmaxf(hi * scale, -127.0f), 127.0f) + 12582912.0f;
-        return __byte_perm(__float_as_uint(a), __float_as_uint(b), 0x0040);     // bytes 0, 1: the two codes
+        // stage of the kernel).  ONE fused multiply-add forms v * scale + 1.5 * 2^23 with a single rounding, to nearest even
+        // at unit spacing: the float's bit pattern is then 0x4B400000 + rint(v * scale) (two's complement in the mantissa),
+        // exact rint of the UNROUNDED product.  The clip to +-127 is taken on those bits as signed integers, which order like
+        // the floats they encode (anything beyond +-2^22, where the spacing is no longer 1, lands outside the window on the
+        // right side; negative floats are negative integers), and the code is the low byte.
+        constexpr int kMagicBits = 0x4B400000;
+        const int a = min(max(__float_as_int(fmaf(lo, scale, 12582912.0f)), kMagicBits - 127), kMagicBits + 127);
+        const int b = min(max(__float_as_int(fmaf(hi, scale, 12582912.0f)), kMagicBits - 127), kMagicBits + 127);
+        return __byte_perm(static_cast<uint32_t>(a), static_cast<uint32_t>(b), 0x0040);     // bytes 0, 1: the two codes
     } else {
         return pack_half2(lo, hi);
     }
