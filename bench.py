@@ -71,12 +71,19 @@ def parse_args():
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
     ap.add_argument("--kernel", default="auto", choices=["auto", "single", "pair", "simt"],
                     help="force a kernel variant (default: the library's own choice)")
-    ap.add_argument("--piece", default="xengine", choices=["xengine", "corner_turn", "fengine", "fengine_ci8"],
+    ap.add_argument("--piece", default="xengine", choices=["xengine", "corner_turn", "fengine", "fengine_ci8", "fx_chain", "fx_chain_f16"],
                     help="corner_turn: time the standalone corner-turn kernel (SURVEY 8(a) a1) on the workload's input; "
                          "fengine: time corr_fengine (SURVEY 8(f) rank 2) on 512 streams x 8192 spectra of 256 real int8 samples")
     ap.add_argument("--shard", default="none", choices=["none", "channels"],
                     help="channels: the N ranks split ONE workload's channels into windows (strong scaling, SURVEY 8(f) rank 3); "
                          "default: N independent replicas (north_star: the path does not shard)")
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"],
+                    help="torch.distributed backend for the barrier / max-over-ranks (gloo: several ranks may share one GPU, "
+                         "LOCAL_RANK is mapped modulo the device count)")
+    ap.add_argument("--channels", type=int, default=0, help="cut the workload to its first CHANNELS channels (sharding tests)")
+    ap.add_argument("--check", action="store_true",
+                    help="--shard channels: gather every rank's slabs on rank 0 (test-only gather; the data path keeps no "
+                         "collective) and compare them word for word with ONE unsharded launch on the same input")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-gemm-peak", action="store_true",
@@ -89,9 +96,11 @@ def parse_args():
     return ap.parse_args()
 
 
-def workload(name):
+def workload(name, channels=0):
     from paper_1305_5639_b200 import inputs
     cfg = dict(inputs.CONFIGS[name])
+    if channels:
+        cfg["C"] = min(cfg["C"], int(channels))
     N, P, C, T = cfg["N"], cfg["P"], cfg["C"], cfg["T"]
     B = N * cfg["Nb"] if cfg.get("Nb") else N * (N + 1) // 2       # rectangle (cross workload) or packed triangle
     cfg["name"] = name
@@ -462,13 +471,69 @@ def time_fengine(pk, K, W, M=512, A=8192, ci8=False):
                          "kernel_ms": ms, "algorithmic_bytes_per_launch": nbytes}}
 
 
+def time_fx_chain(pk, K, W, ci8=True, N=256, P=2, A=8192):
+    """The paper's FX pair as ONE timed unit ("the F-engine and the X-engine"; its only single-GPU figure, ~105
+    GFLOPS on a C2075, is for both together): N*P streams of A*256 real int8 samples -> corr_fengine_ci8
+    (or corr_fengine, fp16) -> corr_xengine on the 128 channels x A spectra it wrote, one CUDA-event interval around both
+    launches.  Ops counted as the paper counts them, necessary operations only: X = 8 per complex MAC over
+    the N(N+1)/2 pairs; F = 2.5 n log2 n per real length-n transform (n = 256: 5120), the usual split-radix convention."""
+    import torch
+    from paper_1305_5639_b200 import binding
+    M = N * P
+    g = torch.Generator(device="cuda"); g.manual_seed(1900)
+    s = torch.clamp(torch.round(torch.randn((M, A * 256), generator=g, device="cuda") * 20.0), -127, 127).to(torch.int8)
+    scale = 1.0 / 20 if ci8 else None
+    dtype = "ci8" if ci8 else "cf16"
+    with binding.Correlator(N, P, 128, A, dtype) as h:
+        spec = binding.fengine(s, scale=scale)                        # [A, 128, M, 2] = the X-engine's [T, C, N, P, 2]
+        x = spec.view(A, 128, N, P, 2)
+        out = h.xengine(x)
+        for _ in range(W):
+            binding.fengine(s, spec, scale=scale); h.xengine(x, out)
+        torch.cuda.synchronize()
+        ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
+        for a, b, c in ev:
+            a.record(); binding.fengine(s, spec, scale=scale); b.record(); h.xengine(x, out); c.record()
+        torch.cuda.synchronize()
+        kernel = h.kernel
+    ms = sum(a.elapsed_time(c) for a, _, c in ev) / K
+    ms_f = sum(a.elapsed_time(b) for a, b, _ in ev) / K
+    ms_x = sum(b.elapsed_time(c) for _, b, c in ev) / K
+    ops_x = 8.0 * 128 * A * (N * (N + 1) // 2) * P * P
+    ops_f = 2.5 * 256 * 8 * M * A
+    nbytes = s.numel() + 2 * spec.numel() * spec.element_size() + out.numel() * 4      # F: read + write; X: read + write
+    gbs = nbytes / (ms * 1e-3) / 1e9
+    return {"metric": "fx_chain_tops", "value": (ops_x + ops_f) / (ms * 1e-3) / 1e12, "unit": UNIT, "n_gpus": 1, "steps": K,
+            "warmup": W, "ms_per_step": ms, "higher_is_better": True, "dtype": "s8 x s8 -> s32" if ci8 else "f16 x f16 -> f32",
+            "data": "synthetic",
+            "config": {"workload": "fx_%s: %d stations x %d pol = %d streams x %d spectra of 256 real int8 samples (sigma 20) -> F-engine "
+                                   "(128 complex %s channels) -> X-engine (T = %d, %s kernel)"
+                                   % ("ci8" if ci8 else "f16", N, P, M, A, "int8, scale 1/20" if ci8 else "fp16", A, kernel),
+                       "l2": "every buffer of the chain (%.0f MiB moved) larger than L2" % (nbytes / 2 ** 20),
+                       "gsamples_per_s": s.numel() / (ms * 1e-3) / 1e9,
+                       "ops": {"x_engine_8_per_cmac": ops_x, "f_engine_2.5nlog2n": ops_f}},
+            "gpu_launches": 2 * K,
+            "fengine_ms": ms_f, "xengine_ms": ms_x,
+            "xengine_tops": ops_x / (ms_x * 1e-3) / 1e12,
+            "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s", "frac": gbs / pk["hbm"],
+                         "traffic": None, "kernel": "fengtc::fengine_tc_kernel + xtc::xengine_%s_kernel" % kernel, "kernel_ms": ms,
+                         "algorithmic_bytes_per_launch": nbytes,
+                         "note": "the pair of launches against the HBM roof of the bytes both must move; the X-engine half alone "
+                                 "is tensor-bound at this geometry (xengine_tops)"}}
+
+
 def run_piece(args):
     import torch
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device")
     torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
     K, W = args.steps, max(args.warmup, 3)
-    rec = time_corner_turn(workload(args.workload), peaks(), K, W, args.planes) if args.piece == "corner_turn" else time_fengine(peaks(), K, W, ci8=args.piece == "fengine_ci8")
+    if args.piece == "corner_turn":
+        rec = time_corner_turn(workload(args.workload), peaks(), K, W, args.planes)
+    elif args.piece.startswith("fx_chain"):
+        rec = time_fx_chain(peaks(), K, W, ci8=args.piece == "fx_chain")
+    else:
+        rec = time_fengine(peaks(), K, W, ci8=args.piece == "fengine_ci8")
     print(json.dumps(rec), flush=True)
 
 
@@ -619,6 +684,8 @@ def workload_key(rec, k):
         key = "fengine_ci8" if "int8 (requantised" in w else "fengine_f16"
     elif rec.get("metric") == "corner_turn_gbs":
         key = "corner_turn"
+    elif rec.get("metric") == "fx_chain_tops":
+        key = "fx_ci8" if w.startswith("fx_ci8") else "fx_f16"
     return _cut(key, 16)
 
 
@@ -644,7 +711,7 @@ def compact_headline(full, others):
     cfg, roof, sus, cpu, e2e, clk = (full.get(k) or {} for k in ("config", "roofline", "sustained", "cpu_baseline", "e2e", "clocks"))
     line = {k: _r(full.get(k)) for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better",
                                         "scaling", "vs_baseline", "dtype", "data", "gpu_launches")}
-    line["config"] = {"workload": _cut(cfg.get("workload"), 160), "parallelism": _cut(cfg.get("parallelism"), 80),
+    line["config"] = {"workload": _cut(cfg.get("workload"), 132), "parallelism": _cut(cfg.get("parallelism"), 80),
                       "l2": _cut(cfg.get("l2"), 60)}
     line["clocks"] = {k: _r(clk.get(k)) for k in ("sm_mhz", "sm_max_mhz", "power_w_max", "reasons")} if clk else None
     line["e2e"] = {k: _r(e2e.get(k)) for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "steps", "ms_per_step")} if e2e else None
@@ -665,6 +732,8 @@ def compact_headline(full, others):
                             "sample": _cut(cpu.get("sample"), 72), "threads_1": _r((cpu.get("threads_1") or {}).get("value")),
                             "cpu_model": _cut(cpu.get("cpu_model"), 48)} if cpu else None
     line["workloads"] = workloads_summary(others) if others else None
+    if full.get("check"):
+        line["check"] = {k: full["check"].get(k) for k in ("sharded_equals_unsharded", "words", "ranks_with_work", "sha256")}
     line["full"] = "gpurun_out/bench_full.json"
     for drop in (None, "full", ("cpu_baseline", "sample"), ("config", "l2"), "workloads", ("cpu_baseline", "sample"), ("cpu_baseline", "cpu_model"), ("config", "l2"),
                  ("config", "parallelism"), ("roofline", "traffic_source"), "sustained", ("config", "workload")):
@@ -677,6 +746,40 @@ def compact_headline(full, others):
         if len(text.encode()) < HEADLINE_MAX_BYTES:
             break
     return text
+
+
+def sharded_check(cfg, r, window, rank, world, dist):
+    """--shard channels --check: every rank runs one more step and sends the slabs its window plan wrote to rank 0
+    (a test-only gather of host copies; the data path itself has no collective).  Rank 0 puts them together in channel order
+    and compares them with ONE unsharded launch on the same seeded input: bit for bit (per-channel work is identical
+    whichever plan runs it).  Returns the record for the headline on rank 0, None elsewhere."""
+    import numpy as np
+    import torch
+    from paper_1305_5639_b200 import binding
+    mine = None
+    if r is not None:
+        r.step()
+        torch.cuda.synchronize()
+        c0, n = window
+        mine = (c0, r.out[c0:c0 + n].cpu().numpy())
+    parts = [None] * world if rank == 0 else None
+    dist.gather_object(mine, parts, dst=0)
+    if rank != 0:
+        return None
+    parts = sorted((p for p in parts if p is not None), key=lambda p: p[0])
+    covered = sum(p[1].shape[0] for p in parts)
+    contiguous = all(parts[k][0] + parts[k][1].shape[0] == parts[k + 1][0] for k in range(len(parts) - 1))
+    full = np.concatenate([p[1] for p in parts])
+    with binding.Correlator(cfg["N"], cfg["P"], cfg["C"], cfg["T"], cfg["dtype"]) as h:
+        ref = None
+        for k, x in enumerate(r.xs):
+            ref = h.xengine(x, ref, accumulate=k > 0)
+        torch.cuda.synchronize()
+        ref = ref.cpu().numpy()
+    same = parts[0][0] == 0 and covered == cfg["C"] and contiguous and full.shape == ref.shape and bool(
+        (full.view(np.uint32) == ref.view(np.uint32)).all())
+    return {"sharded_equals_unsharded": same, "words": int(ref.size), "ranks_with_work": len(parts),
+            "windows": [[int(p[0]), int(p[1].shape[0])] for p in parts], "sha256": hashlib.sha256(full.tobytes()).hexdigest()}
 
 
 def emit(full, others):
@@ -722,12 +825,17 @@ def run_native(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the X-engine has no CPU fallback")
+    local = local % torch.cuda.device_count()       # (gloo runs: several ranks on one GPU)
     torch.cuda.set_device(local)
+    red_dev = "cuda" if args.backend == "nccl" else "cpu"           # where the max-over-ranks scalars live
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if args.backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group("gloo")
     binding.lib()                                   # raises if libcorr.so is missing / cannot be built
 
-    cfg = workload(args.workload)
+    cfg = workload(args.workload, args.channels)
     sharded = args.shard == "channels" and world > 1
     window = None
     share = 1.0                                     # this rank's share of the workload's ops / bytes
@@ -774,7 +882,7 @@ def run_native(args):
     barrier()
     w1 = time.time()
     clocks = sampler.stop(w0, w1) if rank == 0 else None
-    total_ms = max_over_ranks(sum(call_ms), dist, world, "cuda")          # device time of exactly K steps, slowest rank
+    total_ms = max_over_ranks(sum(call_ms), dist, world, red_dev)         # device time of exactly K steps, slowest rank
     ops_step = cfg["ops_per_call"] * calls
     if sharded:
         value = whole_job_value(ops_step, K, 1, total_ms) / 1e12          # strong scaling: the job is ONE workload
@@ -799,7 +907,8 @@ def run_native(args):
             except Exception as e:                                    # a failed side run must not lose the headline
                 others.append({"workload": name, "error": repr(e)})
         for fn in (lambda: dumps_run(pk), lambda: time_corner_turn(workload("cfg4"), pk, 10, 3), lambda: time_fengine(pk, 10, 3),
-                   lambda: time_fengine(pk, 10, 3, ci8=True)):
+                   lambda: time_fengine(pk, 10, 3, ci8=True), lambda: time_fx_chain(pk, 10, 3, ci8=True),
+                   lambda: time_fx_chain(pk, 10, 3, ci8=False)):
             try:
                 others.append(fn())
             except Exception as e:
@@ -813,19 +922,21 @@ def run_native(args):
 
     # ---- sustained: the same step back to back for >= 2 s (power-capped clocks), its own clock record -----------
     sustained = None
-    if not args.no_sustained and not idle:
+    if not args.no_sustained:                       # (idle ranks of a sharded run take part in the barriers and the reduction)
         est = max(kernel_ms * calls, 1e-3)
-        Ks = max(K, int(2200.0 / est) + 1)
+        Ks = 0 if idle else max(K, int(2200.0 / est) + 1)
+        if sharded:                                 # one step count for the whole job: the slowest rank's
+            Ks = max(K, int(max_over_ranks(Ks, dist, world, red_dev)))
         s2 = ClockSampler(local)
         if rank == 0:
             s2.start()
             time.sleep(0.1)
         barrier()
         t0 = time.time()
-        ms2 = r.timed(Ks, cold=True)
+        ms2 = [0.0] if idle else r.timed(Ks, cold=True)
         barrier()
         t1 = time.time()
-        tot2 = max_over_ranks(sum(ms2), dist, world, "cuda")
+        tot2 = max_over_ranks(sum(ms2), dist, world, red_dev)
         k_ms = sum(ms2) / len(ms2)
         sustained = {"steps": Ks, "seconds": tot2 * 1e-3, "ms_per_step": tot2 / Ks,
                      "value": whole_job_value(ops_step, Ks, 1 if sharded else world, tot2) / 1e12, "unit": UNIT,
@@ -851,7 +962,7 @@ def run_native(args):
         for _ in range(Ke):
             host_step()                  # blocking: returns after the D2H copy has completed
         barrier()
-        te = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
+        te = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=red_dev)
         if world > 1:
             dist.all_reduce(te, op=dist.ReduceOp.MAX)
         e2e = {"value": world * Ke * ops_step / float(te.item()) / 1e12, "unit": UNIT,
@@ -865,6 +976,8 @@ def run_native(args):
         del xh, oh
     elif not args.no_sha and rank == 0 and r is not None:
         sha = [sha256_tensor(x) for x in r.xs]
+
+    check = sharded_check(cfg, r, window, rank, world, dist) if (args.check and sharded) else None
 
     if rank != 0:
         if world > 1:
@@ -909,7 +1022,11 @@ def run_native(args):
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_call * calls * K,
         "roofline": roofline, "sustained": sustained, "cpu_baseline": cpu,
     }
+    if check is not None:
+        line["check"] = check
     emit(line, others)
+    if check is not None and not check["sharded_equals_unsharded"]:
+        raise SystemExit("--check: the gathered channel windows differ from the unsharded launch")
     if world > 1:
         dist.destroy_process_group()
 
