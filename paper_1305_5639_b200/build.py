@@ -63,6 +63,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
             fd, tmp = tempfile.mkstemp(prefix="libcorr.", suffix=".so.tmp", dir=HERE)
             os.close(fd)
             cmd = [_nvcc()] + NVCC_FLAGS + ["-I", INCLUDE]
+            # developer A/B builds, e.g. CORR_EXTRA_NVCC_FLAGS=-DCORR_FEED_RELEASE_ARRIVE (csrc/ptx.cuh); always with --force
+            cmd += os.environ.get("CORR_EXTRA_NVCC_FLAGS", "").split()
             if verbose:
                 cmd += ["-Xptxas", "-v"]
             cmd += _sources() + ["-o", tmp]

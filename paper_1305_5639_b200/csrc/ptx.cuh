@@ -287,9 +287,20 @@ __device__ __forceinline__ void fence_acq_rel_cluster() { asm volatile("fence.ac
 // assembler cannot know.  (Round 1 used `dep & 0`, which ptxas folds away: the arrive then issued right behind the load
 // and, with 64 KB pipeline stages, a slow epilogue warp now and then read the NEXT round's tile index -- found by
 // tests/test_stress_gpu.py, see profiles/r2_feed_race.md.  A `.release.cluster` arrive is also correct but costs 8 - 20 %.)
+// The register dependency orders instruction ISSUE; the PTX memory model itself promises no load-to-arrive ordering for a
+// relaxed arrive, so this fast path rests on the hardware executing the arrive after its address operand is available --
+// guarded by tests/test_stress_gpu.py and by tests/test_sass_feed_dependency.py, which checks in the built library's SASS
+// that the arrive's address register is still computed from the LDS result (a toolchain that folds it again fails there).
+// -DCORR_FEED_RELEASE_ARRIVE (CORR_EXTRA_NVCC_FLAGS, see build.py) builds the memory-model-clean `.release.cluster` form
+// instead, for A/B runs of the stress tests.
 __device__ __forceinline__ void mbar_arrive_cluster_after(uint32_t cluster_addr, uint32_t dep) {
+#ifdef CORR_FEED_RELEASE_ARRIVE
+    (void)dep;
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+#else
     asm volatile("{\n\t.reg .b32 t;\n\tshr.u32 t, %1, 31;\n\tadd.u32 t, t, %0;\n\t"
                  "mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [t];\n\t}" ::"r"(cluster_addr), "r"(dep) : "memory");
+#endif
 }
 // wait with cluster-scope acquire: the waiter then sees shared-memory data a remote CTA stored before its arrive
 __device__ __forceinline__ bool mbar_try_wait_cluster(uint32_t bar, uint32_t parity) {
