@@ -71,7 +71,7 @@ def parse_args():
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
     ap.add_argument("--kernel", default="auto", choices=["auto", "single", "pair", "simt"],
                     help="force a kernel variant (default: the library's own choice)")
-    ap.add_argument("--piece", default="xengine", choices=["xengine", "corner_turn", "fengine", "fengine_ci8", "fx_chain", "fx_chain_f16"],
+    ap.add_argument("--piece", default="xengine", choices=["xengine", "corner_turn", "fengine", "fengine_ci8", "fx_chain", "fx_chain_f16", "dumps"],
                     help="corner_turn: time the standalone corner-turn kernel (SURVEY 8(a) a1) on the workload's input; "
                          "fengine: time corr_fengine (SURVEY 8(f) rank 2) on 512 streams x 8192 spectra of 256 real int8 samples")
     ap.add_argument("--shard", default="none", choices=["none", "channels"],
@@ -466,7 +466,7 @@ def time_fengine(pk, K, W, M=512, A=8192, ci8=False):
             "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s", "frac": gbs / pk["hbm"],
                          "traffic": (2.094e9 if ci8 else 3.163e9) if (M, A) == (512, 8192) else None,
                          "traffic_source": "profiles/r2b_ncu_final.md (ncu capture)" if (M, A) == (512, 8192) else None,
-                         "kernel": ("fengtc::fengine_tc_kernel<%s>" % ("true" if ci8 else "false"))
+                         "kernel": ("fengtc::fengine_tc_kernel<%s, %s>" % ("true" if ci8 else "false", "true" if M % 64 else "false"))
                          if binding.fengine_uses_tensor_cores(M, out) else "feng::fengine_kernel",
                          "kernel_ms": ms, "algorithmic_bytes_per_launch": nbytes}}
 
@@ -530,6 +530,8 @@ def run_piece(args):
     K, W = args.steps, max(args.warmup, 3)
     if args.piece == "corner_turn":
         rec = time_corner_turn(workload(args.workload), peaks(), K, W, args.planes)
+    elif args.piece == "dumps":
+        rec = dumps_run(peaks(), K, W)
     elif args.piece.startswith("fx_chain"):
         rec = time_fx_chain(peaks(), K, W, ci8=args.piece == "fx_chain")
     else:

@@ -175,7 +175,9 @@ int corr_xengine_dumps(corr_handle h, const void* in, void* out, int n_dump, voi
  *         (stream m = s * n_pol + p) this IS corr_xengine's CORR_CF16 input [n_time = n_spectra][n_chan = 128]
  *         [n_station][n_pol]: no corner turn between the engines.
  * Stateless (no handle), asynchronous on `stream`; CORR_OK or a negative code, message via corr_last_error(NULL).
- * Kernels: with n_stream a multiple of 64 and a 16-byte aligned `out` the transform runs as a dense contraction on the
+ * Kernels: with n_stream a multiple of 8 and at least 32 (whole half tiles of 64 streams plus at most one ragged one whose
+ * padding does not more than double the work: 32, 40, ..., 64, 72, 96, 200, ...) and a 16-byte aligned `out` the transform
+ * runs as a dense contraction on the
  * tcgen05 tensor cores (the real-input DFT folded onto 128 samples, twiddle matrices split into fp16 hi + lo parts,
  * fp32 accumulation: csrc/fengine_tc.cuh); every other geometry runs on the CUDA-core radix-16 x 16 FFT kernel
  * (csrc/fengine.cuh).  Both meet the same bound against the fp64 definition: 0.5 ulp of the fp16 output plus
@@ -195,7 +197,7 @@ int corr_fengine_uses_tensor_cores(int n_stream, const void* out);
  * formed and rounded to an integer by a single fused multiply-add on its fp32 sum S -- while the CUDA-core kernel rounds the
  * fp32 product first and then to an integer; the two can differ by one code only within an fp32 rounding error of a tie).  `scale` > 0 is the
  * caller's requantisation gain (e.g. 1 / (sigma_in * 16) * target sigma); `out` needs 2-byte alignment.  Everything
- * else as corr_fengine, the kernel choice included: a multiple of 64 streams and a 16-byte aligned `out` run on the
+ * else as corr_fengine, the kernel choice included: the same stream counts and a 16-byte aligned `out` run on the
  * tensor cores (the rounding decision is taken on that kernel's fp32 sums), other geometries on the CUDA-core kernel.
  */
 int corr_fengine_ci8(const void* in, void* out, int n_stream, long long n_spectra, float scale, void* stream);

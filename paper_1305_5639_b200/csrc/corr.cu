@@ -169,8 +169,10 @@ FengTcState* fengine_tc_state() {
     void* d_tw = nullptr;
     if (cudaMalloc(&d_tw, tw.size() * sizeof(__half)) != cudaSuccess) { cudaGetLastError(); return nullptr; }
     if (cudaMemcpy(d_tw, tw.data(), tw.size() * sizeof(__half), cudaMemcpyHostToDevice) != cudaSuccess ||
-        cudaFuncSetAttribute(fengtc::fengine_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fengtc::kSmemBytes) != cudaSuccess ||
-        cudaFuncSetAttribute(fengtc::fengine_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fengtc::kSmemBytes) != cudaSuccess) {
+        cudaFuncSetAttribute(fengtc::fengine_tc_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fengtc::kSmemBytes) != cudaSuccess ||
+        cudaFuncSetAttribute(fengtc::fengine_tc_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fengtc::kSmemBytes) != cudaSuccess ||
+        cudaFuncSetAttribute(fengtc::fengine_tc_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fengtc::kSmemBytes) != cudaSuccess ||
+        cudaFuncSetAttribute(fengtc::fengine_tc_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fengtc::kSmemBytes) != cudaSuccess) {
         cudaGetLastError();
         cudaFree(d_tw);
         return nullptr;
@@ -673,9 +675,13 @@ int corr_set_kernel(corr_handle h, int kernel) {
 }
 int corr_last_launch_count(corr_handle h) { return h ? h->last_launches : CORR_EINVAL; }
 
-// tensor-core path (fp16 output and requantised int8 output): whole tiles of 64 streams, 16-byte aligned output rows
+// tensor-core path (fp16 output and requantised int8 output): half tiles of 64 streams, the last one possibly ragged.  Taken
+// when the output rows are 16-byte aligned (n_stream a multiple of 8: rows of n_stream x 2 or 4 bytes) and the padding of the
+// ragged tile at most doubles the tensor work (n_stream >= 32 or a multiple of 64 ... 72 and 96 streams used to drop to the
+// CUDA-core kernel at 0.40 of the HBM roof); below that the CUDA-core kernel wastes less.
 static bool fengine_tc_applies(const void* out, int n_stream) {
-    return n_stream % fengtc::kTileStreams == 0 && (reinterpret_cast<uintptr_t>(out) & 15) == 0;
+    const int padded = (n_stream + fengtc::kTileStreams - 1) / fengtc::kTileStreams * fengtc::kTileStreams;
+    return n_stream % 8 == 0 && padded <= 2 * n_stream && (reinterpret_cast<uintptr_t>(out) & 15) == 0;
 }
 
 static int run_fengine_tc(FengTcState* st, const void* in, void* out, int n_stream, long long n_spectra, bool int8_out, float scale,
@@ -695,11 +701,15 @@ static int run_fengine_tc(FengTcState* st, const void* in, void* out, int n_stre
     prm.tw = static_cast<const uint4*>(st->d_tw);
     prm.n_stream = n_stream;
     prm.n_spectra = n_spectra;
-    prm.n_half = n_spectra * (n_stream / fengtc::kTileStreams);
+    prm.n_half = n_spectra * ((n_stream + fengtc::kTileStreams - 1) / fengtc::kTileStreams);
     prm.n_tiles = (prm.n_half + 1) / 2;
     const long long grid = prm.n_tiles < st->sm_count ? prm.n_tiles : st->sm_count;
-    if (int8_out) fengtc::fengine_tc_kernel<true><<<static_cast<unsigned>(grid), fengtc::kThreads, fengtc::kSmemBytes, stream>>>(map_raw, prm);
-    else fengtc::fengine_tc_kernel<false><<<static_cast<unsigned>(grid), fengtc::kThreads, fengtc::kSmemBytes, stream>>>(map_raw, prm);
+    const unsigned g = static_cast<unsigned>(grid);
+    const bool ragged = n_stream % fengtc::kTileStreams != 0;
+    if (int8_out && ragged) fengtc::fengine_tc_kernel<true, true><<<g, fengtc::kThreads, fengtc::kSmemBytes, stream>>>(map_raw, prm);
+    else if (int8_out) fengtc::fengine_tc_kernel<true, false><<<g, fengtc::kThreads, fengtc::kSmemBytes, stream>>>(map_raw, prm);
+    else if (ragged) fengtc::fengine_tc_kernel<false, true><<<g, fengtc::kThreads, fengtc::kSmemBytes, stream>>>(map_raw, prm);
+    else fengtc::fengine_tc_kernel<false, false><<<g, fengtc::kThreads, fengtc::kSmemBytes, stream>>>(map_raw, prm);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail_cuda(nullptr, e, "fengine_tc_kernel launch");
     return CORR_OK;

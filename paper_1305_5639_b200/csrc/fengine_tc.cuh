@@ -44,7 +44,7 @@ namespace fengtc {
 constexpr int kFft = 256;
 constexpr int kChan = 128;                    // channels kept = MMA N
 constexpr int kFold = 128;                    // folded samples = GEMM K
-constexpr int kTileStreams = 64;              // streams of one half tile (n_stream must be a multiple of it)
+constexpr int kTileStreams = 64;              // streams of one half tile (a ragged last one: TMA zero-fills, stores are predicated)
 constexpr int kFoldWarps = 8, kEpiWarps = 8;
 constexpr int kThreads = 64 + 32 * (kFoldWarps + kEpiWarps);
 constexpr int kRawBytes = kTileStreams * kFft;               // one half tile: 16 KB (two boxes of 64 rows x 128 B)
@@ -72,7 +72,7 @@ struct Params {
     const uint4* tw;         // DEVICE: twiddles [cos_hi | cos_lo | -sin_hi | -sin_lo | nyquist][128 channels][128 samples] fp16
     int n_stream;            // multiple of 64
     long long n_spectra;
-    long long n_half;        // half tiles: n_spectra * n_stream / 64
+    long long n_half;        // half tiles: n_spectra * ceil(n_stream / 64)
     long long n_tiles;       // (n_half + 1) / 2
 };
 
@@ -147,7 +147,10 @@ __device__ __forceinline__ uint32_t raw_unit(uint32_t slot_base, int b, int r, i
     return slot_base + b * (kRawBytes / 2) + r * 128 + ((u ^ (r & 7)) << 4);
 }
 
-template <bool kInt8>
+// kRagged: n_stream is not a multiple of 64 -- the last half tile of every spectrum is partly beyond the tensor map and the
+// epilogue's stores are predicated.  A separate instantiation: the predicates cost the whole-tile kernel 6 % (fp16 output)
+// to 11 % (int8 output, a register spill) when they were compiled in unconditionally.
+template <bool kInt8, bool kRagged>
 __global__ void __launch_bounds__(kThreads, 1)
 fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm) {
     extern __shared__ uint8_t smem_raw[];
@@ -200,7 +203,10 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
     ptx::tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
 
-    const int n_sb = prm.n_stream / kTileStreams;           // half tiles per spectrum: consecutive half tiles share a spectrum
+    // half tiles per spectrum (consecutive half tiles share a spectrum).  The last one may be ragged: the tensor map ends at
+    // n_stream, so TMA zero-fills the rows beyond it (the full box still counts on the barrier), the fold and the MMAs run on
+    // zeros there, and the epilogue stores only streams < n_stream.
+    const int n_sb = (prm.n_stream + kTileStreams - 1) / kTileStreams;
     const long long first = blockIdx.x, step = gridDim.x;
 
     if (warp == 0) {
@@ -351,6 +357,8 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
             const int m0 = static_cast<int>(hidx - a * n_sb) * kTileStreams;
             OutT* dst = out + (a * kChan + 64 * chalf) * prm.n_stream + m0 + r;         // channel 64 chalf of this stream
             OutT* dst_line = out + (a * kChan + 64 * chalf) * prm.n_stream + m0;        // ... of the half tile's first stream
+            const bool row_ok = !kRagged || m0 + r < prm.n_stream;        // this thread's stream exists (ragged last half tile)
+            const bool pair_ok = !kRagged || m0 + 2 * lane < prm.n_stream;    // int8 output: the two streams this lane ships (n_stream is even)
             uint32_t rr[32];                                 // Re of this thread's 64 channels as packed pairs
             ptx::mbar_wait_uniform(re_full, it & 1u);
             ptx::tc_fence_after();
@@ -396,7 +404,8 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
                         for (int k = 0; k < 16; ++k) {
                             const int ch = (quarter & 1) * 16 + k;
                             const uint32_t word = lds_u32(xchg + ch * 128 + lane * 4);
-                            stg_stream(reinterpret_cast<uint32_t*>(dst_line + static_cast<long long>(32 * part + ch) * prm.n_stream) + lane, word, policy);
+                            if (pair_ok)
+                                stg_stream(reinterpret_cast<uint32_t*>(dst_line + static_cast<long long>(32 * part + ch) * prm.n_stream) + lane, word, policy);
                         }
                         pair_sync(1 + pair_id);              // the buffer may be overwritten
                     } else {
@@ -408,8 +417,10 @@ fengine_tc_kernel(const __grid_constant__ CUtensorMap tmap_raw, const Params prm
                             // (re, im) half2 words of channels 2c and 2c + 1: one 128-byte line per channel and warp
                             // (lane pairs trading words for 8-byte stores of two lines per instruction: no gain, the
                             // write path is bound by lines, not by instructions)
-                            stg_stream(d0, __byte_perm(re2, ii, 0x5410), policy);
-                            stg_stream(d0 + prm.n_stream, __byte_perm(re2, ii, 0x7632), policy);
+                            if (row_ok) {
+                                stg_stream(d0, __byte_perm(re2, ii, 0x5410), policy);
+                                stg_stream(d0 + prm.n_stream, __byte_perm(re2, ii, 0x7632), policy);
+                            }
                         }
                     }
                 }

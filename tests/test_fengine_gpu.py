@@ -35,18 +35,21 @@ def check(corr, s, simt=False):
         assert bad.size == 0, "part %d first mismatches (a,k,m): %s" % (part, bad[:6].tolist())
 
 
-@pytest.mark.parametrize("M,A", [(1, 1), (2, 3), (7, 2), (32, 4), (33, 5), (64, 16), (100, 9), (512, 8)])
+@pytest.mark.parametrize("M,A", [(1, 1), (2, 3), (7, 2), (24, 3), (32, 4), (33, 5), (64, 16), (100, 9), (512, 8)])
 def test_fengine_random_full_range(corr, M, A):
     rng = np.random.default_rng(9000 + M)
     s = rng.integers(-128, 128, size=(M, A * 256), dtype=np.int8)
-    assert corr.fengine_uses_tensor_cores(M) == (M % 64 == 0)
+    # tensor cores: rows 16-byte aligned (M % 8 == 0) and a ragged last half tile that at most doubles the work
+    assert corr.fengine_uses_tensor_cores(M) == (M % 8 == 0 and -(-M // 64) * 64 <= 2 * M)
     check(corr, s)
     check(corr, s, simt=True)                            # the CUDA-core kernel on the same input
 
 
-@pytest.mark.parametrize("M,A", [(64, 1), (64, 149), (128, 33), (192, 7), (320, 2), (512, 300), (1024, 37)])
+@pytest.mark.parametrize("M,A", [(64, 1), (64, 149), (128, 33), (192, 7), (320, 2), (512, 300), (1024, 37),
+                                 (32, 5), (40, 7), (72, 149), (96, 33), (200, 3), (456, 21)])
 def test_fengine_tensor_core_path(corr, M, A):
-    """The tcgen05 kernel (stream counts that are multiples of 64): more tiles than SMs, a single tile, odd tile counts;
+    """The tcgen05 kernel (whole half tiles of 64 streams, and stream counts with a RAGGED last half tile -- 72 and 96 used to
+    fall back to the CUDA-core kernel): more tiles than SMs, a single tile, odd tile counts;
     full-range int8 including -128; the same bound as the CUDA-core kernel, and the two kernels agree to one fp16 ulp
     plus both fp32 round-off allowances."""
     rng = np.random.default_rng(9100 + M + A)
@@ -137,9 +140,10 @@ def test_fengine_argument_errors(corr):
 # ---- requantised int8 output (corr_fengine_ci8): the code is decided by rint of an fp32 product on the GPU and of an
 # fp64 product in the oracle, so the two must agree EXACTLY except where the scaled value lies within the fp32 round-off
 # bound of a rounding tie, and there they may differ by one code (quantised decisions) ----
-# (stream counts that are a multiple of 64 run on the tensor-core kernel, the others on the CUDA-core kernel)
+# (stream counts that are a multiple of 8, at least 32, run on the tensor-core kernel, the others on the CUDA-core kernel)
 @pytest.mark.parametrize("M,A,scale", [(2, 3, 1.0 / 64), (33, 4, 1.0 / 40), (64, 8, 0.05), (100, 5, 1.0 / 300),
-                                       (128, 33, 1.0 / 40), (192, 7, 1.0 / 25), (512, 40, 1.0 / 64)])
+                                       (128, 33, 1.0 / 40), (192, 7, 1.0 / 25), (512, 40, 1.0 / 64),
+                                       (40, 9, 1.0 / 40), (72, 150, 1.0 / 30), (96, 33, 0.05), (200, 7, 1.0 / 64)])
 def test_fengine_ci8_codes(corr, M, A, scale):
     from oracle import fengine as fo
     rng = np.random.default_rng(9100 + M)
