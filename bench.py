@@ -51,13 +51,17 @@ FALLBACK_HBM_GBS = 6650.0
 # committed `ncu --set full` captures of the SAME kernel and geometry -- not measured by this run, and emitted only when
 # the kernel that ran is the one that was captured: workload -> (kernel, bytes, capture file)
 NCU_TRAFFIC = {
-    "cfg4": ("pair", (3.198e9 + 3 * 4.275e9) / 4, "profiles/r2b_ncu_final.md"),     # accumulate = 0 once, = 1 three times
-    "cfg3": ("pair", 4.756e9, "profiles/r2b_ncu_final.md"),
-    "cfg2": ("pair", 0.3152e9, "profiles/r2b_ncu_final.md"),
-    "cfg5_n128": ("pair", 1.325e9, "profiles/r2b_ncu_final.md"),
-    "cfg5_n1024": ("pair", 3.168e9, "profiles/r2b_ncu_final.md"),
-    "cross_n256": ("pair", 3.190e9, "profiles/r2b_ncu_final.md"),
-}      # (no row = no capture of the shipped kernel at that geometry: `traffic` is null there)
+    "cfg4": ("pair", (3.1978e9 + 3 * 4.2746e9) / 4, "profiles/r3_ncu_final.md"),     # accumulate = 0 once, = 1 three times
+    "cfg3": ("pair", 4.7305e9, "profiles/r3_ncu_final.md"),
+    "cfg2": ("pair", 0.3158e9, "profiles/r3_ncu_final.md"),
+    "cfg5_n32": ("single", 1.1387e9, "profiles/r3_ncu_final.md"),
+    "cfg5_n64": ("pair", 1.1988e9, "profiles/r3_ncu_final.md"),
+    "cfg5_n128": ("pair", 1.3251e9, "profiles/r3_ncu_final.md"),
+    "cfg5_n256": ("pair", 1.5835e9, "profiles/r3_ncu_final.md"),
+    "cfg5_n512": ("pair", 2.1053e9, "profiles/r3_ncu_final.md"),
+    "cfg5_n1024": ("pair", 3.1701e9, "profiles/r3_ncu_final.md"),
+    "cross_n256": ("pair", 3.1890e9, "profiles/r3_ncu_final.md"),
+}      # every row: the shipped kernel at that geometry, captured at the end of round 3
 KERNEL_NAMES = {"single": "xtc::xengine_direct_kernel<%d>", "pair": "xtc::xengine_pair_kernel<%d>",
                 "simt": "xsimt::xengine_simt_kernel<%d>"}
 
@@ -432,8 +436,8 @@ def time_corner_turn(cfg, pk, K, W, planes=1):
                        "l2": "input + workspace (%.0f MiB) larger than L2" % (nbytes / 2 ** 20)},
             "gpu_launches": K,
             "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s", "frac": gbs / pk["hbm"],
-                         "traffic": 4.246e9 if (cfg["name"] == "cfg4" and planes == 1) else None,
-                         "traffic_source": "profiles/r2_ncu_final.md (ncu capture)" if (cfg["name"] == "cfg4" and planes == 1) else None,
+                         "traffic": 4.2471e9 if (cfg["name"] == "cfg4" and planes == 1) else None,
+                         "traffic_source": "profiles/r3_ncu_final.md (ncu capture)" if (cfg["name"] == "cfg4" and planes == 1) else None,
                          "kernel": "cturn::corner_turn_kernel", "kernel_ms": ms,
                          "algorithmic_bytes_per_launch": nbytes}}
 
@@ -464,8 +468,8 @@ def time_fengine(pk, K, W, M=512, A=8192, ci8=False):
                        "gsamples_per_s": s.numel() / (ms * 1e-3) / 1e9},
             "gpu_launches": K,
             "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s", "frac": gbs / pk["hbm"],
-                         "traffic": (2.094e9 if ci8 else 3.163e9) if (M, A) == (512, 8192) else None,
-                         "traffic_source": "profiles/r2b_ncu_final.md (ncu capture)" if (M, A) == (512, 8192) else None,
+                         "traffic": (2.0917e9 if ci8 else 3.1619e9) if (M, A) == (512, 8192) else None,
+                         "traffic_source": "profiles/r3_ncu_final.md (ncu capture)" if (M, A) == (512, 8192) else None,
                          "kernel": ("fengtc::fengine_tc_kernel<%s, %s>" % ("true" if ci8 else "false", "true" if M % 64 else "false"))
                          if binding.fengine_uses_tensor_cores(M, out) else "feng::fengine_kernel",
                          "kernel_ms": ms, "algorithmic_bytes_per_launch": nbytes}}
@@ -658,7 +662,9 @@ def dumps_run(pk, K=10, W=3):
     return {"workload": "dumps: N=%d, %d pol, %d channels, T=%d cut into %d integrations of %d samples, int8" % (N, P, C, T, nd, T // nd),
             "ms_per_call": ms, "value": ops / (ms * 1e-3) / 1e12, "unit": UNIT,
             "hbm": {"algorithmic_bytes_per_launch": nbytes, "achieved_gbs": nbytes / (ms * 1e-3) / 1e9,
-                    "frac": nbytes / (ms * 1e-3) / 1e9 / pk["hbm"]}}
+                    "frac": nbytes / (ms * 1e-3) / 1e9 / pk["hbm"],
+                    "traffic": 4.7919e9 if (N, P, C, T, nd) == (256, 2, 256, 2048, 16) else None,
+                    "traffic_source": "profiles/r3_ncu_final.md (ncu capture)"}}
 
 
 # ------------------------------------------------------------------------------------------------
